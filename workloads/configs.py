@@ -1,0 +1,305 @@
+"""The BASELINE.json workloads as seeded *inputs* (structure + values).
+
+A workload is: two sector lists (enlarged left block A, enlarged right block B),
+a target charge, a list of stored operators (each a set of blocks (q+dq, q) on
+one half with an RNG stream for its values) and a list of operator-pair terms
+(L index, R index, coefficient, transpose flags).  What the terms *mean* — the
+product, the fermionic sign, the accumulation — is the method and lives in
+``oracle/`` and in the CUDA library, separately.
+
+Sources: BASELINE.json configs; SURVEY.md §8.0 (term families F0-F4 and their
+counts, which follow from PAPER.md Eq. (1), line 58), §8(c) readings r14-r18,
+§8(d) concrete inputs.  The paper's own operator values (converged DMRG
+environments in its optimised bases) are not available, so the *structure* is
+the lattice's and the *values* are synthetic (r17).
+"""
+from dataclasses import dataclass, field
+from itertools import product
+import math
+import numpy as np
+
+from .rng import normal12, uniform_u64
+from .sectors import gaussian_sectors, binom
+
+PSI_STREAM = 7
+COEF_STREAM = 9
+SHIFT_STREAM = 11
+OP_STREAM0 = 16
+
+
+def op_stream_id(op_index):
+    return OP_STREAM0 + op_index
+
+
+@dataclass
+class OpSpec:
+    half: str            # "A" or "B"
+    dq: tuple            # charge shift: blocks (row sector q+dq, column sector q)
+    parity: int          # 0 even, 1 odd (fermionic)
+    symmetric: bool = False   # dq == 0 and every diagonal block symmetrised
+    scale_mode: str = "rsqrt_cols"   # "one" (config 2) or "rsqrt_cols" (configs 3-5)
+    tag: str = ""
+
+
+@dataclass
+class TermSpec:
+    L: object            # index into ops, or None for the identity on A
+    R: object            # index into ops, or None for the identity on B
+    coef: float
+    trans_L: bool = False
+    trans_R: bool = False
+    family: str = ""
+
+
+@dataclass
+class Workload:
+    name: str
+    seed: int
+    n_charges: int
+    sectors_A: list      # [(charge tuple, dim)]
+    sectors_B: list
+    target: tuple
+    ops: list = field(default_factory=list)
+    terms: list = field(default_factory=list)
+    hermitian: bool = False
+
+    @property
+    def M_A(self):
+        return sum(d for _, d in self.sectors_A)
+
+    @property
+    def M_B(self):
+        return sum(d for _, d in self.sectors_B)
+
+    def sectors(self, half):
+        return self.sectors_A if half == "A" else self.sectors_B
+
+
+# ----------------------------------------------------------------------------
+# block tables (pure index bookkeeping; the library recomputes its own)
+# ----------------------------------------------------------------------------
+def _add(q, dq):
+    return tuple(a + b for a, b in zip(q, dq))
+
+
+def op_block_table(sectors, dq):
+    """Blocks of an operator with shift dq: [(row_idx, col_idx, rows, cols, offset)].
+
+    One block for every column sector q (in sector order) such that q+dq is also
+    a sector; offsets count *unpadded* elements, block after block.
+    """
+    index = {q: i for i, (q, _) in enumerate(sectors)}
+    out, off = [], 0
+    for ci, (q, cols) in enumerate(sectors):
+        r = index.get(_add(q, dq))
+        if r is None or cols == 0 or sectors[r][1] == 0:
+            continue
+        rows = sectors[r][1]
+        out.append((r, ci, rows, cols, off))
+        off += rows * cols
+    return out
+
+
+def psi_block_table(sectors_A, sectors_B, target):
+    """ψ blocks (qA, qB) with qA+qB = target, in A-sector order."""
+    index_B = {q: i for i, (q, _) in enumerate(sectors_B)}
+    out, off = [], 0
+    for ai, (qa, rows) in enumerate(sectors_A):
+        qb = tuple(t - a for t, a in zip(target, qa))
+        bi = index_B.get(qb)
+        if bi is None or rows == 0 or sectors_B[bi][1] == 0:
+            continue
+        cols = sectors_B[bi][1]
+        out.append((ai, bi, rows, cols, off))
+        off += rows * cols
+    return out
+
+
+# ----------------------------------------------------------------------------
+# values
+# ----------------------------------------------------------------------------
+def _block_scale(spec, cols):
+    return 1.0 if spec.scale_mode == "one" else 1.0 / math.sqrt(cols)
+
+
+def fill_op_host(wl, op_index, only_blocks=None):
+    """Blocks of stored operator ``op_index`` as {(row_idx, col_idx): ndarray}.
+
+    value(r, c) = scale * g(off + r*cols + c), g = normal12 of the operator's
+    stream; for a ``symmetric`` operator a (square, diagonal-sector) block is
+    0.5*(g(r,c) + g(c,r)) * scale.  ``only_blocks`` restricts to a set of
+    (row_idx, col_idx) keys (used to regenerate sampled blocks at full size).
+    """
+    spec = wl.ops[op_index]
+    sectors = wl.sectors(spec.half)
+    stream = op_stream_id(op_index)
+    out = {}
+    for (ri, ci, rows, cols, off) in op_block_table(sectors, spec.dq):
+        if only_blocks is not None and (ri, ci) not in only_blocks:
+            continue
+        idx = off + np.arange(rows * cols, dtype=np.uint64).reshape(rows, cols)
+        g = normal12(wl.seed, stream, idx)
+        if spec.symmetric:
+            assert ri == ci and rows == cols
+            g = (g + g.T) * 0.5
+        out[(ri, ci)] = g * _block_scale(spec, cols)
+    return out
+
+
+def fill_psi_host(wl, stream=PSI_STREAM):
+    """ψ blocks {(a_idx, b_idx): ndarray} with N(0,1)-like entries (normal12)."""
+    out = {}
+    for (ai, bi, rows, cols, off) in psi_block_table(wl.sectors_A, wl.sectors_B, wl.target):
+        idx = off + np.arange(rows * cols, dtype=np.uint64).reshape(rows, cols)
+        out[(ai, bi)] = normal12(wl.seed, stream, idx)
+    return out
+
+
+# ----------------------------------------------------------------------------
+# config 2: synthetic block-sparse matvec (BASELINE.json configs[1]; r14, r15)
+# ----------------------------------------------------------------------------
+def synthetic_config2(M=1024, n_q=33, K=512, seed=2, width2=32.0, name=None):
+    """U(1) charge, sectors q=0..n_q-1 ∝ exp(-(q-c)²/width2) with c=(n_q-1)/2,
+    ψ blocks where qA+qB = n_q-1, K pairs with δ_L uniform in {-2..2},
+    δ_R = -δ_L, parity δ_L mod 2, entries and c_k N(0,1).  Not symmetric."""
+    c = (n_q - 1) / 2.0
+    w = [math.exp(-((q - c) ** 2) / width2) for q in range(n_q)]
+    caps = [binom(n_q - 1, q) for q in range(n_q)]
+    dims = gaussian_sectors(M, w, caps)
+    sectors = [((q,), d) for q, d in enumerate(dims)]
+    wl = Workload(name or f"config2_M{M}_K{K}", seed, 1, sectors, list(sectors), (n_q - 1,))
+    shifts = (uniform_u64(seed, SHIFT_STREAM, np.arange(K)) % np.uint64(5)).astype(np.int64) - 2
+    coefs = normal12(seed, COEF_STREAM, np.arange(K))
+    for k in range(K):
+        d = int(shifts[k])
+        wl.ops.append(OpSpec("A", (d,), d & 1, False, "one", f"L{k}"))
+        wl.ops.append(OpSpec("B", (-d,), d & 1, False, "one", f"R{k}"))
+        wl.terms.append(TermSpec(2 * k, 2 * k + 1, float(coefs[k]), False, False, "syn"))
+    return wl
+
+
+# ----------------------------------------------------------------------------
+# configs 3-5: lattice-shaped operator-pair lists (SURVEY §8.0 families)
+# ----------------------------------------------------------------------------
+def _family_builder(wl, mode_shifts_A, mode_shifts_B, pair_fraction=None, keep=None):
+    """Append ops and terms of families F0-F4 for modes with the given charge
+    shifts (one tuple per mode = the shift of its creation operator).
+
+    Hermitian construction (r18): every δ≠0 (or p≠s) pair is stored once and its
+    h.c. partner re-uses the same stored blocks through the transpose flags,
+    with coefficient −c for fermionic (odd) pairs and +c for even ones; the
+    self-adjoint operators (H_A, H_B, c†_p c_p and its complement) have
+    symmetrised blocks.  ``keep(family, ordinal)`` may thin the list (used for
+    scaled-down copies and for the executed subset of config 5).
+    """
+    zero = tuple(0 for _ in wl.target)
+    neg = lambda d: tuple(-x for x in d)
+    add = lambda a, b: tuple(x + y for x, y in zip(a, b))
+    keep = keep or (lambda fam, i: True)
+
+    def new_op(half, dq, parity, sym, tag):
+        wl.ops.append(OpSpec(half, tuple(dq), parity, sym, "rsqrt_cols", tag))
+        return len(wl.ops) - 1
+
+    def pair(Lop, Rop, coef, fam, partner_coef=None):
+        wl.terms.append(TermSpec(Lop, Rop, coef, False, False, fam))
+        if partner_coef is not None:
+            wl.terms.append(TermSpec(Lop, Rop, partner_coef, True, True, fam + "^hc"))
+
+    # F0: H_A ⊗ 1 and 1 ⊗ H_B
+    hA = new_op("A", zero, 0, True, "H_A")
+    hB = new_op("B", zero, 0, True, "H_B")
+    wl.terms.append(TermSpec(hA, None, 1.0, False, False, "F0"))
+    wl.terms.append(TermSpec(None, hB, 1.0, False, False, "F0"))
+    # F1: for p in B:  −S^A_p ⊗ c†_p  and  +S^A_p† ⊗ c_p
+    for i, s in enumerate(mode_shifts_B):
+        if not keep("F1", i):
+            continue
+        Lop = new_op("A", neg(s), 1, False, f"S^A_{i}")
+        Rop = new_op("B", s, 1, False, f"c†_B{i}")
+        pair(Lop, Rop, -1.0, "F1", +1.0)
+    # F2: for p in A:  +c†_p ⊗ S^B_p  and  −c_p ⊗ S^B_p†
+    cdag_A = {}
+    for i, s in enumerate(mode_shifts_A):
+        if not keep("F2", i):
+            continue
+        Lop = new_op("A", s, 1, False, f"c†_A{i}")
+        Rop = new_op("B", neg(s), 1, False, f"S^B_{i}")
+        cdag_A[i] = Lop
+        pair(Lop, Rop, +1.0, "F2", -1.0)
+    # F3: for p<q in A:  c†_p c†_q ⊗ P^B_pq  and h.c. (even, +1/+1)
+    nA = len(mode_shifts_A)
+    o = 0
+    for p in range(nA):
+        for q in range(p + 1, nA):
+            o += 1
+            if not keep("F3", o - 1):
+                continue
+            d = add(mode_shifts_A[p], mode_shifts_A[q])
+            Lop = new_op("A", d, 0, False, f"c†c†_{p},{q}")
+            Rop = new_op("B", neg(d), 0, False, f"P^B_{p},{q}")
+            pair(Lop, Rop, +1.0, "F3", +1.0)
+    # F4: for p,s in A:  c†_p c_s ⊗ Q^B_ps ; (s,p) is the h.c. of (p,s)
+    o = 0
+    for p in range(nA):
+        for s in range(p, nA):
+            o += 1
+            if not keep("F4", o - 1):
+                continue
+            d = add(mode_shifts_A[p], neg(mode_shifts_A[s]))
+            if p == s:
+                Lop = new_op("A", zero, 0, True, f"n_{p}")
+                Rop = new_op("B", zero, 0, True, f"Q^B_{p},{p}")
+                pair(Lop, Rop, +1.0, "F4")
+            else:
+                Lop = new_op("A", d, 0, False, f"c†c_{p},{s}")
+                Rop = new_op("B", neg(d), 0, False, f"Q^B_{p},{s}")
+                pair(Lop, Rop, +1.0, "F4", +1.0)
+    wl.hermitian = True
+    return wl
+
+
+def spinless_term_structure(n_A, n_B):
+    """(mode shifts of A, mode shifts of B) for spinless fermions: one U(1)."""
+    return [(1,)] * n_A, [(1,)] * n_B
+
+
+def hubbard_term_structure(n_orb_A, n_orb_B):
+    """Spin-orbital order (site ↑, site ↓, ...) — reading r8; charges (n↑, n↓)."""
+    return [(1, 0), (0, 1)] * n_orb_A, [(1, 0), (0, 1)] * n_orb_B
+
+
+def lattice_workload(kind, n_half, M, seed, name=None, width2=None, keep=None):
+    """Configs 3-5 and their scaled-down copies.
+
+    kind = "spinless": n_half modes per half, sectors q=0..n_half,
+           w_q = exp(-(q-n_half/2)²/width2), width2 default n_half (σ² = n_half/2:
+           32 for the 8×8 half, 72 for the 12×12 half), caps C(n_half, q),
+           target N = n_half (half filling of 2·n_half modes).
+    kind = "hubbard":  n_half spatial orbitals per half, sectors (n↑,n↓) in
+           [0,n_half]², w = exp(-((n↑-c)²+(n↓-c)²)/width2), c = n_half/2,
+           width2 default 8·n_half/18 (8 for the 6×6 half), caps
+           C(n_half,n↑)·C(n_half,n↓), target (n_half, n_half).
+    """
+    if kind == "spinless":
+        width2 = float(n_half) if width2 is None else width2
+        c = n_half / 2.0
+        qs = [(q,) for q in range(n_half + 1)]
+        w = [math.exp(-((q[0] - c) ** 2) / width2) for q in qs]
+        caps = [binom(n_half, q[0]) for q in qs]
+        target = (n_half,)
+        shifts = spinless_term_structure(n_half, n_half)
+    elif kind == "hubbard":
+        width2 = 8.0 * n_half / 18.0 if width2 is None else width2
+        c = n_half / 2.0
+        qs = [(u, d) for u in range(n_half + 1) for d in range(n_half + 1)]
+        w = [math.exp(-(((u - c) ** 2) + ((d - c) ** 2)) / width2) for u, d in qs]
+        caps = [binom(n_half, u) * binom(n_half, d) for u, d in qs]
+        target = (n_half, n_half)
+        shifts = hubbard_term_structure(n_half, n_half)
+    else:
+        raise ValueError(kind)
+    dims = gaussian_sectors(M, w, caps)
+    sectors = [(q, d) for q, d in zip(qs, dims)]
+    wl = Workload(name or f"{kind}_n{n_half}_M{M}", seed, len(target), sectors, list(sectors), target)
+    return _family_builder(wl, shifts[0], shifts[1], keep=keep)
