@@ -1,0 +1,232 @@
+/* dmrgk.h — C ABI of the B200-native H_eff·ψ / Davidson hot path of arXiv 2311.14106.
+ *
+ * What the library computes (§II.A: "iterative diagonalization of the effective
+ * Hamiltonian built from renormalized block operators"; BASELINE.json north_star):
+ *
+ *     σ = Σ_k c_k (L_k ⊗ R_k) ψ ,   per block:
+ *     σ[qA+δ_k, qB−δ_k] += c_k · (−1)^{π_k·N(qA)} · L_k[qA+δ_k, qA] · ψ[qA, qB] · R_k[qB−δ_k, qB]ᵀ
+ *
+ * ψ is the two-site wavefunction as a block-sparse matrix ψ[a, b] over the U(1) (or U(1)×U(1))
+ * sectors of the enlarged left block A and the enlarged right block B, with blocks only where
+ * q_A + q_B = target.  π_k is the fermion parity of pair k; N(q) is the particle number of the
+ * INPUT A sector (sum of the charge components).  Everything is FP64.
+ *
+ * Conventions
+ *  - Every function returns 0 (DMRGK_OK) or a negative dmrgk_status.  Nothing throws or aborts across
+ *    the ABI.  dmrgk_last_error() returns a thread-local message for the last failure.
+ *  - Handles are opaque; *_create writes the handle to *out; *_destroy(NULL) is a no-op.
+ *  - OWNERSHIP: the caller owns every large buffer (operator arenas, ψ, σ, Davidson basis, workspace,
+ *    pinned host arenas).  The library borrows raw pointers; buffers must stay alive until the stream
+ *    work using them has completed.  The library owns only its metadata.  "dev" = device pointer,
+ *    "host" = host pointer; every device pointer must be 128-byte aligned (DMRGK_EALIGN otherwise).
+ *  - Streams are cudaStream_t passed as void* (NULL = legacy default stream).
+ *  - ASYNCHRONY: heff_apply, heff_diag and the vec_* calls enqueue work and return; the
+ *    davidson_* calls and *_host calls synchronise the stream (they read scalars back).
+ *  - LAYOUT: a block (rows × cols) is row-major with leading dimension ld = round_up(cols, 16)
+ *    doubles; the padding columns must be zero (pack/fill write zeros; every kernel of the library
+ *    preserves zeros there).  A block-sparse object is one packed arena plus a block table; block
+ *    offsets (in doubles) are multiples of 16.  ψ, σ, diag(H_eff) and all Davidson vectors share the
+ *    layout of dmrgk_layout, so vector kernels run over the flat padded arena.
+ *    The "unpadded" form used by pack/unpack and by the seeded fill is: block after block in table
+ *    order, each block rows×cols row-major with no padding.
+ */
+#ifndef DMRGK_H
+#define DMRGK_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum dmrgk_status {
+    DMRGK_OK = 0,
+    DMRGK_EINVAL = -1,   /* NULL pointer, negative size, bad flag                       */
+    DMRGK_ESHAPE = -2,   /* operator space is not the layout's, sizes disagree           */
+    DMRGK_ECHARGE = -3,  /* charge shifts of a pair do not cancel / parity mismatch      */
+    DMRGK_EALIGN = -4,   /* device pointer not 128-byte aligned                          */
+    DMRGK_ENOMEM = -5,   /* host or device allocation of library metadata failed         */
+    DMRGK_ECUDA = -6,    /* a CUDA runtime call failed (message holds the CUDA error)    */
+    DMRGK_ENOTCONV = -7, /* davidson_solve hit max_iter                                  */
+    DMRGK_ESTATE = -8    /* call out of order (unbound operator, solver not started)     */
+} dmrgk_status;
+
+typedef struct dmrgk_ctx dmrgk_ctx;
+typedef struct dmrgk_space dmrgk_space;
+typedef struct dmrgk_layout dmrgk_layout;
+typedef struct dmrgk_op dmrgk_op;
+typedef struct dmrgk_heff dmrgk_heff;
+typedef struct dmrgk_davidson dmrgk_davidson;
+
+const char* dmrgk_last_error(void);
+/* Library version string, e.g. "dmrgk 0.1 sm_100a". */
+const char* dmrgk_version(void);
+
+/* ---- context ------------------------------------------------------------------------------ */
+/* Binds the library to CUDA device `device` (cudaSetDevice on every call that launches work).
+ * Fails with DMRGK_ECUDA when no device is present: there is no CPU fallback. */
+int32_t dmrgk_ctx_create(int32_t device, dmrgk_ctx** out);
+void dmrgk_ctx_destroy(dmrgk_ctx* ctx);
+/* Number of SMs and bytes of L2 of the bound device. */
+int32_t dmrgk_ctx_query(const dmrgk_ctx* ctx, int32_t* n_sm, int64_t* l2_bytes, int64_t* hbm_bytes);
+
+/* ---- a1: sector index / block layout ("Tables") ------------- */
+/* One space per half (A, B).  charges is [n_sectors][n_charges] (n_charges 1 or 2), dims[i] ≥ 0
+ * (dim 0 = empty sector, skipped everywhere).  Charge tuples must be distinct. */
+int32_t dmrgk_space_create(dmrgk_ctx* ctx, int32_t n_charges, int32_t n_sectors,
+                           const int32_t* charges, const int32_t* dims, dmrgk_space** out);
+void dmrgk_space_destroy(dmrgk_space* s);
+
+/* ψ layout: one block (a, b) for every A sector a (in A order) whose partner charge
+ * target − q_a is a B sector, both dims > 0.  A layout with no block is valid (n_blocks = 0). */
+int32_t dmrgk_layout_create(dmrgk_ctx* ctx, const dmrgk_space* A, const dmrgk_space* B,
+                            const int32_t* target, dmrgk_layout** out);
+void dmrgk_layout_destroy(dmrgk_layout* l);
+/* n_elems = Σ rows·cols (unpadded), n_padded = doubles of the packed arena (multiple of 16). */
+int32_t dmrgk_layout_query(const dmrgk_layout* l, int64_t* n_blocks, int64_t* n_elems,
+                           int64_t* n_padded);
+/* Block table; each output array has n_blocks entries (any may be NULL).  offset is in doubles
+ * into the packed arena. */
+int32_t dmrgk_layout_blocks(const dmrgk_layout* l, int32_t* a_idx, int32_t* b_idx, int32_t* rows,
+                            int32_t* cols, int32_t* ld, int64_t* offset);
+/* Host-side test aids: unpadded ↔ packed (host pointers; pack zero-fills the padding). */
+int32_t dmrgk_layout_pack(const dmrgk_layout* l, const double* unpadded_host, double* packed_host);
+int32_t dmrgk_layout_unpack(const dmrgk_layout* l, const double* packed_host, double* unpadded_host);
+
+/* A stored operator on one half with charge shift dq: one block (q+dq, q) for every column sector
+ * q (in sector order) such that q+dq is a sector and both dims > 0.  parity: 0 even, 1 odd. */
+int32_t dmrgk_op_create(dmrgk_ctx* ctx, const dmrgk_space* space, const int32_t* dq, int32_t parity,
+                        dmrgk_op** out);
+void dmrgk_op_destroy(dmrgk_op* op);
+int32_t dmrgk_op_query(const dmrgk_op* op, int64_t* n_blocks, int64_t* n_elems, int64_t* n_padded);
+int32_t dmrgk_op_blocks(const dmrgk_op* op, int32_t* row_idx, int32_t* col_idx, int32_t* rows,
+                        int32_t* cols, int32_t* ld, int64_t* offset);
+int32_t dmrgk_op_pack(const dmrgk_op* op, const double* unpadded_host, double* packed_host);
+/* Resident operator: packed arena in device memory (n_padded doubles, 128-B aligned). */
+int32_t dmrgk_op_bind_device(dmrgk_op* op, const double* arena_dev);
+/* Staged operator ("H2D IO"): packed arena in PINNED host memory;
+ * heff_apply copies it through the staging ring on the copy stream each time it is needed. */
+int32_t dmrgk_op_bind_pinned(dmrgk_op* op, const double* arena_pinned_host);
+
+/* ---- a2: operator-pair task list ---------------------------------------- */
+enum {
+    DMRGK_TRANS_L = 1u, /* apply the transpose of the stored L operator (h.c. partner)  */
+    DMRGK_TRANS_R = 2u, /* apply the transpose of the stored R operator                 */
+    DMRGK_IDENT_L = 4u, /* L is the identity on A (L[k] must be NULL)                   */
+    DMRGK_IDENT_R = 8u  /* R is the identity on B (R[k] must be NULL)                   */
+};
+
+typedef struct dmrgk_heff_opts {
+    int64_t t_chunk_bytes;  /* cap on the L_k·ψ intermediate workspace per chunk of pairs
+                               (0 = default 4 GiB); pairs are processed chunk by chunk       */
+    int64_t ring_bytes;     /* staging ring for pinned operators, split in two halves
+                               (0 = no ring: binding a pinned operator is then an error)     */
+    int32_t kernel;         /* 0 = DMMA tensor-core kernel (product path),
+                               1 = scalar check kernel (same task lists; debugging aid)     */
+    int32_t split_waves;    /* phase-2 split-k target: units per CTA slot (0 = default 8)   */
+    int32_t reserved[4];
+} dmrgk_heff_opts;
+
+/* Builds the task list of σ = Σ_k coef[k] (L[k] ⊗ R[k]) ψ for the given layout: enumerates
+ * (k, input block) pairs whose L and R blocks exist and whose output block is in the layout, folds
+ * coef[k]·(−1)^{π_k N(q_A)} into one scalar per task, groups tasks by OUTPUT block (accumulation
+ * needs no atomics), tiles, plans split-k, cuts the pair list into chunks, uploads the metadata.
+ * Every operator must already be bound.  K = 0 is valid (σ = 0).
+ * Errors: DMRGK_ESHAPE (operator space ≠ layout's), DMRGK_ECHARGE (applied shifts do not cancel, or
+ * parities differ), DMRGK_ESTATE (unbound operator; pinned operator without ring), DMRGK_EINVAL. */
+int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
+                          dmrgk_op* const* L, dmrgk_op* const* R, const double* coef,
+                          const uint32_t* flags, const dmrgk_heff_opts* opts, dmrgk_heff** out);
+void dmrgk_heff_destroy(dmrgk_heff* h);
+/* flops_alg = Σ_tasks min(2m′n(m+n′), 2mn′(n+m′)) (identity factor → one product),
+ * flops_exec = flops the kernels actually issue for useful elements (L-first order),
+ * op_bytes = 8·Σ_tasks (m′m + n′n), workspace_bytes = what heff_apply needs (128-B aligned). */
+int32_t dmrgk_heff_query(const dmrgk_heff* h, int64_t* n_tasks, double* flops_alg,
+                         double* flops_exec, int64_t* op_bytes, int64_t* workspace_bytes,
+                         int64_t* n_chunks, int64_t* n_launches_per_apply);
+
+/* ---- a3 + a5..a7: σ = H_eff ψ ------------------------------------------------------------- */
+/* Overwrites sigma_dev (whole padded arena).  psi_dev and sigma_dev must not alias.
+ * stream_copy is used only when pinned operators are present (may equal NULL otherwise). */
+int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev,
+                         void* workspace_dev, void* stream_main, void* stream_copy);
+/* End-to-end form with HOST buffers (packed layout, pinned recommended): H2D ψ, apply, D2H σ,
+ * synchronises.  psi_dev / sigma_dev are device scratch arenas of n_padded doubles. */
+int32_t dmrgk_heff_apply_host(dmrgk_heff* h, const double* psi_host, double* sigma_host,
+                              double* psi_dev, double* sigma_dev, void* workspace_dev,
+                              void* stream_main, void* stream_copy);
+/* a4: diag(H_eff) in ψ layout: Σ over tasks whose input block = output block of
+ * coef·sign·L[i,i]·R[j,j].  Pinned operators are read through the ring like in apply. */
+int32_t dmrgk_heff_diag(dmrgk_heff* h, double* diag_dev, void* workspace_dev, void* stream_main,
+                        void* stream_copy);
+
+/* ---- a8: vector kernels over the flat padded arena (n doubles) ---------------------------- */
+/* Reductions are two-stage and fixed-order (bit-reproducible); scratch_dev needs
+ * dmrgk_vec_scratch_bytes(nv) bytes; results land in out_dev[nv] (device) — asynchronous. */
+int64_t dmrgk_vec_scratch_bytes(int32_t nv);
+/* out[j] = Σ_i X[j·stride + i] · y[i], j < nv. */
+int32_t dmrgk_vec_multi_dot(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double* X_dev,
+                            int64_t stride, const double* y_dev, double* out_dev,
+                            void* scratch_dev, void* stream);
+/* y[i] = beta·y[i] + Σ_j coef_dev[j]·X[j·stride + i]  (coefficients read from device memory;
+ * beta = 0 overwrites without reading y). */
+int32_t dmrgk_vec_multi_axpy(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double* X_dev,
+                             int64_t stride, const double* coef_dev, double beta, double* y_dev,
+                             void* stream);
+/* y = alpha·x + beta·y with host scalars. */
+int32_t dmrgk_vec_axpby(dmrgk_ctx* ctx, int64_t n, double alpha, const double* x_dev, double beta,
+                        double* y_dev, void* stream);
+/* x *= (*alpha_dev) if inv == 0, x /= (*alpha_dev) if inv != 0. */
+int32_t dmrgk_vec_scal_dev(dmrgk_ctx* ctx, int64_t n, const double* alpha_dev, int32_t inv,
+                           double* x_dev, void* stream);
+/* Davidson residual and correction (SURVEY §8(c) "Davidson, step by step"):
+ *   r = Σ_j y[j]·(W_j − θ V_j);  out[0] = ‖r‖²  (y, θ from device: coef_dev[0..m) = y, coef_dev[m] = θ) */
+int32_t dmrgk_vec_residual(dmrgk_ctx* ctx, int64_t n, int32_t m, const double* V_dev,
+                           const double* W_dev, int64_t stride, const double* coef_dev,
+                           double* r_dev, double* out_dev, void* scratch_dev, void* stream);
+/*   t[i] = r[i] / den, den = θ − d[i], |den| < 1e-10 → ±1e-10 (sign of den, +0 → +). */
+int32_t dmrgk_vec_precond(dmrgk_ctx* ctx, int64_t n, const double* r_dev, const double* diag_dev,
+                          const double* theta_dev, double* t_dev, void* stream);
+
+/* ---- a8 + a9: Davidson (ε_Davidson = residual 2-norm) ----- */
+/* basis_V_dev / basis_W_dev hold m_max vectors of n_padded doubles each (caller-owned), diag_dev the
+ * diagonal from dmrgk_heff_diag, workspace_dev the heff_apply workspace plus
+ * dmrgk_davidson_extra_bytes(m_max, n_padded) bytes after it. */
+int64_t dmrgk_davidson_extra_bytes(int32_t m_max, int64_t n_padded);
+int32_t dmrgk_davidson_create(dmrgk_heff* h, int32_t m_max, double tol, int32_t max_iter,
+                              double* basis_V_dev, double* basis_W_dev, const double* diag_dev,
+                              void* workspace_dev, void* stream_main, void* stream_copy,
+                              dmrgk_davidson** out);
+void dmrgk_davidson_destroy(dmrgk_davidson* d);
+/* V_0 = x0/‖x0‖, W_0 = H V_0, m = 1. */
+int32_t dmrgk_davidson_start(dmrgk_davidson* d, const double* x0_dev);
+/* One pass of the loop = exactly one H_eff apply (none if it converges first):
+ * Rayleigh–Ritz on the current basis → θ, residual norm; if not converged: (collapse restart if
+ * m = m_max), preconditioned correction, 2× Gram–Schmidt, normalise, apply, append. */
+int32_t dmrgk_davidson_step(dmrgk_davidson* d, double* theta, double* resnorm, int32_t* converged);
+/* Steps until ‖r‖ ≤ tol or max_iter applies; writes the Ritz vector to x_dev (n_padded doubles).
+ * Returns DMRGK_ENOTCONV (θ and x still written) when max_iter is reached. */
+int32_t dmrgk_davidson_solve(dmrgk_davidson* d, double* theta, double* resnorm, double* x_dev,
+                             int32_t* n_apply);
+/* Current subspace size m. */
+int32_t dmrgk_davidson_query(const dmrgk_davidson* d, int32_t* m, int32_t* n_apply);
+
+/* ---- harness kernels (outside the hot path): seeded inputs and FP64 pipe probes ----------- */
+/* Counter-based values, bit-identical to workloads/rng.py normal12(seed, stream, index): fills the
+ * packed arena of an operator / a ψ layout from the UNPADDED element index of each entry, times
+ * scale (scale_mode 0: 1, 1: 1/sqrt(cols of the block)); symmetric != 0: square diagonal-sector
+ * blocks get 0.5·(g(r,c)+g(c,r)).  Padding is zero-filled. */
+int32_t dmrgk_op_fill_normal(const dmrgk_op* op, double* arena_dev, uint64_t seed, uint64_t stream_id,
+                             int32_t scale_mode, int32_t symmetric, void* stream);
+int32_t dmrgk_layout_fill_normal(const dmrgk_layout* l, double* arena_dev, uint64_t seed,
+                                 uint64_t stream_id, void* stream);
+/* Register-only FP64 pipe probes: every warp of a full grid issues `iters` rounds of 16 independent
+ * mma.sync.m8n8k4.f64 (kind 0) or 32 independent fma.rn.f64 per lane (kind 1).  Returns the flops
+ * issued in *flops; the caller times the stream with events. */
+int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* sink_dev,
+                         double* flops, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DMRGK_H */

@@ -1,0 +1,205 @@
+// internal.h — private structures of libdmrgk (not part of the ABI; see include/dmrgk.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+#include <unordered_map>
+#include "../../include/dmrgk.h"
+
+namespace dmrgk {
+
+// ---- error plumbing ----------------------------------------------------------------------------
+int32_t fail(int32_t code, const char* fmt, ...);
+#define DMRGK_CUDA(call)                                                                         \
+    do {                                                                                         \
+        cudaError_t e__ = (call);                                                                \
+        if (e__ != cudaSuccess)                                                                  \
+            return dmrgk::fail(DMRGK_ECUDA, "%s failed: %s (%s:%d)", #call,                      \
+                               cudaGetErrorString(e__), __FILE__, __LINE__);                     \
+    } while (0)
+#define DMRGK_TRY(call)                                                                          \
+    do {                                                                                         \
+        int32_t s__ = (call);                                                                    \
+        if (s__ != DMRGK_OK) return s__;                                                         \
+    } while (0)
+
+static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+static inline bool aligned128(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 127u) == 0; }
+
+constexpr int LD_PAD = 16;  // leading dimensions and block offsets are multiples of 16 doubles (128 B)
+
+// ---- a1: sectors and blocks --------------------------------------------------------------------
+struct Block {
+    int32_t r_idx, c_idx;  // sector indices (row, column); for ψ: (a, b)
+    int32_t rows, cols, ld;
+    int64_t off;           // doubles into the packed arena
+    int64_t uoff;          // elements into the unpadded form
+};
+
+// Block table mirrored on the device for the fill kernel.
+struct DevBlock {
+    int64_t off, uoff;
+    int32_t rows, cols, ld, square_diag;
+};
+
+}  // namespace dmrgk
+
+struct dmrgk_ctx {
+    int device = 0;
+    int n_sm = 0;
+    int64_t l2_bytes = 0, hbm_bytes = 0;
+    int smem_optin = 0;
+};
+
+struct dmrgk_space {
+    dmrgk_ctx* ctx;
+    int n_charges;
+    std::vector<int32_t> q;     // [n][2] (second component 0 for one charge)
+    std::vector<int32_t> dim;
+    std::unordered_map<int64_t, int32_t> index;
+    static int64_t key(int32_t a, int32_t b) { return (int64_t(a) << 32) ^ int64_t(uint32_t(b)); }
+    int n() const { return int(dim.size()); }
+    int find(int32_t a, int32_t b) const {
+        auto it = index.find(key(a, b));
+        return it == index.end() ? -1 : it->second;
+    }
+    int parity(int i) const { return (q[2 * i] + q[2 * i + 1]) & 1; }
+};
+
+struct dmrgk_layout {
+    dmrgk_ctx* ctx;
+    const dmrgk_space *A, *B;
+    int32_t target[2];
+    std::vector<dmrgk::Block> blocks;
+    std::vector<int32_t> by_a;   // A sector → block index or −1
+    int64_t n_elems = 0, n_padded = 0;
+    dmrgk::DevBlock* dev_table = nullptr;
+};
+
+struct dmrgk_op {
+    dmrgk_ctx* ctx;
+    const dmrgk_space* space;
+    int32_t dq[2];
+    int32_t parity;
+    std::vector<dmrgk::Block> blocks;
+    std::vector<int32_t> by_col, by_row;   // sector → block index or −1
+    int64_t n_elems = 0, n_padded = 0;
+    const double* dev = nullptr;
+    const double* pinned = nullptr;
+    dmrgk::DevBlock* dev_table = nullptr;
+};
+
+namespace dmrgk {
+
+// ---- a2: device-side work descriptions ---------------------------------------------------------
+// Pointers that depend on heff_apply arguments (ψ, σ, workspace) are stored as byte offsets plus a
+// 2-bit base selector; the kernels add the base passed at launch (Bases).  Resident operator blocks
+// are absolute addresses (selector 0, base 0).
+enum : uint32_t { BASE_ABS = 0u, BASE_WS = 1u, BASE_PSI = 2u, BASE_SIGMA = 3u };
+struct Bases {
+    unsigned long long b[4];
+};
+
+// One GEMM "segment": C_tile += A[i, k]·B[k, j] over k < klen.  A is K-major (A[i·lda + k]) or
+// M-major (A[k·lda + i]); B is K-major (B[j·ldb + k]) or N-major (B[k·ldb + j]).
+enum : uint32_t {
+    SEG_A_MMAJOR = 1u,
+    SEG_B_NMAJOR = 2u,
+    SEG_A_SEL_SHIFT = 4,   // bits 4-5: base selector of A
+    SEG_B_SEL_SHIFT = 6    // bits 6-7: base selector of B
+};
+struct Seg {
+    unsigned long long A, B;   // byte address / byte offset of the operand BLOCK origin
+    int32_t lda, ldb;
+    int32_t klen;
+    uint32_t flags;
+};  // 32 B
+
+// One CTA work unit: a (≤64 × ≤64) tile of C summed over segments [seg_begin, seg_end).
+enum : uint32_t { UNIT_ACCUM = 1u, UNIT_C_SEL_SHIFT = 4 };
+struct Unit {
+    unsigned long long C;   // byte address / offset of the tile origin
+    double alpha;
+    int32_t ldc;
+    int32_t i0, j0;     // tile origin inside the operand blocks
+    int32_t mrows;      // block rows (A-operand row extent)
+    int32_t ncols;      // block cols (B-operand column extent)
+    int32_t ncols_st;   // columns to store (padded ld of the C block); columns ≥ ncols get zeros
+    int32_t seg_begin, seg_end;
+    uint32_t mode;      // UNIT_ACCUM | selector << UNIT_C_SEL_SHIFT
+    int32_t nkt;        // Σ over the unit's segments of ceil(klen/16)
+};  // 56 B
+
+// Fixed-order reduction of split-k partial tiles into σ: C[r, c] += Σ_s P[s][r·64 + c].
+struct RUnit {
+    unsigned long long C;   // byte offset into σ of the tile origin
+    unsigned long long P;   // byte offset into the workspace of the first partial tile (64×64 each)
+    int32_t ldc, rows, cols, n_split;
+};  // 32 B
+
+// diag(H_eff) work: ψ block `DiagBlock` sums alpha·L[i,i]·R[j,j] over tasks [t_begin, t_end).
+struct DiagTask {
+    unsigned long long L, R;   // block origins; the diagonal is walked with stride ld+1
+    double alpha;
+    int32_t ldl, ldr;
+    uint32_t sel;              // selector of L in bits 0-1, of R in bits 2-3
+    int32_t pad_;
+};
+struct DiagBlock {
+    int64_t off;               // doubles into the ψ-layout arena
+    int32_t rows, cols, ld;
+    int32_t t_begin, t_end;
+    int32_t pad_;
+};
+
+constexpr int TILE_M = 64, TILE_N = 64;
+
+// kernel launchers (heff_kernels.cu)
+int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
+                          const Bases& bases, cudaStream_t st);
+int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cudaStream_t st);
+int32_t launch_diag(const DiagBlock* blocks_dev, const DiagTask* tasks_dev, int64_t n_blocks,
+                    double* diag, const Bases& bases, cudaStream_t st);
+int32_t gemm_kernel_setup();   // opt-in shared memory attribute, once
+
+// chunk = contiguous range of operator pairs processed together
+struct StageCopy {
+    const double* src_host;
+    int64_t ring_off;   // doubles into the ring half
+    int64_t n;          // doubles
+};
+struct Chunk {
+    int64_t p1_unit0 = 0, p1_units = 0, p1_seg0 = 0;
+    int64_t p2_unit0 = 0, p2_units = 0, p2_seg0 = 0;
+    int64_t r_unit0 = 0, r_units = 0;
+    int64_t p1_segs = 0, p2_segs = 0;
+    int64_t d_block0 = 0, d_blocks = 0;
+    std::vector<StageCopy> copies;
+    int ring_half = -1;
+};
+
+}  // namespace dmrgk
+
+struct dmrgk_heff {
+    dmrgk_ctx* ctx;
+    const dmrgk_layout* layout;
+    dmrgk_heff_opts opts;
+    int64_t n_tasks = 0;
+    double flops_alg = 0, flops_exec = 0;
+    int64_t op_bytes = 0;
+    int64_t t_bytes = 0, partial_bytes = 0, ring_bytes = 0, ring_half_bytes = 0, workspace_bytes = 0;
+    bool done_recorded[2] = {false, false};
+    std::vector<dmrgk::Chunk> chunks;
+    // device metadata (library-owned)
+    dmrgk::Unit* units_dev = nullptr;
+    dmrgk::Seg* segs_dev = nullptr;
+    dmrgk::RUnit* runits_dev = nullptr;
+    dmrgk::DiagBlock* dblocks_dev = nullptr;
+    dmrgk::DiagTask* dtasks_dev = nullptr;
+    int64_t n_dblocks = 0;
+    double* ident_dev = nullptr;       // identity block for IDENT_L / IDENT_R factors
+    cudaEvent_t ev_copy[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
+    int64_t n_launches = 0;
+    bool has_pinned = false;
+};

@@ -1,0 +1,625 @@
+// tasklist.cu — a2/a3/a5-a7 host side: the operator-pair task list and σ = H_eff ψ
+// ("enumerate (k, input block) … group by output block, tile, split-k plan";
+// PAPER.md:142 "Tables", "H2D IO" for the staging of pinned operators).
+//
+// For pair k and ψ block (a, b):   σ[a′, b′] += c_k·s · Lapp[a′, a] · ψ[a, b] · Rapp[b′, b]ᵀ,
+// s = −1 iff the pair is fermionic (odd) and the INPUT A sector has odd particle number
+// (SURVEY.md §8.0).  Work is cut into chunks of consecutive pairs; per chunk
+//   phase 1:  T_t = c·s · Lapp ψ[a, b]                 one GEMM unit per 64×64 tile of T_t
+//   phase 2:  σ[a′, b′] += [T_t …]·[Rapp_t …]ᵀ          tasks grouped by OUTPUT block and stacked
+//             along the contraction axis; a tile is owned by one CTA, or split along the task list
+//             into partial tiles that a fixed-order reduction kernel adds up — never atomics.
+#include "internal.h"
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+using namespace dmrgk;
+
+namespace {
+
+struct Task {
+    int32_t k;
+    int32_t ib, ob;          // input / output ψ block
+    int32_t mo, m, n, no;    // m′, m, n, n′
+    Seg s1, s2;              // phase-1 / phase-2 segment templates (A of s2 filled per chunk)
+    double alpha;
+    bool diag;
+};
+
+struct OpRef {               // where an operator block lives
+    unsigned long long addr; // absolute byte address, or byte offset inside the ring half
+    uint32_t sel;            // BASE_ABS or BASE_WS (ring offset still to be added)
+    int ld;
+};
+
+int64_t cost_of(int rows, int cols, int64_t nkt) {
+    return int64_t((rows + 7) / 8) * ((cols + 7) / 8) * nkt;
+}
+
+template <class T>
+int32_t upload(const std::vector<T>& v, T** out) {
+    *out = nullptr;
+    if (v.empty()) return DMRGK_OK;
+    DMRGK_CUDA(cudaMalloc(out, v.size() * sizeof(T)));
+    DMRGK_CUDA(cudaMemcpy(*out, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return DMRGK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+void dmrgk_heff_destroy(dmrgk_heff* h) {
+    if (!h) return;
+    cudaFree(h->units_dev);
+    cudaFree(h->segs_dev);
+    cudaFree(h->runits_dev);
+    cudaFree(h->dblocks_dev);
+    cudaFree(h->dtasks_dev);
+    cudaFree(h->ident_dev);
+    for (int i = 0; i < 2; ++i) {
+        if (h->ev_copy[i]) cudaEventDestroy(h->ev_copy[i]);
+        if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
+    }
+    delete h;
+}
+
+int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
+                          dmrgk_op* const* L, dmrgk_op* const* R, const double* coef,
+                          const uint32_t* flags, const dmrgk_heff_opts* opts, dmrgk_heff** out) {
+    if (!out) return fail(DMRGK_EINVAL, "heff_create: out is NULL");
+    *out = nullptr;
+    if (!ctx || !layout) return fail(DMRGK_EINVAL, "heff_create: NULL ctx or layout");
+    if (K < 0 || (K > 0 && (!L || !R || !coef || !flags)))
+        return fail(DMRGK_EINVAL, "heff_create: bad pair arrays (K = %lld)", (long long)K);
+    DMRGK_CUDA(cudaSetDevice(ctx->device));
+    dmrgk_heff_opts o;
+    memset(&o, 0, sizeof(o));
+    if (opts) o = *opts;
+    if (o.t_chunk_bytes <= 0) o.t_chunk_bytes = int64_t(4) << 30;
+    if (o.split_waves <= 0) o.split_waves = 8;
+    if (o.ring_bytes < 0 || (o.kernel != 0 && o.kernel != 1))
+        return fail(DMRGK_EINVAL, "heff_create: bad options");
+    const int64_t ring_half = (o.ring_bytes / 2) / 128 * 128;
+
+    const dmrgk_space *SA = layout->A, *SB = layout->B;
+    const std::vector<Block>& pb = layout->blocks;
+
+    // ---- validation of every pair (SURVEY §8(b) "validation errors that must be reported") ----
+    for (int64_t k = 0; k < K; ++k) {
+        const uint32_t f = flags[k];
+        if (f & ~15u) return fail(DMRGK_EINVAL, "heff_create: pair %lld has unknown flag bits 0x%x", (long long)k, f);
+        if (bool(f & DMRGK_IDENT_L) != (L[k] == nullptr) || bool(f & DMRGK_IDENT_R) != (R[k] == nullptr))
+            return fail(DMRGK_EINVAL, "heff_create: pair %lld: IDENT flag and NULL operator must go together", (long long)k);
+        if (L[k] && L[k]->space != SA) return fail(DMRGK_ESHAPE, "heff_create: pair %lld: L is not on the layout's A space", (long long)k);
+        if (R[k] && R[k]->space != SB) return fail(DMRGK_ESHAPE, "heff_create: pair %lld: R is not on the layout's B space", (long long)k);
+        int dl[2] = {0, 0}, dr[2] = {0, 0};
+        if (L[k]) for (int c = 0; c < 2; ++c) dl[c] = (f & DMRGK_TRANS_L) ? -L[k]->dq[c] : L[k]->dq[c];
+        if (R[k]) for (int c = 0; c < 2; ++c) dr[c] = (f & DMRGK_TRANS_R) ? -R[k]->dq[c] : R[k]->dq[c];
+        if (dl[0] + dr[0] != 0 || dl[1] + dr[1] != 0)
+            return fail(DMRGK_ECHARGE, "heff_create: pair %lld: applied shifts (%d,%d)+(%d,%d) do not cancel", (long long)k, dl[0], dl[1], dr[0], dr[1]);
+        if (L[k] && R[k] && L[k]->parity != R[k]->parity)
+            return fail(DMRGK_ECHARGE, "heff_create: pair %lld: parities of L and R differ", (long long)k);
+        for (const dmrgk_op* op : {(const dmrgk_op*)L[k], (const dmrgk_op*)R[k]}) {
+            if (!op || op->n_padded == 0) continue;
+            if (!op->dev && !op->pinned) return fail(DMRGK_ESTATE, "heff_create: pair %lld has an unbound operator", (long long)k);
+            if (op->pinned && ring_half == 0) return fail(DMRGK_ESTATE, "heff_create: pair %lld has a pinned operator but ring_bytes = 0", (long long)k);
+            if (op->pinned && op->n_padded * 8 > ring_half)
+                return fail(DMRGK_ENOMEM, "heff_create: pinned operator of %lld bytes exceeds half the ring (%lld)", (long long)(op->n_padded * 8), (long long)ring_half);
+        }
+    }
+
+    dmrgk_heff* h = new (std::nothrow) dmrgk_heff;
+    if (!h) return fail(DMRGK_ENOMEM, "heff_create: out of host memory");
+    h->ctx = ctx;
+    h->layout = layout;
+    h->opts = o;
+    auto bail = [&](int32_t s) {
+        dmrgk_heff_destroy(h);
+        return s;
+    };
+
+    // identity block for IDENT factors
+    int max_dim = 0;
+    for (const Block& b : pb) max_dim = std::max(max_dim, std::max(b.rows, b.cols));
+    const int ident_ld = int(round_up(std::max(max_dim, 1), LD_PAD));
+    bool need_ident = false;
+    for (int64_t k = 0; k < K; ++k) need_ident |= (flags[k] & (DMRGK_IDENT_L | DMRGK_IDENT_R)) != 0;
+    if (need_ident) {
+        std::vector<double> id(size_t(ident_ld) * ident_ld, 0.0);
+        for (int i = 0; i < ident_ld; ++i) id[size_t(i) * ident_ld + i] = 1.0;
+        cudaError_t e = cudaMalloc(&h->ident_dev, id.size() * 8);
+        if (e == cudaSuccess) e = cudaMemcpy(h->ident_dev, id.data(), id.size() * 8, cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) return bail(fail(DMRGK_ECUDA, "heff_create: identity block: %s", cudaGetErrorString(e)));
+    }
+
+    // ---- chunking of the pair list + task enumeration ----------------------------------------
+    std::vector<Unit> units;
+    std::vector<Seg> segs;
+    std::vector<RUnit> runits;
+    std::vector<DiagBlock> dblocks;
+    std::vector<DiagTask> dtasks;
+    const int64_t slots = int64_t(ctx->n_sm) * 3;
+    int64_t max_t_bytes = 0, max_partial_tiles = 0;
+
+    int64_t k0 = 0;
+    while (k0 < K) {
+        Chunk ch;
+        ch.ring_half = int(h->chunks.size() & 1);
+        std::vector<Task> tasks;
+        std::unordered_map<const dmrgk_op*, int64_t> staged;   // pinned op → ring offset (bytes)
+        int64_t ring_used = 0, t_bytes = 0;
+        int64_t k = k0;
+        for (; k < K; ++k) {
+            const uint32_t f = flags[k];
+            // staging need of this pair
+            int64_t need = 0;
+            for (const dmrgk_op* op : {(const dmrgk_op*)L[k], (const dmrgk_op*)R[k]})
+                if (op && op->pinned && op->n_padded && !staged.count(op)) need += round_up(op->n_padded * 8, 128);
+            // T bytes of this pair
+            int64_t tb = 0;
+            std::vector<Task> mine;
+            for (int ib = 0; ib < int(pb.size()); ++ib) {
+                const int a = pb[ib].r_idx, b = pb[ib].c_idx;
+                Task t;
+                memset(&t, 0, sizeof(t));
+                t.k = int32_t(k);
+                t.ib = ib;
+                t.m = pb[ib].rows;
+                t.n = pb[ib].cols;
+                int ao, bo;
+                // L applied to sector a
+                if (!L[k]) {
+                    ao = a;
+                    t.mo = t.m;
+                    t.s1.A = (unsigned long long)(uintptr_t)h->ident_dev;
+                    t.s1.lda = ident_ld;
+                    t.s1.flags = BASE_ABS << SEG_A_SEL_SHIFT;
+                } else {
+                    const int bi = (f & DMRGK_TRANS_L) ? L[k]->by_row[a] : L[k]->by_col[a];
+                    if (bi < 0) continue;
+                    const Block& lb = L[k]->blocks[bi];
+                    ao = (f & DMRGK_TRANS_L) ? lb.c_idx : lb.r_idx;
+                    t.mo = (f & DMRGK_TRANS_L) ? lb.cols : lb.rows;
+                    t.s1.lda = lb.ld;
+                    t.s1.flags = (f & DMRGK_TRANS_L) ? SEG_A_MMAJOR : 0u;
+                    if (L[k]->dev) {
+                        t.s1.A = (unsigned long long)(uintptr_t)(L[k]->dev + lb.off);
+                        t.s1.flags |= BASE_ABS << SEG_A_SEL_SHIFT;
+                    } else {
+                        t.s1.A = (unsigned long long)(lb.off * 8);   // ring offset added below
+                        t.s1.flags |= BASE_WS << SEG_A_SEL_SHIFT;
+                    }
+                }
+                if (!R[k]) {
+                    bo = b;
+                    t.no = t.n;
+                    t.s2.B = (unsigned long long)(uintptr_t)h->ident_dev;
+                    t.s2.ldb = ident_ld;
+                    t.s2.flags = BASE_ABS << SEG_B_SEL_SHIFT;
+                } else {
+                    const int bi = (f & DMRGK_TRANS_R) ? R[k]->by_row[b] : R[k]->by_col[b];
+                    if (bi < 0) continue;
+                    const Block& rb = R[k]->blocks[bi];
+                    bo = (f & DMRGK_TRANS_R) ? rb.c_idx : rb.r_idx;
+                    t.no = (f & DMRGK_TRANS_R) ? rb.cols : rb.rows;
+                    t.s2.ldb = rb.ld;
+                    t.s2.flags = (f & DMRGK_TRANS_R) ? SEG_B_NMAJOR : 0u;
+                    if (R[k]->dev) {
+                        t.s2.B = (unsigned long long)(uintptr_t)(R[k]->dev + rb.off);
+                        t.s2.flags |= BASE_ABS << SEG_B_SEL_SHIFT;
+                    } else {
+                        t.s2.B = (unsigned long long)(rb.off * 8);
+                        t.s2.flags |= BASE_WS << SEG_B_SEL_SHIFT;
+                    }
+                }
+                const int ob = layout->by_a[ao];
+                if (ob < 0 || pb[ob].c_idx != bo) continue;
+                t.ob = ob;
+                const int par = L[k] ? L[k]->parity : (R[k] ? R[k]->parity : 0);
+                t.alpha = coef[k] * ((par && SA->parity(a)) ? -1.0 : 1.0);
+                t.diag = (ob == ib);
+                // phase-1 B operand = ψ block (N-major), phase-2 A operand = T (K-major, set per chunk)
+                t.s1.B = (unsigned long long)(pb[ib].off * 8);
+                t.s1.ldb = pb[ib].ld;
+                t.s1.klen = t.m;
+                t.s1.flags |= SEG_B_NMAJOR | (BASE_PSI << SEG_B_SEL_SHIFT);
+                t.s2.lda = pb[ib].ld;
+                t.s2.klen = t.n;
+                t.s2.flags |= BASE_WS << SEG_A_SEL_SHIFT;
+                tb += int64_t(t.mo) * pb[ib].ld * 8;
+                mine.push_back(t);
+            }
+            const bool nonempty = !tasks.empty() || !staged.empty();
+            if (nonempty && (t_bytes + tb > o.t_chunk_bytes || ring_used + need > ring_half)) break;
+            // accept pair k into the chunk
+            for (const dmrgk_op* op : {(const dmrgk_op*)L[k], (const dmrgk_op*)R[k]})
+                if (op && op->pinned && op->n_padded && !staged.count(op)) {
+                    staged[op] = ring_used;
+                    ch.copies.push_back({op->pinned, ring_used / 8, op->n_padded});
+                    ring_used += round_up(op->n_padded * 8, 128);
+                }
+            for (Task& t : mine) {
+                if (L[k] && !L[k]->dev) t.s1.A += (unsigned long long)staged[L[k]];
+                if (R[k] && !R[k]->dev) t.s2.B += (unsigned long long)staged[R[k]];
+                tasks.push_back(t);
+            }
+            t_bytes += tb;
+        }
+        k0 = k;
+        max_t_bytes = std::max(max_t_bytes, t_bytes);
+
+        // ---- flop / byte accounting ----
+        for (const Task& t : tasks) {
+            const double mo = t.mo, m = t.m, n = t.n, no = t.no;
+            const bool il = !L[t.k], ir = !R[t.k];
+            if (il && ir) {
+            } else if (il) {
+                h->flops_alg += 2 * m * n * no;
+            } else if (ir) {
+                h->flops_alg += 2 * mo * m * n;
+            } else {
+                h->flops_alg += std::min(2 * mo * n * (m + no), 2 * m * no * (n + mo));
+            }
+            h->flops_exec += 2 * mo * m * n + 2 * mo * n * no;
+            if (!il) h->op_bytes += int64_t(8) * t.mo * t.m;
+            if (!ir) h->op_bytes += int64_t(8) * t.no * t.n;
+        }
+        h->n_tasks += int64_t(tasks.size());
+
+        // ---- phase 1: one segment + tiles per task; T laid out task after task ----
+        ch.p1_unit0 = int64_t(units.size());
+        ch.p1_seg0 = int64_t(segs.size());
+        {
+            std::vector<int64_t> t_off(tasks.size());
+            int64_t off = 0;
+            for (size_t i = 0; i < tasks.size(); ++i) {
+                t_off[i] = off;
+                off += int64_t(tasks[i].mo) * pb[tasks[i].ib].ld * 8;
+            }
+            struct U1 {
+                int64_t cost;
+                Unit u;
+            };
+            std::vector<U1> tmp;
+            for (size_t i = 0; i < tasks.size(); ++i) {
+                Task& t = tasks[i];
+                segs.push_back(t.s1);   // a staged A still lacks the ring base (added below)
+                t.s2.A = (unsigned long long)t_off[i];
+                const int ldt = pb[t.ib].ld;
+                const int64_t nkt = (t.m + 15) / 16;
+                for (int i0 = 0; i0 < t.mo; i0 += TILE_M)
+                    for (int j0 = 0; j0 < ldt; j0 += TILE_N) {
+                        Unit u;
+                        memset(&u, 0, sizeof(u));
+                        u.C = (unsigned long long)(t_off[i] + (int64_t(i0) * ldt + j0) * 8);
+                        u.alpha = t.alpha;
+                        u.ldc = ldt;
+                        u.i0 = i0;
+                        u.j0 = j0;
+                        u.mrows = t.mo;
+                        u.ncols = t.n;
+                        u.ncols_st = ldt;
+                        u.seg_begin = int32_t(i);   // chunk-local, rebased below
+                        u.seg_end = int32_t(i) + 1;
+                        u.mode = BASE_WS << UNIT_C_SEL_SHIFT;
+                        u.nkt = int32_t(nkt);
+                        tmp.push_back({cost_of(std::min(TILE_M, t.mo - i0), std::min(TILE_N, ldt - j0), nkt), u});
+                    }
+            }
+            std::stable_sort(tmp.begin(), tmp.end(), [](const U1& a, const U1& b) { return a.cost > b.cost; });
+            for (const U1& x : tmp) units.push_back(x.u);
+            ch.p1_units = int64_t(tmp.size());
+            ch.p1_segs = int64_t(tasks.size());
+        }
+
+        // ---- phase 2: group by output block, stack along k, split-k plan ----
+        ch.p2_unit0 = int64_t(units.size());
+        ch.p2_seg0 = int64_t(segs.size());
+        ch.r_unit0 = int64_t(runits.size());
+        {
+            std::vector<std::vector<int>> by_ob(pb.size());
+            for (size_t i = 0; i < tasks.size(); ++i) by_ob[tasks[i].ob].push_back(int(i));
+            // total cost → target cost of a unit
+            int64_t total_cost = 0;
+            for (size_t ob = 0; ob < pb.size(); ++ob) {
+                int64_t nkt = 0;
+                for (int i : by_ob[ob]) nkt += (tasks[i].n + 15) / 16;
+                for (int i0 = 0; i0 < pb[ob].rows; i0 += TILE_M)
+                    for (int j0 = 0; j0 < pb[ob].ld; j0 += TILE_N)
+                        total_cost += cost_of(std::min(TILE_M, pb[ob].rows - i0), std::min(TILE_N, pb[ob].ld - j0), nkt);
+            }
+            const int64_t target = std::max<int64_t>(64 * 16, total_cost / std::max<int64_t>(1, slots * o.split_waves));
+            struct U2 {
+                int64_t cost;
+                Unit u;
+            };
+            std::vector<U2> tmp;
+            int64_t partial_tiles = 0;
+            for (size_t ob = 0; ob < pb.size(); ++ob) {
+                if (by_ob[ob].empty()) continue;
+                const int seg0 = int(segs.size() - ch.p2_seg0);
+                std::vector<int64_t> prefix(1, 0);
+                for (int i : by_ob[ob]) {
+                    segs.push_back(tasks[i].s2);
+                    prefix.push_back(prefix.back() + (tasks[i].n + 15) / 16);
+                }
+                const int ns = int(by_ob[ob].size());
+                const int64_t nkt = prefix.back();
+                const Block& B = pb[ob];
+                for (int i0 = 0; i0 < B.rows; i0 += TILE_M)
+                    for (int j0 = 0; j0 < B.ld; j0 += TILE_N) {
+                        const int rt = std::min(TILE_M, B.rows - i0), ct = std::min(TILE_N, B.ld - j0);
+                        const int64_t c = cost_of(rt, ct, nkt);
+                        int n_split = int(std::min<int64_t>(ns, (c + target - 1) / target));
+                        if (n_split < 1) n_split = 1;
+                        Unit u;
+                        memset(&u, 0, sizeof(u));
+                        u.alpha = 1.0;
+                        u.i0 = i0;
+                        u.j0 = j0;
+                        u.mrows = B.rows;
+                        u.ncols = B.cols;
+                        u.ncols_st = B.ld;
+                        const unsigned long long c_sigma = (unsigned long long)((B.off + int64_t(i0) * B.ld + j0) * 8);
+                        if (n_split == 1) {
+                            u.C = c_sigma;
+                            u.ldc = B.ld;
+                            u.seg_begin = seg0;
+                            u.seg_end = seg0 + ns;
+                            u.mode = UNIT_ACCUM | (BASE_SIGMA << UNIT_C_SEL_SHIFT);
+                            u.nkt = int32_t(nkt);
+                            tmp.push_back({c, u});
+                        } else {
+                            RUnit r;
+                            r.C = c_sigma;
+                            r.P = (unsigned long long)(partial_tiles * TILE_M * TILE_N * 8);   // rebased below
+                            r.ldc = B.ld;
+                            r.rows = rt;
+                            r.cols = ct;
+                            int made = 0, sb = 0;
+                            for (int s = 0; s < n_split; ++s) {
+                                // even split of the k-tiles along segment boundaries
+                                const int64_t want = nkt * (s + 1) / n_split;
+                                int se = sb;
+                                while (se < ns && prefix[se] < want) ++se;
+                                if (s == n_split - 1) se = ns;
+                                if (se == sb) continue;
+                                u.C = (unsigned long long)((partial_tiles + made) * TILE_M * TILE_N * 8);
+                                u.ldc = TILE_N;
+                                u.seg_begin = seg0 + sb;
+                                u.seg_end = seg0 + se;
+                                u.mode = BASE_WS << UNIT_C_SEL_SHIFT;
+                                u.nkt = int32_t(prefix[se] - prefix[sb]);
+                                tmp.push_back({cost_of(rt, ct, u.nkt), u});
+                                ++made;
+                                sb = se;
+                            }
+                            r.n_split = made;
+                            partial_tiles += made;
+                            runits.push_back(r);
+                        }
+                    }
+            }
+            std::stable_sort(tmp.begin(), tmp.end(), [](const U2& a, const U2& b) { return a.cost > b.cost; });
+            for (const U2& x : tmp) units.push_back(x.u);
+            ch.p2_units = int64_t(tmp.size());
+            ch.p2_segs = int64_t(segs.size()) - ch.p2_seg0;
+            ch.r_units = int64_t(runits.size()) - ch.r_unit0;
+            max_partial_tiles = std::max(max_partial_tiles, partial_tiles);
+        }
+
+        // ---- a4: diagonal tasks of this chunk, grouped by block ----
+        {
+            std::vector<std::vector<int>> by_b(pb.size());
+            for (size_t i = 0; i < tasks.size(); ++i)
+                if (tasks[i].diag) by_b[tasks[i].ib].push_back(int(i));
+            ch.d_block0 = int64_t(dblocks.size());
+            for (size_t b = 0; b < pb.size(); ++b) {
+                if (by_b[b].empty()) continue;
+                DiagBlock d;
+                d.off = pb[b].off;
+                d.rows = pb[b].rows;
+                d.cols = pb[b].cols;
+                d.ld = pb[b].ld;
+                d.t_begin = int32_t(dtasks.size());
+                for (int i : by_b[b]) {
+                    const Task& t = tasks[i];
+                    DiagTask dt;
+                    memset(&dt, 0, sizeof(dt));
+                    dt.L = t.s1.A;
+                    dt.R = t.s2.B;
+                    dt.alpha = t.alpha;
+                    dt.ldl = t.s1.lda;
+                    dt.ldr = t.s2.ldb;
+                    dt.sel = ((t.s1.flags >> SEG_A_SEL_SHIFT) & 3u) | (((t.s2.flags >> SEG_B_SEL_SHIFT) & 3u) << 2);
+                    dtasks.push_back(dt);
+                }
+                d.t_end = int32_t(dtasks.size());
+                d.pad_ = 0;
+                dblocks.push_back(d);
+            }
+            ch.d_blocks = int64_t(dblocks.size()) - ch.d_block0;
+        }
+        h->chunks.push_back(std::move(ch));
+    }
+
+    // ---- workspace layout: [T | partial tiles | ring half 0 | ring half 1] --------------------
+    h->t_bytes = round_up(max_t_bytes, 128);
+    h->partial_bytes = max_partial_tiles * TILE_M * TILE_N * 8;
+    bool any_pinned = false;
+    for (const Chunk& c : h->chunks) any_pinned |= !c.copies.empty();
+    h->has_pinned = any_pinned;
+    h->ring_bytes = any_pinned ? 2 * ring_half : 0;
+    h->ring_half_bytes = ring_half;
+    h->workspace_bytes = std::max<int64_t>(128, h->t_bytes + h->partial_bytes + h->ring_bytes);
+    const unsigned long long part_base = (unsigned long long)h->t_bytes;
+    const unsigned long long ring_base = part_base + (unsigned long long)h->partial_bytes;
+
+    // rebase: chunk-local segment indices → global, partial offsets → workspace, ring offsets
+    for (const Chunk& c : h->chunks) {
+        const unsigned long long ring = ring_base + (unsigned long long)(c.ring_half) * ring_half;
+        for (int64_t i = c.p1_unit0; i < c.p1_unit0 + c.p1_units; ++i) {
+            units[i].seg_begin += int32_t(c.p1_seg0);
+            units[i].seg_end += int32_t(c.p1_seg0);
+        }
+        for (int64_t i = c.p2_unit0; i < c.p2_unit0 + c.p2_units; ++i) {
+            units[i].seg_begin += int32_t(c.p2_seg0);
+            units[i].seg_end += int32_t(c.p2_seg0);
+            if (!(units[i].mode & UNIT_ACCUM)) units[i].C += part_base;
+        }
+        for (int64_t i = c.r_unit0; i < c.r_unit0 + c.r_units; ++i) runits[i].P += part_base;
+        for (int64_t s = c.p1_seg0; s < c.p1_seg0 + c.p1_segs; ++s)
+            if (((segs[s].flags >> SEG_A_SEL_SHIFT) & 3u) == BASE_WS) segs[s].A += ring;   // staged L block
+        for (int64_t s = c.p2_seg0; s < c.p2_seg0 + c.p2_segs; ++s)
+            if (((segs[s].flags >> SEG_B_SEL_SHIFT) & 3u) == BASE_WS) segs[s].B += ring;   // staged R block
+        for (int64_t b = c.d_block0; b < c.d_block0 + c.d_blocks; ++b)
+            for (int t = dblocks[b].t_begin; t < dblocks[b].t_end; ++t) {
+                if ((dtasks[t].sel & 3u) == BASE_WS) dtasks[t].L += ring;
+                if (((dtasks[t].sel >> 2) & 3u) == BASE_WS) dtasks[t].R += ring;
+            }
+    }
+    if (int64_t(segs.size()) > 0x7fffffffLL) return bail(fail(DMRGK_EINVAL, "heff_create: too many segments"));
+
+    h->n_launches = 1;
+    for (const Chunk& c : h->chunks) h->n_launches += (c.p1_units > 0) + (c.p2_units > 0) + (c.r_units > 0);
+
+    int32_t s = upload(units, &h->units_dev);
+    if (s == DMRGK_OK) s = upload(segs, &h->segs_dev);
+    if (s == DMRGK_OK) s = upload(runits, &h->runits_dev);
+    if (s == DMRGK_OK) s = upload(dblocks, &h->dblocks_dev);
+    if (s == DMRGK_OK) s = upload(dtasks, &h->dtasks_dev);
+    if (s != DMRGK_OK) return bail(s);
+    if (any_pinned)
+        for (int i = 0; i < 2; ++i) {
+            cudaError_t e = cudaEventCreateWithFlags(&h->ev_copy[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming);
+            if (e != cudaSuccess) return bail(fail(DMRGK_ECUDA, "heff_create: event: %s", cudaGetErrorString(e)));
+        }
+    *out = h;
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_heff_query(const dmrgk_heff* h, int64_t* n_tasks, double* flops_alg, double* flops_exec,
+                         int64_t* op_bytes, int64_t* workspace_bytes, int64_t* n_chunks,
+                         int64_t* n_launches_per_apply) {
+    if (!h) return fail(DMRGK_EINVAL, "heff_query: heff is NULL");
+    if (n_tasks) *n_tasks = h->n_tasks;
+    if (flops_alg) *flops_alg = h->flops_alg;
+    if (flops_exec) *flops_exec = h->flops_exec;
+    if (op_bytes) *op_bytes = h->op_bytes;
+    if (workspace_bytes) *workspace_bytes = h->workspace_bytes;
+    if (n_chunks) *n_chunks = int64_t(h->chunks.size());
+    if (n_launches_per_apply) *n_launches_per_apply = h->n_launches;
+    return DMRGK_OK;
+}
+
+}  // extern "C"
+
+namespace dmrgk {
+
+// Stage the pinned operators of chunk c into its ring half on the copy stream, ordered after the
+// last compute that read that half and before the compute that needs it (a3).
+static int32_t stage_chunk(dmrgk_heff* h, const Chunk& c, char* ws, cudaStream_t main, cudaStream_t copy) {
+    if (c.copies.empty()) return DMRGK_OK;
+    const int hf = c.ring_half;
+    char* ring = ws + h->t_bytes + h->partial_bytes + int64_t(hf) * h->ring_half_bytes;
+    if (h->done_recorded[hf]) DMRGK_CUDA(cudaStreamWaitEvent(copy, h->ev_done[hf], 0));
+    for (const StageCopy& sc : c.copies)
+        DMRGK_CUDA(cudaMemcpyAsync(ring + sc.ring_off * 8, sc.src_host, size_t(sc.n) * 8, cudaMemcpyHostToDevice, copy));
+    DMRGK_CUDA(cudaEventRecord(h->ev_copy[hf], copy));
+    DMRGK_CUDA(cudaStreamWaitEvent(main, h->ev_copy[hf], 0));
+    return DMRGK_OK;
+}
+
+static int32_t chunk_done(dmrgk_heff* h, const Chunk& c, cudaStream_t main) {
+    if (c.copies.empty()) return DMRGK_OK;
+    DMRGK_CUDA(cudaEventRecord(h->ev_done[c.ring_half], main));
+    h->done_recorded[c.ring_half] = true;
+    return DMRGK_OK;
+}
+
+}  // namespace dmrgk
+
+extern "C" {
+
+int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev, void* workspace_dev,
+                         void* stream_main, void* stream_copy) {
+    if (!h) return fail(DMRGK_EINVAL, "heff_apply: heff is NULL");
+    const int64_t n = h->layout->n_padded;
+    if (n == 0) return DMRGK_OK;
+    if (!psi_dev || !sigma_dev) return fail(DMRGK_EINVAL, "heff_apply: NULL vector");
+    if (psi_dev == sigma_dev) return fail(DMRGK_EINVAL, "heff_apply: psi and sigma alias");
+    if (!workspace_dev && h->n_tasks) return fail(DMRGK_EINVAL, "heff_apply: NULL workspace");
+    if (!aligned128(psi_dev) || !aligned128(sigma_dev) || !aligned128(workspace_dev))
+        return fail(DMRGK_EALIGN, "heff_apply: pointers must be 128-byte aligned");
+    DMRGK_CUDA(cudaSetDevice(h->ctx->device));
+    cudaStream_t main = (cudaStream_t)stream_main, copy = (cudaStream_t)stream_copy;
+    if (h->has_pinned && copy == main)
+        return fail(DMRGK_EINVAL, "heff_apply: pinned operators need a copy stream distinct from the main stream");
+    Bases bases;
+    bases.b[BASE_ABS] = 0;
+    bases.b[BASE_WS] = (unsigned long long)(uintptr_t)workspace_dev;
+    bases.b[BASE_PSI] = (unsigned long long)(uintptr_t)psi_dev;
+    bases.b[BASE_SIGMA] = (unsigned long long)(uintptr_t)sigma_dev;
+    DMRGK_CUDA(cudaMemsetAsync(sigma_dev, 0, size_t(n) * 8, main));
+    // copies of chunk c+1 are enqueued before the compute of chunk c so that they overlap it
+    const size_t nc = h->chunks.size();
+    if (nc) DMRGK_TRY(stage_chunk(h, h->chunks[0], (char*)workspace_dev, main, copy));
+    for (size_t c = 0; c < nc; ++c) {
+        const Chunk& ch = h->chunks[c];
+        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, main));
+        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, main));
+        DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, main));
+        DMRGK_TRY(chunk_done(h, ch, main));
+        if (c + 1 < nc) DMRGK_TRY(stage_chunk(h, h->chunks[c + 1], (char*)workspace_dev, main, copy));
+    }
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_heff_apply_host(dmrgk_heff* h, const double* psi_host, double* sigma_host,
+                              double* psi_dev, double* sigma_dev, void* workspace_dev,
+                              void* stream_main, void* stream_copy) {
+    if (!h) return fail(DMRGK_EINVAL, "heff_apply_host: heff is NULL");
+    const int64_t n = h->layout->n_padded;
+    if (n == 0) return DMRGK_OK;
+    if (!psi_host || !sigma_host || !psi_dev || !sigma_dev) return fail(DMRGK_EINVAL, "heff_apply_host: NULL buffer");
+    DMRGK_CUDA(cudaSetDevice(h->ctx->device));
+    cudaStream_t main = (cudaStream_t)stream_main;
+    DMRGK_CUDA(cudaMemcpyAsync(psi_dev, psi_host, size_t(n) * 8, cudaMemcpyHostToDevice, main));
+    DMRGK_TRY(dmrgk_heff_apply(h, psi_dev, sigma_dev, workspace_dev, stream_main, stream_copy));
+    DMRGK_CUDA(cudaMemcpyAsync(sigma_host, sigma_dev, size_t(n) * 8, cudaMemcpyDeviceToHost, main));
+    DMRGK_CUDA(cudaStreamSynchronize(main));
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_heff_diag(dmrgk_heff* h, double* diag_dev, void* workspace_dev, void* stream_main,
+                        void* stream_copy) {
+    if (!h) return fail(DMRGK_EINVAL, "heff_diag: heff is NULL");
+    const int64_t n = h->layout->n_padded;
+    if (n == 0) return DMRGK_OK;
+    if (!diag_dev) return fail(DMRGK_EINVAL, "heff_diag: NULL vector");
+    if (!aligned128(diag_dev) || !aligned128(workspace_dev)) return fail(DMRGK_EALIGN, "heff_diag: pointers must be 128-byte aligned");
+    if (h->has_pinned && !workspace_dev) return fail(DMRGK_EINVAL, "heff_diag: NULL workspace");
+    DMRGK_CUDA(cudaSetDevice(h->ctx->device));
+    cudaStream_t main = (cudaStream_t)stream_main, copy = (cudaStream_t)stream_copy;
+    if (h->has_pinned && copy == main)
+        return fail(DMRGK_EINVAL, "heff_diag: pinned operators need a copy stream distinct from the main stream");
+    Bases bases;
+    bases.b[BASE_ABS] = 0;
+    bases.b[BASE_WS] = (unsigned long long)(uintptr_t)workspace_dev;
+    bases.b[BASE_PSI] = 0;
+    bases.b[BASE_SIGMA] = 0;
+    DMRGK_CUDA(cudaMemsetAsync(diag_dev, 0, size_t(n) * 8, main));
+    for (const Chunk& ch : h->chunks) {
+        if (ch.d_blocks == 0) continue;
+        DMRGK_TRY(stage_chunk(h, ch, (char*)workspace_dev, main, copy));
+        DMRGK_TRY(launch_diag(h->dblocks_dev + ch.d_block0, h->dtasks_dev, ch.d_blocks, diag_dev, bases, main));
+        DMRGK_TRY(chunk_done(h, ch, main));
+    }
+    return DMRGK_OK;
+}
+
+}  // extern "C"
