@@ -168,17 +168,18 @@ int64_t dmrgk_vec_scratch_bytes(int32_t nv);
 int32_t dmrgk_vec_multi_dot(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double* X_dev,
                             int64_t stride, const double* y_dev, double* out_dev,
                             void* scratch_dev, void* stream);
-/* y[i] = beta·y[i] + Σ_j coef_dev[j]·X[j·stride + i]  (coefficients read from device memory;
- * beta = 0 overwrites without reading y). */
+/* y[i] = beta·y[i] + alpha·Σ_j coef_dev[j]·X[j·stride + i]  (coefficients read from device memory,
+ * nv ≤ 64; beta = 0 overwrites without reading y). */
 int32_t dmrgk_vec_multi_axpy(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double* X_dev,
-                             int64_t stride, const double* coef_dev, double beta, double* y_dev,
-                             void* stream);
+                             int64_t stride, const double* coef_dev, double alpha, double beta,
+                             double* y_dev, void* stream);
 /* y = alpha·x + beta·y with host scalars. */
 int32_t dmrgk_vec_axpby(dmrgk_ctx* ctx, int64_t n, double alpha, const double* x_dev, double beta,
                         double* y_dev, void* stream);
-/* x *= (*alpha_dev) if inv == 0, x /= (*alpha_dev) if inv != 0. */
-int32_t dmrgk_vec_scal_dev(dmrgk_ctx* ctx, int64_t n, const double* alpha_dev, int32_t inv,
-                           double* x_dev, void* stream);
+/* y = f·x with f from a device scalar a = *alpha_dev: mode 0: f = a, 1: f = 1/a, 2: f = sqrt(a),
+ * 3: f = 1/sqrt(a)  (normalisation by a squared norm without a host round trip).  y may alias x. */
+int32_t dmrgk_vec_scal_dev(dmrgk_ctx* ctx, int64_t n, const double* alpha_dev, int32_t mode,
+                           const double* x_dev, double* y_dev, void* stream);
 /* Davidson residual and correction (SURVEY §8(c) "Davidson, step by step"):
  *   r = Σ_j y[j]·(W_j − θ V_j);  out[0] = ‖r‖²  (y, θ from device: coef_dev[0..m) = y, coef_dev[m] = θ) */
 int32_t dmrgk_vec_residual(dmrgk_ctx* ctx, int64_t n, int32_t m, const double* V_dev,

@@ -1,0 +1,391 @@
+"""ctypes binding of libdmrgk.so — same names as include/dmrgk.h, argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; this module converts Python ints,
+NumPy arrays (host metadata) and device pointers (``torch.Tensor.data_ptr()``) into the C types of
+the ABI, checks the returned status and raises ``DmrgkError`` with ``dmrgk_last_error()``.
+There is no fallback of any kind: if the shared library is missing, ``load()`` raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "_build", "libdmrgk.so")
+
+OK, EINVAL, ESHAPE, ECHARGE, EALIGN, ENOMEM, ECUDA, ENOTCONV, ESTATE = 0, -1, -2, -3, -4, -5, -6, -7, -8
+TRANS_L, TRANS_R, IDENT_L, IDENT_R = 1, 2, 4, 8
+
+_STATUS_NAMES = {0: "OK", -1: "EINVAL", -2: "ESHAPE", -3: "ECHARGE", -4: "EALIGN", -5: "ENOMEM",
+                 -6: "ECUDA", -7: "ENOTCONV", -8: "ESTATE"}
+
+
+class DmrgkError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(f"dmrgk status {status} ({_STATUS_NAMES.get(status, '?')}): {message}")
+        self.status = status
+        self.message = message
+
+
+class HeffOpts(C.Structure):
+    _fields_ = [("t_chunk_bytes", C.c_int64), ("ring_bytes", C.c_int64), ("kernel", C.c_int32),
+                ("split_waves", C.c_int32), ("reserved", C.c_int32 * 4)]
+
+
+_p, _i32, _i64, _u64, _f64 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_double
+_pp = C.POINTER(C.c_void_p)
+_pi32, _pi64, _pf64 = C.POINTER(C.c_int32), C.POINTER(C.c_int64), C.POINTER(C.c_double)
+
+# name -> (restype, argtypes); the list of symbols include/dmrgk.h declares.
+SIGNATURES = {
+    "dmrgk_last_error": (C.c_char_p, []),
+    "dmrgk_version": (C.c_char_p, []),
+    "dmrgk_ctx_create": (_i32, [_i32, _pp]),
+    "dmrgk_ctx_destroy": (None, [_p]),
+    "dmrgk_ctx_query": (_i32, [_p, _pi32, _pi64, _pi64]),
+    "dmrgk_space_create": (_i32, [_p, _i32, _i32, _p, _p, _pp]),
+    "dmrgk_space_destroy": (None, [_p]),
+    "dmrgk_layout_create": (_i32, [_p, _p, _p, _p, _pp]),
+    "dmrgk_layout_destroy": (None, [_p]),
+    "dmrgk_layout_query": (_i32, [_p, _pi64, _pi64, _pi64]),
+    "dmrgk_layout_blocks": (_i32, [_p, _p, _p, _p, _p, _p, _p]),
+    "dmrgk_layout_pack": (_i32, [_p, _p, _p]),
+    "dmrgk_layout_unpack": (_i32, [_p, _p, _p]),
+    "dmrgk_op_create": (_i32, [_p, _p, _p, _i32, _pp]),
+    "dmrgk_op_destroy": (None, [_p]),
+    "dmrgk_op_query": (_i32, [_p, _pi64, _pi64, _pi64]),
+    "dmrgk_op_blocks": (_i32, [_p, _p, _p, _p, _p, _p, _p]),
+    "dmrgk_op_pack": (_i32, [_p, _p, _p]),
+    "dmrgk_op_bind_device": (_i32, [_p, _p]),
+    "dmrgk_op_bind_pinned": (_i32, [_p, _p]),
+    "dmrgk_heff_create": (_i32, [_p, _p, _i64, _p, _p, _p, _p, _p, _pp]),
+    "dmrgk_heff_destroy": (None, [_p]),
+    "dmrgk_heff_query": (_i32, [_p, _pi64, _pf64, _pf64, _pi64, _pi64, _pi64, _pi64]),
+    "dmrgk_heff_apply": (_i32, [_p, _p, _p, _p, _p, _p]),
+    "dmrgk_heff_apply_host": (_i32, [_p, _p, _p, _p, _p, _p, _p, _p]),
+    "dmrgk_heff_diag": (_i32, [_p, _p, _p, _p, _p]),
+    "dmrgk_vec_scratch_bytes": (_i64, [_i32]),
+    "dmrgk_vec_multi_dot": (_i32, [_p, _i64, _i32, _p, _i64, _p, _p, _p, _p]),
+    "dmrgk_vec_multi_axpy": (_i32, [_p, _i64, _i32, _p, _i64, _p, _f64, _f64, _p, _p]),
+    "dmrgk_vec_axpby": (_i32, [_p, _i64, _f64, _p, _f64, _p, _p]),
+    "dmrgk_vec_scal_dev": (_i32, [_p, _i64, _p, _i32, _p, _p, _p]),
+    "dmrgk_vec_residual": (_i32, [_p, _i64, _i32, _p, _p, _i64, _p, _p, _p, _p, _p]),
+    "dmrgk_vec_precond": (_i32, [_p, _i64, _p, _p, _p, _p, _p]),
+    "dmrgk_davidson_extra_bytes": (_i64, [_i32, _i64]),
+    "dmrgk_davidson_create": (_i32, [_p, _i32, _f64, _i32, _p, _p, _p, _p, _p, _p, _pp]),
+    "dmrgk_davidson_destroy": (None, [_p]),
+    "dmrgk_davidson_start": (_i32, [_p, _p]),
+    "dmrgk_davidson_step": (_i32, [_p, _pf64, _pf64, _pi32]),
+    "dmrgk_davidson_solve": (_i32, [_p, _pf64, _pf64, _p, _pi32]),
+    "dmrgk_davidson_query": (_i32, [_p, _pi32, _pi32]),
+    "dmrgk_op_fill_normal": (_i32, [_p, _p, _u64, _u64, _i32, _i32, _p]),
+    "dmrgk_layout_fill_normal": (_i32, [_p, _p, _u64, _u64, _p]),
+    "dmrgk_probe_fp64": (_i32, [_p, _i32, _i64, _p, _pf64, _p]),
+}
+
+_lib = None
+
+
+def load(path=None):
+    """dlopen libdmrgk.so and declare every prototype.  Raises if the library is not built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise FileNotFoundError(
+            f"{path} not found: build it with `python -m paper_2311_14106_b200.build` "
+            "(dmrgk has no CPU or PyTorch fallback)")
+    lib = C.CDLL(path)
+    for name, (res, args) in SIGNATURES.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def last_error():
+    return load().dmrgk_last_error().decode("utf-8", "replace")
+
+
+def check(status):
+    if status != OK:
+        raise DmrgkError(status, last_error())
+
+
+def _dev(t):
+    """Device pointer of a torch tensor (or a raw int / None)."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    return t.data_ptr()
+
+
+def _stream(s):
+    if s is None:
+        return None
+    if isinstance(s, int):
+        return s
+    return s.cuda_stream
+
+
+def _i32arr(x):
+    return np.ascontiguousarray(np.asarray(x, dtype=np.int32))
+
+
+class Ctx:
+    def __init__(self, device=0):
+        self.lib = load()
+        h = C.c_void_p()
+        check(self.lib.dmrgk_ctx_create(device, C.byref(h)))
+        self.h = h
+        self.device = device
+
+    def query(self):
+        n_sm, l2, hbm = C.c_int32(), C.c_int64(), C.c_int64()
+        check(self.lib.dmrgk_ctx_query(self.h, C.byref(n_sm), C.byref(l2), C.byref(hbm)))
+        return n_sm.value, l2.value, hbm.value
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.dmrgk_ctx_destroy(self.h)
+            self.h = None
+
+
+class Space:
+    """dmrgk_space: sectors = [(charge tuple, dim)]."""
+
+    def __init__(self, ctx, n_charges, sectors):
+        self.ctx, self.lib = ctx, ctx.lib
+        self.sectors = list(sectors)
+        q = _i32arr([list(s[0]) for s in sectors]).reshape(-1)
+        d = _i32arr([s[1] for s in sectors])
+        h = C.c_void_p()
+        check(self.lib.dmrgk_space_create(ctx.h, n_charges, len(sectors), q.ctypes.data, d.ctypes.data, C.byref(h)))
+        self.h = h
+        self.n_charges = n_charges
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.dmrgk_space_destroy(self.h)
+            self.h = None
+
+
+class _Blocked:
+    """Shared query helpers of Layout and Op (block table as NumPy arrays)."""
+    _query = _blocks = None
+
+    def query(self):
+        nb, ne, npad = C.c_int64(), C.c_int64(), C.c_int64()
+        check(getattr(self.lib, self._query)(self.h, C.byref(nb), C.byref(ne), C.byref(npad)))
+        return nb.value, ne.value, npad.value
+
+    def blocks(self):
+        nb = self.query()[0]
+        r, c, rows, cols, ld = (np.zeros(nb, np.int32) for _ in range(5))
+        off = np.zeros(nb, np.int64)
+        check(getattr(self.lib, self._blocks)(self.h, r.ctypes.data, c.ctypes.data, rows.ctypes.data,
+                                              cols.ctypes.data, ld.ctypes.data, off.ctypes.data))
+        return r, c, rows, cols, ld, off
+
+
+class Layout(_Blocked):
+    _query, _blocks = "dmrgk_layout_query", "dmrgk_layout_blocks"
+
+    def __init__(self, ctx, A, B, target):
+        self.ctx, self.lib, self.A, self.B = ctx, ctx.lib, A, B
+        t = _i32arr(list(target))
+        h = C.c_void_p()
+        check(self.lib.dmrgk_layout_create(ctx.h, A.h, B.h, t.ctypes.data, C.byref(h)))
+        self.h = h
+        self.n_blocks, self.n_elems, self.n_padded = self.query()
+
+    def pack(self, unpadded):
+        u = np.ascontiguousarray(unpadded, dtype=np.float64)
+        assert u.size == self.n_elems
+        p = np.zeros(self.n_padded, np.float64)
+        check(self.lib.dmrgk_layout_pack(self.h, u.ctypes.data, p.ctypes.data))
+        return p
+
+    def unpack(self, packed):
+        p = np.ascontiguousarray(packed, dtype=np.float64)
+        assert p.size == self.n_padded
+        u = np.zeros(self.n_elems, np.float64)
+        check(self.lib.dmrgk_layout_unpack(self.h, p.ctypes.data, u.ctypes.data))
+        return u
+
+    def fill_normal(self, arena, seed, stream_id, stream=None):
+        check(self.lib.dmrgk_layout_fill_normal(self.h, _dev(arena), seed, stream_id, _stream(stream)))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.dmrgk_layout_destroy(self.h)
+            self.h = None
+
+
+class Op(_Blocked):
+    _query, _blocks = "dmrgk_op_query", "dmrgk_op_blocks"
+
+    def __init__(self, ctx, space, dq, parity):
+        self.ctx, self.lib, self.space = ctx, ctx.lib, space
+        d = _i32arr(list(dq))
+        h = C.c_void_p()
+        check(self.lib.dmrgk_op_create(ctx.h, space.h, d.ctypes.data, int(parity), C.byref(h)))
+        self.h = h
+        self.n_blocks, self.n_elems, self.n_padded = self.query()
+        self._keep = None
+
+    def pack(self, unpadded):
+        u = np.ascontiguousarray(unpadded, dtype=np.float64)
+        assert u.size == self.n_elems
+        p = np.zeros(self.n_padded, np.float64)
+        check(self.lib.dmrgk_op_pack(self.h, u.ctypes.data, p.ctypes.data))
+        return p
+
+    def bind_device(self, arena):
+        check(self.lib.dmrgk_op_bind_device(self.h, _dev(arena)))
+        self._keep = arena
+
+    def bind_pinned(self, arena):
+        check(self.lib.dmrgk_op_bind_pinned(self.h, _dev(arena)))
+        self._keep = arena
+
+    def fill_normal(self, arena, seed, stream_id, scale_mode, symmetric, stream=None):
+        check(self.lib.dmrgk_op_fill_normal(self.h, _dev(arena), seed, stream_id, int(scale_mode),
+                                            int(bool(symmetric)), _stream(stream)))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.dmrgk_op_destroy(self.h)
+            self.h = None
+
+
+class Heff:
+    """dmrgk_heff: terms = [(L Op or None, R Op or None, coef, trans_L, trans_R)]."""
+
+    def __init__(self, ctx, layout, terms, t_chunk_bytes=0, ring_bytes=0, kernel=0, split_waves=0):
+        self.ctx, self.lib, self.layout = ctx, ctx.lib, layout
+        K = len(terms)
+        Larr = (C.c_void_p * max(K, 1))()
+        Rarr = (C.c_void_p * max(K, 1))()
+        coef = np.zeros(max(K, 1), np.float64)
+        flags = np.zeros(max(K, 1), np.uint32)
+        self._ops = []
+        for k, (L, R, c, tL, tR) in enumerate(terms):
+            Larr[k] = L.h if L is not None else None
+            Rarr[k] = R.h if R is not None else None
+            coef[k] = c
+            flags[k] = ((TRANS_L if tL else 0) | (TRANS_R if tR else 0) |
+                        (IDENT_L if L is None else 0) | (IDENT_R if R is None else 0))
+            self._ops += [L, R]
+        opts = HeffOpts(int(t_chunk_bytes), int(ring_bytes), int(kernel), int(split_waves))
+        h = C.c_void_p()
+        check(self.lib.dmrgk_heff_create(ctx.h, layout.h, K, Larr, Rarr, coef.ctypes.data, flags.ctypes.data,
+                                         C.byref(opts), C.byref(h)))
+        self.h = h
+        q = self.query()
+        self.n_tasks, self.flops_alg, self.flops_exec = q["n_tasks"], q["flops_alg"], q["flops_exec"]
+        self.op_bytes, self.workspace_bytes = q["op_bytes"], q["workspace_bytes"]
+        self.n_chunks, self.n_launches = q["n_chunks"], q["n_launches"]
+
+    def query(self):
+        nt, ob, wb, nc, nl = (C.c_int64() for _ in range(5))
+        fa, fe = C.c_double(), C.c_double()
+        check(self.lib.dmrgk_heff_query(self.h, C.byref(nt), C.byref(fa), C.byref(fe), C.byref(ob), C.byref(wb),
+                                        C.byref(nc), C.byref(nl)))
+        return {"n_tasks": nt.value, "flops_alg": fa.value, "flops_exec": fe.value, "op_bytes": ob.value,
+                "workspace_bytes": wb.value, "n_chunks": nc.value, "n_launches": nl.value}
+
+    def apply(self, psi, sigma, workspace, stream_main=None, stream_copy=None):
+        check(self.lib.dmrgk_heff_apply(self.h, _dev(psi), _dev(sigma), _dev(workspace), _stream(stream_main),
+                                        _stream(stream_copy)))
+
+    def apply_host(self, psi_host, sigma_host, psi, sigma, workspace, stream_main=None, stream_copy=None):
+        check(self.lib.dmrgk_heff_apply_host(self.h, _dev(psi_host), _dev(sigma_host), _dev(psi), _dev(sigma),
+                                             _dev(workspace), _stream(stream_main), _stream(stream_copy)))
+
+    def diag(self, diag, workspace, stream_main=None, stream_copy=None):
+        check(self.lib.dmrgk_heff_diag(self.h, _dev(diag), _dev(workspace), _stream(stream_main),
+                                       _stream(stream_copy)))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.dmrgk_heff_destroy(self.h)
+            self.h = None
+
+
+class Davidson:
+    def __init__(self, heff, m_max, tol, max_iter, V, W, diag, workspace, stream_main=None, stream_copy=None):
+        self.lib, self.heff = heff.lib, heff
+        self._keep = (V, W, diag, workspace, stream_main, stream_copy)
+        h = C.c_void_p()
+        check(self.lib.dmrgk_davidson_create(heff.h, m_max, tol, max_iter, _dev(V), _dev(W), _dev(diag),
+                                             _dev(workspace), _stream(stream_main), _stream(stream_copy),
+                                             C.byref(h)))
+        self.h = h
+
+    def start(self, x0):
+        check(self.lib.dmrgk_davidson_start(self.h, _dev(x0)))
+
+    def step(self):
+        th, rn, cv = C.c_double(), C.c_double(), C.c_int32()
+        check(self.lib.dmrgk_davidson_step(self.h, C.byref(th), C.byref(rn), C.byref(cv)))
+        return th.value, rn.value, bool(cv.value)
+
+    def solve(self, x=None):
+        th, rn, na = C.c_double(), C.c_double(), C.c_int32()
+        st = self.lib.dmrgk_davidson_solve(self.h, C.byref(th), C.byref(rn), _dev(x), C.byref(na))
+        if st not in (OK, ENOTCONV):
+            check(st)
+        return th.value, rn.value, na.value, st == OK
+
+    def query(self):
+        m, na = C.c_int32(), C.c_int32()
+        check(self.lib.dmrgk_davidson_query(self.h, C.byref(m), C.byref(na)))
+        return m.value, na.value
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.dmrgk_davidson_destroy(self.h)
+            self.h = None
+
+
+def davidson_extra_bytes(m_max, n_padded):
+    return load().dmrgk_davidson_extra_bytes(m_max, n_padded)
+
+
+def vec_scratch_bytes(nv):
+    return load().dmrgk_vec_scratch_bytes(nv)
+
+
+def vec_multi_dot(ctx, n, nv, X, stride, y, out, scratch, stream=None):
+    check(ctx.lib.dmrgk_vec_multi_dot(ctx.h, n, nv, _dev(X), stride, _dev(y), _dev(out), _dev(scratch), _stream(stream)))
+
+
+def vec_multi_axpy(ctx, n, nv, X, stride, coef, alpha, beta, y, stream=None):
+    check(ctx.lib.dmrgk_vec_multi_axpy(ctx.h, n, nv, _dev(X), stride, _dev(coef), alpha, beta, _dev(y), _stream(stream)))
+
+
+def vec_axpby(ctx, n, alpha, x, beta, y, stream=None):
+    check(ctx.lib.dmrgk_vec_axpby(ctx.h, n, alpha, _dev(x), beta, _dev(y), _stream(stream)))
+
+
+def vec_scal_dev(ctx, n, alpha_dev, mode, x, y, stream=None):
+    check(ctx.lib.dmrgk_vec_scal_dev(ctx.h, n, _dev(alpha_dev), mode, _dev(x), _dev(y), _stream(stream)))
+
+
+def vec_residual(ctx, n, m, V, W, stride, coef, r, out, scratch, stream=None):
+    check(ctx.lib.dmrgk_vec_residual(ctx.h, n, m, _dev(V), _dev(W), stride, _dev(coef), _dev(r), _dev(out),
+                                     _dev(scratch), _stream(stream)))
+
+
+def vec_precond(ctx, n, r, diag, theta_dev, t, stream=None):
+    check(ctx.lib.dmrgk_vec_precond(ctx.h, n, _dev(r), _dev(diag), _dev(theta_dev), _dev(t), _stream(stream)))
+
+
+def probe_fp64(ctx, kind, iters, sink, stream=None):
+    fl = C.c_double()
+    check(ctx.lib.dmrgk_probe_fp64(ctx.h, kind, iters, _dev(sink), C.byref(fl), _stream(stream)))
+    return fl.value

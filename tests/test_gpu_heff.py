@@ -1,0 +1,240 @@
+"""-m gpu parity: σ = H_eff ψ from the CUDA library (through the C ABI) against the oracle,
+element by element on the same seeded inputs (BASELINE.json: relative max-norm ≤ 1e-11)."""
+import numpy as np
+import pytest
+
+import workloads as wlmod
+from oracle import heff, lattice, dmrg, export
+from _gpu import device_problem, rel_max, padding_is_zero, config1_problem, TOL_SIGMA
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def small_config2():
+    return wlmod.synthetic_config2(M=64, n_q=9, K=32, seed=2, width2=8.0)
+
+
+def medium_config2():
+    # several 64×64 tiles per block, ragged tails (sector sizes 1 … 100), split-k exercised
+    return wlmod.synthetic_config2(M=400, n_q=13, K=40, seed=12, width2=10.0)
+
+
+def small_spinless():
+    return wlmod.lattice_workload("spinless", 5, 24, seed=3)
+
+
+def medium_spinless():
+    thin = lambda fam, i: fam in ("F1", "F2") or i % 5 == 0
+    return wlmod.lattice_workload("spinless", 10, 600, seed=13, width2=4.0, keep=thin)
+
+
+def small_hubbard():
+    thin = lambda fam, i: fam in ("F1", "F2") or i % 3 == 0
+    return wlmod.lattice_workload("hubbard", 2, 14, seed=4, keep=thin)
+
+
+def medium_hubbard():
+    thin = lambda fam, i: fam in ("F1", "F2") or i % 7 == 0
+    return wlmod.lattice_workload("hubbard", 5, 400, seed=14, keep=thin)
+
+
+@pytest.mark.parametrize("make", [small_config2, small_spinless, small_hubbard])
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_sigma_vs_dense_kronecker(make, kernel):
+    """T2: H_eff assembled densely by explicit Kronecker products with Jordan–Wigner signs."""
+    pb = heff.problem_from_workload(make())
+    ref = heff.sigma_dense(pb)
+    dp = device_problem(pb, kernel=kernel)
+    psi = dp.psi_from_host(pb.psi)
+    sigma = dp.apply(psi)
+    assert rel_max(dp.to_blocks(sigma), ref) <= TOL_SIGMA
+    assert padding_is_zero(dp, sigma)
+    assert dp.heff.flops_alg == heff.flops_alg(pb)
+    assert dp.heff.n_tasks == len(heff.enumerate_tasks(pb))
+
+
+@pytest.mark.parametrize("make", [medium_config2, medium_spinless, medium_hubbard])
+@pytest.mark.parametrize("opts", [{}, {"split_waves": 64}, {"t_chunk_bytes": 1 << 20}])
+def test_sigma_vs_blockwise_medium(make, opts):
+    """T3 at sizes spanning several tiles and ragged tails; split-k and chunking variants."""
+    pb = heff.problem_from_workload(make())
+    ref = heff.sigma_blockwise(pb)
+    dp = device_problem(pb, **opts)
+    sigma = dp.apply(dp.psi_from_host(pb.psi))
+    assert rel_max(dp.to_blocks(sigma), ref) <= TOL_SIGMA
+    assert padding_is_zero(dp, sigma)
+    if "t_chunk_bytes" in opts:
+        assert dp.heff.n_chunks > 1
+
+
+def test_device_fill_matches_host_generator():
+    """The library's seeded fill kernel reproduces workloads.fill_op_host bit for bit, so
+    device-generated arenas and the oracle's host blocks are the same inputs."""
+    from paper_2311_14106_b200 import problem
+    for wl in (small_config2(), small_spinless(), small_hubbard()):
+        dp = problem.from_workload(wl)
+        for i in range(len(wl.ops)):
+            host = wlmod.fill_op_host(wl, i)
+            dev = dp.read_op_blocks(i)
+            assert set(host) == set(dev)
+            for k in host:
+                assert np.array_equal(host[k], dev[k]), (wl.name, i, k)
+        psi = dp.to_blocks(dp.psi_fill(wl.seed, wlmod.PSI_STREAM))
+        ref = wlmod.fill_psi_host(wl)
+        for k in ref:
+            assert np.array_equal(psi[k], ref[k])
+
+
+def test_config2_full_size():
+    """BASELINE.json configs[1] (M=1024, 33 sectors, K=512) against T3, all blocks."""
+    from paper_2311_14106_b200 import problem
+    wl = wlmod.synthetic_config2()
+    pb = heff.problem_from_workload(wl)
+    ref = heff.sigma_blockwise(pb)
+    dp = problem.from_workload(wl)
+    sigma = dp.apply(dp.psi_fill(wl.seed, wlmod.PSI_STREAM))
+    assert rel_max(dp.to_blocks(sigma), ref) <= TOL_SIGMA
+    assert dp.heff.flops_alg == heff.flops_alg(pb)
+
+
+@pytest.fixture(scope="module")
+def config1():
+    return config1_problem()
+
+
+def test_config1_sigma_vs_definition_and_kronecker(config1):
+    """σ_gpu vs P†HP ψ (T1, the definition) and vs the dense Kronecker H_eff (T2)."""
+    pb, Heff, x, space = config1
+    dp = device_problem(pb)
+    sigma = dp.to_blocks(dp.apply(dp.psi_from_host(pb.psi)))
+    ref1 = dmrg.vec_to_blocks(space, Heff @ x)
+    assert rel_max(sigma, ref1) <= TOL_SIGMA
+    assert rel_max(sigma, heff.sigma_dense(pb)) <= TOL_SIGMA
+
+
+def test_hermiticity_and_linearity():
+    """⟨x, Hy⟩ = ⟨Hx, y⟩ pins the h.c. pairing and the fermionic sign rule; σ is linear in ψ."""
+    from paper_2311_14106_b200 import problem
+    wl = medium_hubbard()
+    dp = problem.from_workload(wl)
+    n = dp.layout.n_padded
+    x = dp.psi_fill(wl.seed, 101)
+    y = dp.psi_fill(wl.seed, 102)
+    Hx, Hy = dp.apply(x), dp.apply(y)
+    a, b = torch.dot(x[:n], Hy[:n]).item(), torch.dot(Hx[:n], y[:n]).item()
+    scale = torch.linalg.norm(Hx[:n]).item() * torch.linalg.norm(y[:n]).item()
+    assert abs(a - b) <= 1e-12 * scale
+    z = (0.3 * x - 1.7 * y).contiguous()
+    Hz = dp.apply(z)
+    ref = 0.3 * Hx - 1.7 * Hy
+    assert (Hz - ref).abs().max().item() <= 1e-12 * ref.abs().max().item()
+
+
+def test_block_support_single_block_input():
+    """ψ supported on one block reaches only blocks shifted by some δ_k (charge conservation)."""
+    wl = small_spinless()
+    pb = heff.problem_from_workload(wl)
+    keys = pb.psi_blocks()
+    mid = keys[len(keys) // 2]
+    psi = {k: (v if k == mid else np.zeros_like(v)) for k, v in pb.psi.items()}
+    ref = heff.sigma_blockwise(pb, psi)
+    dp = device_problem(pb)
+    got = dp.to_blocks(dp.apply(dp.psi_from_host(psi)))
+    assert rel_max(got, ref) <= TOL_SIGMA
+    for k in ref:
+        if not np.any(ref[k]):
+            assert not np.any(got[k])
+
+
+def test_k_additivity():
+    """σ(K list) = σ(first half) + σ(second half)."""
+    pb = heff.problem_from_workload(medium_config2())
+    dp = device_problem(pb)
+    psi = dp.psi_from_host(pb.psi)
+    full = dp.apply(psi).clone()
+    K = len(pb.terms)
+    parts = []
+    for sl in (slice(0, K // 2), slice(K // 2, K)):
+        dp.build(pb.terms[sl])
+        parts.append(dp.apply(psi).clone())
+    s = parts[0] + parts[1]
+    assert (full - s).abs().max().item() <= 1e-12 * full.abs().max().item()
+
+
+def test_diag_matches_oracle():
+    for make in (small_config2, medium_spinless, small_hubbard):
+        pb = heff.problem_from_workload(make())
+        dp = device_problem(pb)
+        got = dp.to_blocks(dp.diag())
+        ref = heff.diagonal_blockwise(pb)
+        assert rel_max(got, ref) <= 1e-13
+
+
+def test_staged_operators_bit_identical_to_resident():
+    """a3: operators streamed from pinned host memory through the ring give the same bits."""
+    from paper_2311_14106_b200 import problem
+    wl = medium_spinless()
+    res = problem.from_workload(wl)
+    psi = res.psi_fill(wl.seed, wlmod.PSI_STREAM)
+    ref = res.apply(psi).clone()
+    pinned = [i for i in range(len(wl.ops)) if i % 3 == 1]
+    stg = problem.from_workload(wl, pinned=pinned, ring_bytes=1 << 20, t_chunk_bytes=1 << 20)
+    assert stg.heff.n_chunks > 2
+    for _ in range(2):      # second call re-uses the ring halves
+        got = stg.apply(stg.psi_fill(wl.seed, wlmod.PSI_STREAM))
+        torch.cuda.synchronize()
+        assert torch.equal(got, ref)
+    assert torch.equal(stg.diag(), res.diag())
+
+
+def test_apply_host_end_to_end():
+    wl = medium_config2()
+    pb = heff.problem_from_workload(wl)
+    dp = device_problem(pb)
+    psi_dev = dp.psi_from_host(pb.psi)
+    ref = dp.apply(psi_dev).clone()
+    n = dp.layout.n_padded
+    ph = psi_dev[:n].cpu().pin_memory()
+    sh = torch.empty(n, dtype=torch.float64).pin_memory()
+    dp.heff.apply_host(ph, sh, dp.new_vector(), dp.new_vector(), dp.workspace, dp.stream, dp.copy_stream)
+    assert torch.equal(sh, ref[:n].cpu())
+
+
+def test_edge_cases_and_errors():
+    from paper_2311_14106_b200 import dmrgk, problem
+    sec = [((q,), d) for q, d in enumerate([1, 3, 0, 17, 2])]
+    # K = 0: σ = 0
+    dp = problem.DeviceProblem(1, sec, sec, (4,))
+    dp.create_ops([])
+    dp.build([])
+    sigma = dp.apply(dp.psi_fill(1, 7))
+    assert dp.heff.n_tasks == 0 and not torch.any(sigma)
+    # no allowed block: apply is a no-op, Davidson refuses
+    empty = problem.DeviceProblem(1, sec, sec, (99,))
+    assert empty.layout.n_blocks == 0
+    empty.create_ops([])
+    empty.build([])
+    empty.apply(empty.new_vector())
+    # shifts that do not cancel / parity mismatch / wrong space / unbound
+    dp.create_ops([("A", (1,), 1), ("B", (1,), 1), ("B", (-1,), 0), ("A", (-1,), 1)])
+    dp.alloc_resident()
+    for terms, code in (([(0, 1, 1.0, False, False)], dmrgk.ECHARGE),
+                        ([(0, 2, 1.0, False, False)], dmrgk.ECHARGE),
+                        ([(0, 3, 1.0, False, False)], dmrgk.ESHAPE)):
+        with pytest.raises(dmrgk.DmrgkError) as e:
+            dp.build(terms)
+        assert e.value.status == code
+    dp.build([(0, 1, 1.0, False, True)])        # transposing R makes the shifts cancel
+    unb = dmrgk.Op(dp.ctx, dp.A, (1,), 1)
+    with pytest.raises(dmrgk.DmrgkError) as e:
+        dmrgk.Heff(dp.ctx, dp.layout, [(unb, dp.ops[1], 1.0, False, True)])
+    assert e.value.status == dmrgk.ESTATE
+    # misaligned pointers
+    v = dp.new_vector()
+    with pytest.raises(dmrgk.DmrgkError) as e:
+        dp.heff.apply(v.data_ptr() + 8, v, dp.workspace)
+    assert e.value.status == dmrgk.EALIGN
+    with pytest.raises(dmrgk.DmrgkError) as e:
+        dp.heff.apply(v, v, dp.workspace)
+    assert e.value.status == dmrgk.EINVAL
