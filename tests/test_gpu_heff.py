@@ -179,7 +179,7 @@ def test_staged_operators_bit_identical_to_resident():
     psi = res.psi_fill(wl.seed, wlmod.PSI_STREAM)
     ref = res.apply(psi).clone()
     pinned = [i for i in range(len(wl.ops)) if i % 3 == 1]
-    stg = problem.from_workload(wl, pinned=pinned, ring_bytes=1 << 20, t_chunk_bytes=1 << 20)
+    stg = problem.from_workload(wl, pinned=pinned, ring_bytes=4 << 20, t_chunk_bytes=1 << 20)
     assert stg.heff.n_chunks > 2
     for _ in range(2):      # second call re-uses the ring halves
         got = stg.apply(stg.psi_fill(wl.seed, wlmod.PSI_STREAM))
