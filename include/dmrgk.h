@@ -62,6 +62,10 @@ const char* dmrgk_last_error(void);
 /* Library version string, e.g. "dmrgk 0.1 sm_100a". */
 const char* dmrgk_version(void);
 
+/* Number of CUDA kernels this library has launched in the calling process so far (every launch site
+ * counts; memcpys/memsets do not).  reset != 0 returns the count and zeroes it. */
+int64_t dmrgk_launch_count(int32_t reset);
+
 /* ---- context ------------------------------------------------------------------------------ */
 /* Binds the library to CUDA device `device` (cudaSetDevice on every call that launches work).
  * Fails with DMRGK_ECUDA when no device is present: there is no CPU fallback. */
@@ -159,6 +163,14 @@ int32_t dmrgk_heff_apply_host(dmrgk_heff* h, const double* psi_host, double* sig
  * coef·sign·L[i,i]·R[j,j].  Pinned operators are read through the ring like in apply. */
 int32_t dmrgk_heff_diag(dmrgk_heff* h, double* diag_dev, void* workspace_dev, void* stream_main,
                         void* stream_copy);
+
+/* Measurement aid: with enable != 0 every later heff_apply brackets each of its
+ * kernel launches with a CUDA event pair on stream_main; enable (either value) zeroes the sums.
+ * profile_read synchronises on the recorded events and returns the accumulated device time in ms
+ * and the launch counts since the last enable, as ms[3] / launches[3] =
+ * {phase-1 GEMM (a5), phase-2 GEMM (a6), split-k reduce (a7)}.  Either pointer may be NULL. */
+int32_t dmrgk_heff_profile(dmrgk_heff* h, int32_t enable);
+int32_t dmrgk_heff_profile_read(dmrgk_heff* h, double* ms, int64_t* launches);
 
 /* ---- a8: vector kernels over the flat padded arena (n doubles) ---------------------------- */
 /* Reductions are two-stage and fixed-order (bit-reproducible); scratch_dev needs

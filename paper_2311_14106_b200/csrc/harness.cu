@@ -62,6 +62,7 @@ static int32_t fill(const DevBlock* table, const std::vector<Block>& blocks, dou
         for (size_t i = b0; i < b0 + nb; ++i) biggest = std::max<int64_t>(biggest, int64_t(blocks[i].rows) * blocks[i].ld);
         const unsigned gx = unsigned(std::max<int64_t>(1, std::min<int64_t>(1024, (biggest + 255) / 256)));
         fill_normal_kernel<<<dim3(gx, nb), 256, 0, st>>>(table + b0, arena, base, scale_mode, symmetric);
+        count_launch();
         DMRGK_CUDA(cudaGetLastError());
     }
     return DMRGK_OK;
@@ -130,9 +131,11 @@ int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* si
     const int blocks = ctx->n_sm * 4, threads = 256;
     if (kind == 0) {
         probe_dmma_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(iters, sink_dev);
+        count_launch();
         if (flops) *flops = double(blocks) * (threads / 32) * double(iters) * 16.0 * 512.0;
     } else if (kind == 1) {
         probe_dfma_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(iters, sink_dev);
+        count_launch();
         if (flops) *flops = double(blocks) * threads * double(iters) * 32.0 * 2.0;
     } else {
         return fail(DMRGK_EINVAL, "probe_fp64: kind must be 0 (DMMA) or 1 (DFMA)");

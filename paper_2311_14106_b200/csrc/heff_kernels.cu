@@ -324,6 +324,7 @@ int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev
         heff_gemm_scalar_kernel<<<unsigned(n_units), NTHREADS, 0, st>>>(units_dev, segs_dev, bases);
     else
         heff_gemm_dmma_kernel<<<unsigned(n_units), NTHREADS, SMEM_BYTES, st>>>(units_dev, segs_dev, bases);
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }
@@ -331,6 +332,7 @@ int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev
 int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cudaStream_t st) {
     if (n <= 0) return DMRGK_OK;
     heff_reduce_kernel<<<unsigned(n), 256, 0, st>>>(runits_dev, bases);
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }
@@ -340,6 +342,7 @@ int32_t launch_diag(const DiagBlock* blocks_dev, const DiagTask* tasks_dev, int6
     if (n_blocks <= 0) return DMRGK_OK;
     dim3 grid(64, unsigned(n_blocks));
     heff_diag_kernel<<<grid, 256, 0, st>>>(blocks_dev, tasks_dev, diag, bases);
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }

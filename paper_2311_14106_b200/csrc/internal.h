@@ -24,6 +24,9 @@ int32_t fail(int32_t code, const char* fmt, ...);
         if (s__ != DMRGK_OK) return s__;                                                         \
     } while (0)
 
+// Number of kernels the library has launched in this process (dmrgk_launch_count).
+void count_launch(int64_t n = 1);
+
 static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 static inline bool aligned128(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 127u) == 0; }
 
@@ -202,4 +205,11 @@ struct dmrgk_heff {
     cudaEvent_t ev_copy[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
     int64_t n_launches = 0;
     bool has_pinned = false;
+    // optional per-kernel timing (dmrgk_heff_profile): event pairs around every launch of apply
+    bool prof_on = false;
+    std::vector<cudaEvent_t> prof_ev;      // pool, two per launch
+    std::vector<int> prof_kind;            // per recorded pair: 0 phase 1, 1 phase 2, 2 reduce
+    size_t prof_used = 0;                  // pairs recorded since the last read
+    double prof_ms[3] = {0, 0, 0};
+    int64_t prof_launches[3] = {0, 0, 0};
 };

@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <atomic>
 #include <new>
 
 namespace dmrgk {
@@ -18,6 +19,9 @@ int32_t fail(int32_t code, const char* fmt, ...) {
     va_end(ap);
     return code;
 }
+
+static std::atomic<long long> g_launches{0};
+void count_launch(int64_t n) { g_launches.fetch_add((long long)n, std::memory_order_relaxed); }
 
 static int32_t upload_table(const std::vector<Block>& blocks, DevBlock** out) {
     *out = nullptr;
@@ -52,6 +56,9 @@ extern "C" {
 
 const char* dmrgk_last_error(void) { return g_err; }
 const char* dmrgk_version(void) { return "dmrgk 0.1 sm_100a"; }
+int64_t dmrgk_launch_count(int32_t reset) {
+    return reset ? g_launches.exchange(0) : g_launches.load();
+}
 
 int32_t dmrgk_ctx_create(int32_t device, dmrgk_ctx** out) {
     if (!out) return fail(DMRGK_EINVAL, "ctx_create: out is NULL");

@@ -63,6 +63,7 @@ void dmrgk_heff_destroy(dmrgk_heff* h) {
         if (h->ev_copy[i]) cudaEventDestroy(h->ev_copy[i]);
         if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
     }
+    for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
     delete h;
 }
 
@@ -534,6 +535,38 @@ static int32_t stage_chunk(dmrgk_heff* h, const Chunk& c, char* ws, cudaStream_t
     return DMRGK_OK;
 }
 
+// Profiling (dmrgk_heff_profile): an event pair around one launch; the pool grows on demand.
+static int32_t prof_begin(dmrgk_heff* h, int kind, cudaStream_t main) {
+    if (!h->prof_on) return DMRGK_OK;
+    while (h->prof_ev.size() < 2 * (h->prof_used + 1)) {
+        cudaEvent_t e;
+        DMRGK_CUDA(cudaEventCreate(&e));
+        h->prof_ev.push_back(e);
+    }
+    if (h->prof_kind.size() <= h->prof_used) h->prof_kind.resize(h->prof_used + 1);
+    h->prof_kind[h->prof_used] = kind;
+    DMRGK_CUDA(cudaEventRecord(h->prof_ev[2 * h->prof_used], main));
+    return DMRGK_OK;
+}
+static int32_t prof_end(dmrgk_heff* h, cudaStream_t main) {
+    if (!h->prof_on) return DMRGK_OK;
+    DMRGK_CUDA(cudaEventRecord(h->prof_ev[2 * h->prof_used + 1], main));
+    ++h->prof_used;
+    return DMRGK_OK;
+}
+// Fold the recorded pairs into the running sums (synchronises on the last event).
+static int32_t prof_collect(dmrgk_heff* h) {
+    for (size_t i = 0; i < h->prof_used; ++i) {
+        DMRGK_CUDA(cudaEventSynchronize(h->prof_ev[2 * i + 1]));
+        float ms = 0.f;
+        DMRGK_CUDA(cudaEventElapsedTime(&ms, h->prof_ev[2 * i], h->prof_ev[2 * i + 1]));
+        h->prof_ms[h->prof_kind[i]] += ms;
+        ++h->prof_launches[h->prof_kind[i]];
+    }
+    h->prof_used = 0;
+    return DMRGK_OK;
+}
+
 static int32_t chunk_done(dmrgk_heff* h, const Chunk& c, cudaStream_t main) {
     if (c.copies.empty()) return DMRGK_OK;
     DMRGK_CUDA(cudaEventRecord(h->ev_done[c.ring_half], main));
@@ -570,11 +603,44 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
     if (nc) DMRGK_TRY(stage_chunk(h, h->chunks[0], (char*)workspace_dev, main, copy));
     for (size_t c = 0; c < nc; ++c) {
         const Chunk& ch = h->chunks[c];
-        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, main));
-        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, main));
-        DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, main));
+        if (ch.p1_units) {
+            DMRGK_TRY(prof_begin(h, 0, main));
+            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, main));
+            DMRGK_TRY(prof_end(h, main));
+        }
+        if (ch.p2_units) {
+            DMRGK_TRY(prof_begin(h, 1, main));
+            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, main));
+            DMRGK_TRY(prof_end(h, main));
+        }
+        if (ch.r_units) {
+            DMRGK_TRY(prof_begin(h, 2, main));
+            DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, main));
+            DMRGK_TRY(prof_end(h, main));
+        }
         DMRGK_TRY(chunk_done(h, ch, main));
         if (c + 1 < nc) DMRGK_TRY(stage_chunk(h, h->chunks[c + 1], (char*)workspace_dev, main, copy));
+    }
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_heff_profile(dmrgk_heff* h, int32_t enable) {
+    if (!h) return fail(DMRGK_EINVAL, "heff_profile: heff is NULL");
+    if (h->prof_used) DMRGK_TRY(prof_collect(h));
+    h->prof_on = enable != 0;
+    for (int i = 0; i < 3; ++i) {
+        h->prof_ms[i] = 0.0;
+        h->prof_launches[i] = 0;
+    }
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_heff_profile_read(dmrgk_heff* h, double* ms, int64_t* launches) {
+    if (!h) return fail(DMRGK_EINVAL, "heff_profile_read: heff is NULL");
+    DMRGK_TRY(prof_collect(h));
+    for (int i = 0; i < 3; ++i) {
+        if (ms) ms[i] = h->prof_ms[i];
+        if (launches) launches[i] = h->prof_launches[i];
     }
     return DMRGK_OK;
 }

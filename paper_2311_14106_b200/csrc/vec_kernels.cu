@@ -200,6 +200,7 @@ static void launch_dot1(int grid, cudaStream_t st, int64_t n2, int nv, int j0, c
                         const double* y, double* partial, int nv_total) {
     multi_dot_stage1<NV><<<grid, VEC_THREADS, 0, st>>>(n2, nv, j0, reinterpret_cast<const double2*>(X), stride / 2,
                                                        reinterpret_cast<const double2*>(y), partial, nv_total);
+    count_launch();
 }
 
 }  // namespace dmrgk
@@ -235,6 +236,7 @@ int32_t dmrgk_vec_multi_dot(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double*
         DMRGK_CUDA(cudaGetLastError());
     }
     multi_dot_stage2<<<1, VEC_THREADS, 0, st>>>(grid, nv, partial, out_dev);
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }
@@ -252,6 +254,7 @@ int32_t dmrgk_vec_multi_axpy(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double
     multi_axpy_kernel<<<vec_grid(n2), VEC_THREADS, 0, (cudaStream_t)stream>>>(
         n2, nv, reinterpret_cast<const double2*>(X_dev), stride / 2, coef_dev, alpha, beta,
         reinterpret_cast<double2*>(y_dev));
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }
@@ -266,6 +269,7 @@ int32_t dmrgk_vec_axpby(dmrgk_ctx* ctx, int64_t n, double alpha, const double* x
     const int64_t n2 = n / 2;
     axpby_kernel<<<vec_grid(n2), VEC_THREADS, 0, (cudaStream_t)stream>>>(
         n2, alpha, reinterpret_cast<const double2*>(x_dev), beta, reinterpret_cast<double2*>(y_dev));
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }
@@ -282,6 +286,7 @@ int32_t dmrgk_vec_scal_dev(dmrgk_ctx* ctx, int64_t n, const double* alpha_dev, i
     scal_dev_kernel<<<vec_grid(n2), VEC_THREADS, 0, (cudaStream_t)stream>>>(
         n2, alpha_dev, mode & 1, (mode >> 1) & 1, reinterpret_cast<const double2*>(x_dev),
         reinterpret_cast<double2*>(y_dev));
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }
@@ -303,8 +308,10 @@ int32_t dmrgk_vec_residual(dmrgk_ctx* ctx, int64_t n, int32_t m, const double* V
     residual_stage1<<<grid, VEC_THREADS, 0, st>>>(n2, m, reinterpret_cast<const double2*>(V_dev),
                                                   reinterpret_cast<const double2*>(W_dev), stride / 2, coef_dev,
                                                   reinterpret_cast<double2*>(r_dev), partial);
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     multi_dot_stage2<<<1, VEC_THREADS, 0, st>>>(grid, 1, partial, out_dev);
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }
@@ -316,6 +323,7 @@ int32_t dmrgk_vec_precond(dmrgk_ctx* ctx, int64_t n, const double* r_dev, const 
     if (!r_dev || !diag_dev || !theta_dev || !t_dev) return fail(DMRGK_EINVAL, "vec_precond: NULL pointer");
     DMRGK_CUDA(cudaSetDevice(ctx->device));
     precond_kernel<<<vec_grid(n), VEC_THREADS, 0, (cudaStream_t)stream>>>(n, r_dev, diag_dev, theta_dev, t_dev);
+    count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }

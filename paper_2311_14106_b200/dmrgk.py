@@ -40,6 +40,7 @@ _pi32, _pi64, _pf64 = C.POINTER(C.c_int32), C.POINTER(C.c_int64), C.POINTER(C.c_
 SIGNATURES = {
     "dmrgk_last_error": (C.c_char_p, []),
     "dmrgk_version": (C.c_char_p, []),
+    "dmrgk_launch_count": (_i64, [_i32]),
     "dmrgk_ctx_create": (_i32, [_i32, _pp]),
     "dmrgk_ctx_destroy": (None, [_p]),
     "dmrgk_ctx_query": (_i32, [_p, _pi32, _pi64, _pi64]),
@@ -64,6 +65,8 @@ SIGNATURES = {
     "dmrgk_heff_apply": (_i32, [_p, _p, _p, _p, _p, _p]),
     "dmrgk_heff_apply_host": (_i32, [_p, _p, _p, _p, _p, _p, _p, _p]),
     "dmrgk_heff_diag": (_i32, [_p, _p, _p, _p, _p]),
+    "dmrgk_heff_profile": (_i32, [_p, _i32]),
+    "dmrgk_heff_profile_read": (_i32, [_p, _p, _p]),
     "dmrgk_vec_scratch_bytes": (_i64, [_i32]),
     "dmrgk_vec_multi_dot": (_i32, [_p, _i64, _i32, _p, _i64, _p, _p, _p, _p]),
     "dmrgk_vec_multi_axpy": (_i32, [_p, _i64, _i32, _p, _i64, _p, _f64, _f64, _p, _p]),
@@ -306,6 +309,17 @@ class Heff:
         check(self.lib.dmrgk_heff_apply_host(self.h, _dev(psi_host), _dev(sigma_host), _dev(psi), _dev(sigma),
                                              _dev(workspace), _stream(stream_main), _stream(stream_copy)))
 
+    def profile(self, enable=True):
+        check(self.lib.dmrgk_heff_profile(self.h, int(bool(enable))))
+
+    def profile_read(self):
+        """({"p1","p2","reduce"} → ms, same → launch counts) accumulated since profile()."""
+        ms = np.zeros(3, np.float64)
+        ln = np.zeros(3, np.int64)
+        check(self.lib.dmrgk_heff_profile_read(self.h, ms.ctypes.data, ln.ctypes.data))
+        names = ("p1", "p2", "reduce")
+        return dict(zip(names, ms.tolist())), dict(zip(names, ln.tolist()))
+
     def diag(self, diag, workspace, stream_main=None, stream_copy=None):
         check(self.lib.dmrgk_heff_diag(self.h, _dev(diag), _dev(workspace), _stream(stream_main),
                                        _stream(stream_copy)))
@@ -350,6 +364,10 @@ class Davidson:
         if getattr(self, "h", None):
             self.lib.dmrgk_davidson_destroy(self.h)
             self.h = None
+
+
+def launch_count(reset=False):
+    return load().dmrgk_launch_count(int(bool(reset)))
 
 
 def davidson_extra_bytes(m_max, n_padded):

@@ -172,20 +172,30 @@ def test_diag_matches_oracle():
 
 
 def test_staged_operators_bit_identical_to_resident():
-    """a3: operators streamed from pinned host memory through the ring give the same bits."""
+    """a3: operators streamed from pinned host memory through the ring.  With the same chunk
+    boundaries (ring large enough that only t_chunk_bytes cuts the pair list) the staged run gives
+    the same bits as the resident one; with a small ring (more chunks, a different summation order
+    over chunks) it agrees to rounding and is reproducible call after call."""
     from paper_2311_14106_b200 import problem
     wl = medium_spinless()
-    res = problem.from_workload(wl)
+    res = problem.from_workload(wl, t_chunk_bytes=1 << 20)
     psi = res.psi_fill(wl.seed, wlmod.PSI_STREAM)
     ref = res.apply(psi).clone()
     pinned = [i for i in range(len(wl.ops)) if i % 3 == 1]
-    stg = problem.from_workload(wl, pinned=pinned, ring_bytes=4 << 20, t_chunk_bytes=1 << 20)
-    assert stg.heff.n_chunks > 2
+    stg = problem.from_workload(wl, pinned=pinned, ring_bytes=256 << 20, t_chunk_bytes=1 << 20)
+    assert stg.heff.n_chunks == res.heff.n_chunks > 2
     for _ in range(2):      # second call re-uses the ring halves
         got = stg.apply(stg.psi_fill(wl.seed, wlmod.PSI_STREAM))
         torch.cuda.synchronize()
         assert torch.equal(got, ref)
     assert torch.equal(stg.diag(), res.diag())
+    small = problem.from_workload(wl, pinned=pinned, ring_bytes=4 << 20, t_chunk_bytes=1 << 20)
+    assert small.heff.n_chunks > res.heff.n_chunks
+    first = small.apply(psi).clone()
+    again = small.apply(psi)
+    torch.cuda.synchronize()
+    assert torch.equal(first, again)
+    assert float((first - ref).abs().max() / ref.abs().max()) <= 1e-13
 
 
 def test_apply_host_end_to_end():
