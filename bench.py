@@ -244,13 +244,14 @@ def run_ours(args):
 
     # ---- the FP64 ceiling of this box, live: register-only DMMA loop (burst) -------------------
     sink = torch.zeros(16, dtype=torch.float64, device="cuda")
-    dmrgk.probe_fp64(dp.ctx, 0, 200, sink, dp.stream)
-    pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    pe0.record(dp.stream)
-    pf = dmrgk.probe_fp64(dp.ctx, 0, 20000, sink, dp.stream)
-    pe1.record(dp.stream)
-    torch.cuda.synchronize()
-    dmma_probe = pf / pe0.elapsed_time(pe1) / 1e9
+    dmma_probe = 0.0
+    for _ in range(4):      # first call warms up; best of the rest
+        pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        pe0.record(dp.stream)
+        pf = dmrgk.probe_fp64(dp.ctx, 0, 20000, sink, dp.stream)
+        pe1.record(dp.stream)
+        torch.cuda.synchronize()
+        dmma_probe = max(dmma_probe, pf / pe0.elapsed_time(pe1) / 1e9)
     n_sm = dp.ctx.query()[0]
     sm_max = clk.get("sm_max_mhz") or 1965.0
     peak = n_sm * 128 * sm_max * 1e6 / 1e12     # 64 DFMA-equivalents/clk/SM

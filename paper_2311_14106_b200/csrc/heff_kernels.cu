@@ -42,12 +42,6 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                  : "d"(a), "d"(b));
 }
 
-struct SegCursor {
-    int seg;        // current segment index
-    int kt;         // k-tile inside it
-    int nkt;        // k-tiles of the current segment
-};
-
 // Load one BK-deep stage of segment `sg` (k-tile kt) for tile (i0, j0) into sA / sB.
 __device__ __forceinline__ void load_stage(const Seg& sg, const Bases& bases, int kt, int i0, int j0,
                                            int mrows, int ncols, double* sA, double* sB, int tid) {
@@ -92,9 +86,63 @@ __device__ __forceinline__ void load_stage(const Seg& sg, const Bases& bases, in
     }
 }
 
+// One k-tile (BK = 16, `nks` steps of 4) of a warp tile of FM × FN fragments.  FM, FN are compile-time
+// so the accumulator indices are static and no DMMA carries a guard; the caller branches once per
+// k-tile (warp-uniform) into the variant that matches the data this warp really holds.
+template <int FM, int FN, bool FULLK>
+__device__ __forceinline__ void mma_ktile(const double* __restrict__ pa, const double* __restrict__ pb,
+                                          int a_fs, int b_fs, int a_ks4, int b_ks4, int nks,
+                                          double (&acc)[4][4][2]) {
+    if (FULLK) {
+#pragma unroll
+        for (int ks = 0; ks < BK / 4; ++ks) {
+            double af[FM], bf[FN];
+#pragma unroll
+            for (int f = 0; f < FM; ++f) af[f] = pa[f * a_fs + ks * a_ks4];
+#pragma unroll
+            for (int f = 0; f < FN; ++f) bf[f] = pb[f * b_fs + ks * b_ks4];
+#pragma unroll
+            for (int i = 0; i < FM; ++i)
+#pragma unroll
+                for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        }
+    } else {
+#pragma unroll 1
+        for (int ks = 0; ks < nks; ++ks) {
+            double af[FM], bf[FN];
+#pragma unroll
+            for (int f = 0; f < FM; ++f) af[f] = pa[f * a_fs + ks * a_ks4];
+#pragma unroll
+            for (int f = 0; f < FN; ++f) bf[f] = pb[f * b_fs + ks * b_ks4];
+#pragma unroll
+            for (int i = 0; i < FM; ++i)
+#pragma unroll
+                for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        }
+    }
+}
+
+template <int FM>
+__device__ __forceinline__ void mma_ktile_n(int nfn, const double* pa, const double* pb, int a_fs, int b_fs,
+                                            int a_ks4, int b_ks4, int nks, double (&acc)[4][4][2]) {
+    switch (nfn) {
+        case 1: mma_ktile<FM, 1, false>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, nks, acc); break;
+        case 2: mma_ktile<FM, 2, false>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, nks, acc); break;
+        case 3: mma_ktile<FM, 3, false>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, nks, acc); break;
+        default: mma_ktile<FM, 4, false>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, nks, acc); break;
+    }
+}
+
+// Per-stage note left by the loader for the consumers (read after the barrier that publishes the stage).
+struct StageNote {
+    uint32_t flags;   // segment flags (operand majors)
+    int32_t nks;      // k-steps of 4 that hold data in this k-tile (1..4)
+};
+
 __global__ void __launch_bounds__(NTHREADS, 3)
 heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ segs, Bases bases) {
     extern __shared__ __align__(16) double smem[];
+    __shared__ StageNote notes[STAGES];
     const Unit u = units[blockIdx.x];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp >> 1, wn = warp & 1;
@@ -104,7 +152,8 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
     const int rows_t = min(BM, u.mrows - u.i0);
     const int cols_t = min(BN, u.ncols_st - u.j0);
     const int nfm = max(0, min(4, (rows_t - wm * 32 + 7) >> 3));
-    const int nfn = max(0, min(4, (cols_t - wn * 32 + 7) >> 3));
+    const int nfn = max(0, min(4, (min(BN, u.ncols - u.j0) - wn * 32 + 7) >> 3));
+    const bool busy = nfm > 0 && nfn > 0;
 
     double acc[4][4][2];
 #pragma unroll
@@ -112,88 +161,88 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    // total number of k-tiles over all segments
-    SegCursor ld{u.seg_begin, 0, 0}, cp{u.seg_begin, 0, 0};
+    // loader cursor: segment index, its descriptor (kept in registers), k-tile inside it
+    int ld_seg = u.seg_begin, ld_kt = 0, ld_nkt = 0;
+    Seg sg;
+    sg.klen = 0;
+    while (ld_seg < u.seg_end) {
+        sg = segs[ld_seg];
+        ld_nkt = (sg.klen + BK - 1) / BK;
+        if (ld_nkt) break;
+        ++ld_seg;
+    }
     const int total = u.nkt;
-    if (u.seg_begin < u.seg_end) ld.nkt = cp.nkt = (segs[u.seg_begin].klen + BK - 1) / BK;
 
-    auto advance = [&](SegCursor& c) {
-        if (++c.kt == c.nkt) {
-            c.kt = 0;
-            ++c.seg;
-            c.nkt = 0;
-            while (c.seg < u.seg_end) {
-                c.nkt = (segs[c.seg].klen + BK - 1) / BK;
-                if (c.nkt) break;
-                ++c.seg;
+    auto load_next = [&](int stage) {
+        load_stage(sg, bases, ld_kt, u.i0, u.j0, u.mrows, u.ncols, smem + stage * STAGE_DOUBLES,
+                   smem + stage * STAGE_DOUBLES + OPER_DOUBLES, tid);
+        if (tid == 0) {
+            notes[stage].flags = sg.flags;
+            notes[stage].nks = min(BK / 4, (sg.klen - ld_kt * BK + 3) >> 2);
+        }
+        if (++ld_kt == ld_nkt) {
+            ld_kt = 0;
+            ld_nkt = 0;
+            ++ld_seg;
+            while (ld_seg < u.seg_end) {
+                sg = segs[ld_seg];
+                ld_nkt = (sg.klen + BK - 1) / BK;
+                if (ld_nkt) break;
+                ++ld_seg;
             }
         }
     };
-    // skip leading empty segments
-    while (ld.seg < u.seg_end && ld.nkt == 0) {
-        ++ld.seg;
-        if (ld.seg < u.seg_end) ld.nkt = (segs[ld.seg].klen + BK - 1) / BK;
-    }
-    cp = ld;
 
     // prologue: STAGES−1 stages in flight
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
-        if (s < total) {
-            const Seg sg = segs[ld.seg];
-            load_stage(sg, bases, ld.kt, u.i0, u.j0, u.mrows, u.ncols, smem + s * STAGE_DOUBLES,
-                       smem + s * STAGE_DOUBLES + OPER_DOUBLES, tid);
-            advance(ld);
-        }
+        if (s < total) load_next(s);
         cp_async_commit();
     }
 
-    uint32_t cur_flags = 0;
-    int cur_seg = -1;
-    int a_off = 0, b_off = 0, a_fs = 0, a_ks = 0, b_fs = 0, b_ks = 0;
+    uint32_t cur_flags = 0xffffffffu;
+    int a_fs = 0, a_ks4 = 0, b_fs = 0, b_ks4 = 0, a_off = 0, b_off = 0;
+    int stage = 0;
     for (int it = 0; it < total; ++it) {
         cp_async_wait<STAGES - 2>();
         __syncthreads();
         {
             const int nx = it + STAGES - 1;
-            if (nx < total) {
-                const Seg sg = segs[ld.seg];
-                const int s = nx % STAGES;
-                load_stage(sg, bases, ld.kt, u.i0, u.j0, u.mrows, u.ncols, smem + s * STAGE_DOUBLES,
-                           smem + s * STAGE_DOUBLES + OPER_DOUBLES, tid);
-                advance(ld);
-            }
+            int ns = stage + STAGES - 1;
+            if (ns >= STAGES) ns -= STAGES;
+            if (nx < total) load_next(ns);
             cp_async_commit();
         }
-        if (cp.seg != cur_seg) {
-            cur_seg = cp.seg;
-            cur_flags = segs[cp.seg].flags;
+        const StageNote note = notes[stage];
+        if (note.flags != cur_flags) {
+            cur_flags = note.flags;
             // element (i, k) of A: K-major i·20 + k, M-major k·68 + i; same for B with j
             const int a_is = (cur_flags & SEG_A_MMAJOR) ? 1 : KM_STRIDE;
-            a_ks = (cur_flags & SEG_A_MMAJOR) ? MN_STRIDE : 1;
+            const int a_ks = (cur_flags & SEG_A_MMAJOR) ? MN_STRIDE : 1;
             const int b_js = (cur_flags & SEG_B_NMAJOR) ? 1 : KM_STRIDE;
-            b_ks = (cur_flags & SEG_B_NMAJOR) ? MN_STRIDE : 1;
+            const int b_ks = (cur_flags & SEG_B_NMAJOR) ? MN_STRIDE : 1;
             a_off = (wm * 32 + g) * a_is + t4 * a_ks;
             b_off = (wn * 32 + g) * b_js + t4 * b_ks;
             a_fs = 8 * a_is;
             b_fs = 8 * b_js;
+            a_ks4 = 4 * a_ks;
+            b_ks4 = 4 * b_ks;
         }
-        const double* sA = smem + (it % STAGES) * STAGE_DOUBLES;
-        const double* sB = sA + OPER_DOUBLES;
-#pragma unroll
-        for (int ks = 0; ks < BK / 4; ++ks) {
-            double af[4], bf[4];
-#pragma unroll
-            for (int f = 0; f < 4; ++f) af[f] = (f < nfm) ? sA[a_off + f * a_fs + ks * 4 * a_ks] : 0.0;
-#pragma unroll
-            for (int f = 0; f < 4; ++f) bf[f] = (f < nfn) ? sB[b_off + f * b_fs + ks * 4 * b_ks] : 0.0;
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if (i < nfm && j < nfn) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        if (busy) {
+            const double* pa = smem + stage * STAGE_DOUBLES + a_off;
+            const double* pb = smem + stage * STAGE_DOUBLES + OPER_DOUBLES + b_off;
+            if (nfm == 4 && nfn == 4 && note.nks == 4) {
+                mma_ktile<4, 4, true>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, 4, acc);
+            } else {
+                switch (nfm) {
+                    case 1: mma_ktile_n<1>(nfn, pa, pb, a_fs, b_fs, a_ks4, b_ks4, note.nks, acc); break;
+                    case 2: mma_ktile_n<2>(nfn, pa, pb, a_fs, b_fs, a_ks4, b_ks4, note.nks, acc); break;
+                    case 3: mma_ktile_n<3>(nfn, pa, pb, a_fs, b_fs, a_ks4, b_ks4, note.nks, acc); break;
+                    default: mma_ktile_n<4>(nfn, pa, pb, a_fs, b_fs, a_ks4, b_ks4, note.nks, acc); break;
+                }
+            }
         }
-        advance(cp);
+        if (++stage == STAGES) stage = 0;
     }
     cp_async_wait<0>();
 
@@ -203,11 +252,11 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int r = wm * 32 + i * 8 + g;
-        if (i >= nfm || r >= rows_t) continue;
+        if (r >= rows_t) continue;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int c = wn * 32 + j * 8 + 2 * t4;
-            if (j >= nfn || c >= cols_t) continue;
+            if (c >= cols_t) continue;
             double2* p = reinterpret_cast<double2*>(C + int64_t(r) * u.ldc + c);
             double2 v;
             v.x = (u.j0 + c < u.ncols) ? u.alpha * acc[i][j][0] : 0.0;
