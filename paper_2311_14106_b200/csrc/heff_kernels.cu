@@ -42,57 +42,73 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                  : "d"(a), "d"(b));
 }
 
-// Load one BK-deep stage of segment `sg` (k-tile kt) for tile (i0, j0) into sA / sB.
-__device__ __forceinline__ void load_stage(const Seg& sg, const Bases& bases, int kt, int i0, int j0,
-                                           int mrows, int ncols, double* sA, double* sB, int tid) {
-    const double* A = reinterpret_cast<const double*>(bases.b[(sg.flags >> SEG_A_SEL_SHIFT) & 3u] + sg.A);
-    const double* B = reinterpret_cast<const double*>(bases.b[(sg.flags >> SEG_B_SEL_SHIFT) & 3u] + sg.B);
-    const int k0 = kt * BK;
-    if (!(sg.flags & SEG_A_MMAJOR)) {
-        // K-major: 64 rows × 8 chunks of 16 B; the k direction is covered by the zero padding of lda
+// ---- loader ------------------------------------------------------------------------------------
+// Per-thread copy plan of one operand for the current segment: every stage this thread issues four
+// 16-byte cp.async; everything that does not change from k-tile to k-tile is computed once per segment
+// so the per-stage cost is a pointer bump and four predicated copies.
+struct OpPlan {
+    const char* ptr;      // source of copy j = 0 for the next k-tile (bytes)
+    const char* safe;     // a valid address for predicated-off copies (block origin)
+    long long step_j;     // source distance between copies j and j+1 (bytes)
+    long long step_k;     // source advance per k-tile (bytes)
+    uint32_t dst;         // destination of copy j = 0 inside the operand tile (bytes)
+    uint32_t dst_step;    // destination distance between copies (bytes)
+    int32_t mask;         // bit j: copy j is inside the operand along the M/N direction
+    int32_t krow;         // MN-major: k-row of copy 0 (copy j is krow + 4j); K-major: −64 (never cut by klen)
+};
+
+// Operand tile origin `o0` (row/column offset of the tile in the block), `ext` = block extent in that
+// direction (rows for K-major predication; ld for MN-major), `mn_major` = the tile is stored [k][i].
+__device__ __forceinline__ void make_plan(OpPlan& p, const char* base, int ld, bool mn_major, int o0, int ext,
+                                          int tid) {
+    p.safe = base;
+    if (!mn_major) {
+        const int row = tid >> 3, ch = tid & 7;            // copies j: rows row + 16 j, chunk ch
+        p.ptr = base + (int64_t(o0 + row) * ld + ch * 2) * 8;
+        p.step_j = int64_t(16) * ld * 8;
+        p.step_k = BK * 8;
+        p.dst = (row * KM_STRIDE + ch * 2) * 8;
+        p.dst_step = 16 * KM_STRIDE * 8;
+        int m = 0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            int c = tid + NTHREADS * j, row = c >> 3, ch = c & 7;
-            bool p = (i0 + row) < mrows;
-            const double* src = p ? A + int64_t(i0 + row) * sg.lda + k0 + ch * 2 : A;
-            cp_async16(sA + row * KM_STRIDE + ch * 2, src, p);
-        }
+        for (int j = 0; j < 4; ++j) m |= ((o0 + row + 16 * j) < ext) << j;
+        p.mask = m;
+        p.krow = -64;
     } else {
-        // M-major: 16 k-rows × 32 chunks
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            int c = tid + NTHREADS * j, row = c >> 5, ch = c & 31;
-            bool p = (k0 + row) < sg.klen && (i0 + ch * 2) < sg.lda;
-            const double* src = p ? A + int64_t(k0 + row) * sg.lda + i0 + ch * 2 : A;
-            cp_async16(sA + row * MN_STRIDE + ch * 2, src, p);
-        }
-    }
-    if (!(sg.flags & SEG_B_NMAJOR)) {
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            int c = tid + NTHREADS * j, row = c >> 3, ch = c & 7;
-            bool p = (j0 + row) < ncols;
-            const double* src = p ? B + int64_t(j0 + row) * sg.ldb + k0 + ch * 2 : B;
-            cp_async16(sB + row * KM_STRIDE + ch * 2, src, p);
-        }
-    } else {
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            int c = tid + NTHREADS * j, row = c >> 5, ch = c & 31;
-            bool p = (k0 + row) < sg.klen && (j0 + ch * 2) < sg.ldb;
-            const double* src = p ? B + int64_t(k0 + row) * sg.ldb + j0 + ch * 2 : B;
-            cp_async16(sB + row * MN_STRIDE + ch * 2, src, p);
-        }
+        const int row = tid >> 5, ch = tid & 31;           // copies j: k-rows row + 4 j, chunk ch
+        p.ptr = base + (int64_t(row) * ld + o0 + ch * 2) * 8;
+        p.step_j = int64_t(4) * ld * 8;
+        p.step_k = int64_t(BK) * ld * 8;
+        p.dst = (row * MN_STRIDE + ch * 2) * 8;
+        p.dst_step = 4 * MN_STRIDE * 8;
+        p.mask = (o0 + ch * 2) < ext ? 15 : 0;
+        p.krow = row;
     }
 }
 
-// One k-tile (BK = 16, `nks` steps of 4) of a warp tile of FM × FN fragments.  FM, FN are compile-time
-// so the accumulator indices are static and no DMMA carries a guard; the caller branches once per
-// k-tile (warp-uniform) into the variant that matches the data this warp really holds.
-template <int FM, int FN, bool FULLK>
-__device__ __forceinline__ void mma_ktile(const double* __restrict__ pa, const double* __restrict__ pb,
-                                          int a_fs, int b_fs, int a_ks4, int b_ks4, int nks,
+// Issue the four copies of one operand for a k-tile with `rem` contraction elements left (≥ 1).
+__device__ __forceinline__ void issue_plan(OpPlan& p, uint32_t smem_operand, int rem) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const bool ok = ((p.mask >> j) & 1) && (p.krow + 4 * j) < rem;
+        const char* src = ok ? p.ptr + j * p.step_j : p.safe;
+        const int n = ok ? 16 : 0;   // src-size 0 → 16 bytes of zeros
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_operand + p.dst + j * p.dst_step),
+                     "l"(src), "r"(n));
+    }
+    p.ptr += p.step_k;
+}
+
+// ---- consumer ----------------------------------------------------------------------------------
+// One k-tile (BK = 16, `nks` steps of 4) of a warp tile of FM × FN fragments.  FM, FN and the operand
+// layouts are compile-time: accumulator indices are static, no DMMA carries a guard, and every LDS.64
+// has an immediate offset.  Element (i, k) of A sits at i·20 + k (K-major) or k·68 + i (M-major);
+// the same for B with j.
+template <int FM, int FN, bool AM, bool BN_, bool FULLK>
+__device__ __forceinline__ void mma_ktile(const double* __restrict__ pa, const double* __restrict__ pb, int nks,
                                           double (&acc)[4][4][2]) {
+    constexpr int a_fs = 8 * (AM ? 1 : KM_STRIDE), a_ks4 = 4 * (AM ? MN_STRIDE : 1);
+    constexpr int b_fs = 8 * (BN_ ? 1 : KM_STRIDE), b_ks4 = 4 * (BN_ ? MN_STRIDE : 1);
     if (FULLK) {
 #pragma unroll
         for (int ks = 0; ks < BK / 4; ++ks) {
@@ -111,25 +127,45 @@ __device__ __forceinline__ void mma_ktile(const double* __restrict__ pa, const d
         for (int ks = 0; ks < nks; ++ks) {
             double af[FM], bf[FN];
 #pragma unroll
-            for (int f = 0; f < FM; ++f) af[f] = pa[f * a_fs + ks * a_ks4];
+            for (int f = 0; f < FM; ++f) af[f] = pa[f * a_fs];
 #pragma unroll
-            for (int f = 0; f < FN; ++f) bf[f] = pb[f * b_fs + ks * b_ks4];
+            for (int f = 0; f < FN; ++f) bf[f] = pb[f * b_fs];
 #pragma unroll
             for (int i = 0; i < FM; ++i)
 #pragma unroll
                 for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+            pa += a_ks4;
+            pb += b_ks4;
         }
     }
 }
 
-template <int FM>
-__device__ __forceinline__ void mma_ktile_n(int nfn, const double* pa, const double* pb, int a_fs, int b_fs,
-                                            int a_ks4, int b_ks4, int nks, double (&acc)[4][4][2]) {
+template <int FM, bool AM, bool BN_>
+__device__ __forceinline__ void mma_ktile_n(int nfn, const double* pa, const double* pb, int nks,
+                                            double (&acc)[4][4][2]) {
     switch (nfn) {
-        case 1: mma_ktile<FM, 1, false>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, nks, acc); break;
-        case 2: mma_ktile<FM, 2, false>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, nks, acc); break;
-        case 3: mma_ktile<FM, 3, false>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, nks, acc); break;
-        default: mma_ktile<FM, 4, false>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, nks, acc); break;
+        case 1: mma_ktile<FM, 1, AM, BN_, false>(pa, pb, nks, acc); break;
+        case 2: mma_ktile<FM, 2, AM, BN_, false>(pa, pb, nks, acc); break;
+        case 3: mma_ktile<FM, 3, AM, BN_, false>(pa, pb, nks, acc); break;
+        default: mma_ktile<FM, 4, AM, BN_, false>(pa, pb, nks, acc); break;
+    }
+}
+
+// All fragment shapes of one operand-layout combination; branches are warp-uniform.
+template <bool AM, bool BN_>
+__device__ __forceinline__ void mma_layout(int nfm, int nfn, int nks, const double* sA, const double* sB, int wm,
+                                           int wn, int g, int t4, double (&acc)[4][4][2]) {
+    const double* pa = sA + (wm * 32 + g) * (AM ? 1 : KM_STRIDE) + t4 * (AM ? MN_STRIDE : 1);
+    const double* pb = sB + (wn * 32 + g) * (BN_ ? 1 : KM_STRIDE) + t4 * (BN_ ? MN_STRIDE : 1);
+    if (nfm == 4 && nfn == 4 && nks == 4) {
+        mma_ktile<4, 4, AM, BN_, true>(pa, pb, 4, acc);
+    } else {
+        switch (nfm) {
+            case 1: mma_ktile_n<1, AM, BN_>(nfn, pa, pb, nks, acc); break;
+            case 2: mma_ktile_n<2, AM, BN_>(nfn, pa, pb, nks, acc); break;
+            case 3: mma_ktile_n<3, AM, BN_>(nfn, pa, pb, nks, acc); break;
+            default: mma_ktile_n<4, AM, BN_>(nfn, pa, pb, nks, acc); break;
+        }
     }
 }
 
@@ -147,6 +183,7 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp >> 1, wn = warp & 1;
     const int g = lane >> 2, t4 = lane & 3;
+    const uint32_t smem_base = static_cast<uint32_t>(__cvta_generic_to_shared(smem));
 
     // rows / columns of this tile that hold data, in 8-wide fragments, for this warp
     const int rows_t = min(BM, u.mrows - u.i0);
@@ -161,35 +198,41 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    // loader cursor: segment index, its descriptor (kept in registers), k-tile inside it
-    int ld_seg = u.seg_begin, ld_kt = 0, ld_nkt = 0;
-    Seg sg;
-    sg.klen = 0;
-    while (ld_seg < u.seg_end) {
-        sg = segs[ld_seg];
-        ld_nkt = (sg.klen + BK - 1) / BK;
-        if (ld_nkt) break;
-        ++ld_seg;
-    }
+    // loader state: segment cursor, remaining contraction length of the segment, the two copy plans
+    int ld_seg = u.seg_begin, ld_rem = 0;
+    uint32_t ld_flags = 0;
+    OpPlan planA, planB;
+    auto open_segment = [&]() {
+        while (ld_seg < u.seg_end) {
+            const Seg sg = segs[ld_seg];
+            if (sg.klen > 0) {
+                ld_rem = sg.klen;
+                ld_flags = sg.flags;
+                const char* A = reinterpret_cast<const char*>(bases.b[(sg.flags >> SEG_A_SEL_SHIFT) & 3u] + sg.A);
+                const char* B = reinterpret_cast<const char*>(bases.b[(sg.flags >> SEG_B_SEL_SHIFT) & 3u] + sg.B);
+                const bool am = (sg.flags & SEG_A_MMAJOR) != 0, bn = (sg.flags & SEG_B_NMAJOR) != 0;
+                make_plan(planA, A, sg.lda, am, u.i0, am ? sg.lda : u.mrows, tid);
+                make_plan(planB, B, sg.ldb, bn, u.j0, bn ? sg.ldb : u.ncols, tid);
+                return;
+            }
+            ++ld_seg;
+        }
+    };
+    open_segment();
     const int total = u.nkt;
 
     auto load_next = [&](int stage) {
-        load_stage(sg, bases, ld_kt, u.i0, u.j0, u.mrows, u.ncols, smem + stage * STAGE_DOUBLES,
-                   smem + stage * STAGE_DOUBLES + OPER_DOUBLES, tid);
+        const uint32_t sA = smem_base + stage * (STAGE_DOUBLES * 8);
+        issue_plan(planA, sA, ld_rem);
+        issue_plan(planB, sA + OPER_DOUBLES * 8, ld_rem);
         if (tid == 0) {
-            notes[stage].flags = sg.flags;
-            notes[stage].nks = min(BK / 4, (sg.klen - ld_kt * BK + 3) >> 2);
+            notes[stage].flags = ld_flags;
+            notes[stage].nks = min(BK / 4, (ld_rem + 3) >> 2);
         }
-        if (++ld_kt == ld_nkt) {
-            ld_kt = 0;
-            ld_nkt = 0;
+        ld_rem -= BK;
+        if (ld_rem <= 0) {
             ++ld_seg;
-            while (ld_seg < u.seg_end) {
-                sg = segs[ld_seg];
-                ld_nkt = (sg.klen + BK - 1) / BK;
-                if (ld_nkt) break;
-                ++ld_seg;
-            }
+            open_segment();
         }
     };
 
@@ -200,46 +243,25 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
         cp_async_commit();
     }
 
-    uint32_t cur_flags = 0xffffffffu;
-    int a_fs = 0, a_ks4 = 0, b_fs = 0, b_ks4 = 0, a_off = 0, b_off = 0;
     int stage = 0;
     for (int it = 0; it < total; ++it) {
         cp_async_wait<STAGES - 2>();
         __syncthreads();
         {
-            const int nx = it + STAGES - 1;
             int ns = stage + STAGES - 1;
             if (ns >= STAGES) ns -= STAGES;
-            if (nx < total) load_next(ns);
+            if (it + STAGES - 1 < total) load_next(ns);
             cp_async_commit();
         }
-        const StageNote note = notes[stage];
-        if (note.flags != cur_flags) {
-            cur_flags = note.flags;
-            // element (i, k) of A: K-major i·20 + k, M-major k·68 + i; same for B with j
-            const int a_is = (cur_flags & SEG_A_MMAJOR) ? 1 : KM_STRIDE;
-            const int a_ks = (cur_flags & SEG_A_MMAJOR) ? MN_STRIDE : 1;
-            const int b_js = (cur_flags & SEG_B_NMAJOR) ? 1 : KM_STRIDE;
-            const int b_ks = (cur_flags & SEG_B_NMAJOR) ? MN_STRIDE : 1;
-            a_off = (wm * 32 + g) * a_is + t4 * a_ks;
-            b_off = (wn * 32 + g) * b_js + t4 * b_ks;
-            a_fs = 8 * a_is;
-            b_fs = 8 * b_js;
-            a_ks4 = 4 * a_ks;
-            b_ks4 = 4 * b_ks;
-        }
         if (busy) {
-            const double* pa = smem + stage * STAGE_DOUBLES + a_off;
-            const double* pb = smem + stage * STAGE_DOUBLES + OPER_DOUBLES + b_off;
-            if (nfm == 4 && nfn == 4 && note.nks == 4) {
-                mma_ktile<4, 4, true>(pa, pb, a_fs, b_fs, a_ks4, b_ks4, 4, acc);
-            } else {
-                switch (nfm) {
-                    case 1: mma_ktile_n<1>(nfn, pa, pb, a_fs, b_fs, a_ks4, b_ks4, note.nks, acc); break;
-                    case 2: mma_ktile_n<2>(nfn, pa, pb, a_fs, b_fs, a_ks4, b_ks4, note.nks, acc); break;
-                    case 3: mma_ktile_n<3>(nfn, pa, pb, a_fs, b_fs, a_ks4, b_ks4, note.nks, acc); break;
-                    default: mma_ktile_n<4>(nfn, pa, pb, a_fs, b_fs, a_ks4, b_ks4, note.nks, acc); break;
-                }
+            const StageNote note = notes[stage];
+            const double* sA = smem + stage * STAGE_DOUBLES;
+            const double* sB = sA + OPER_DOUBLES;
+            switch (note.flags & (SEG_A_MMAJOR | SEG_B_NMAJOR)) {
+                case 0: mma_layout<false, false>(nfm, nfn, note.nks, sA, sB, wm, wn, g, t4, acc); break;
+                case SEG_A_MMAJOR: mma_layout<true, false>(nfm, nfn, note.nks, sA, sB, wm, wn, g, t4, acc); break;
+                case SEG_B_NMAJOR: mma_layout<false, true>(nfm, nfn, note.nks, sA, sB, wm, wn, g, t4, acc); break;
+                default: mma_layout<true, true>(nfm, nfn, note.nks, sA, sB, wm, wn, g, t4, acc); break;
             }
         }
         if (++stage == STAGES) stage = 0;
