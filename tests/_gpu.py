@@ -46,3 +46,28 @@ def config1_problem():
     pb = export.export_bond(d, space)
     pb.psi = dmrg.vec_to_blocks(space, x)
     return pb, Heff, x, space
+
+
+def oracle_problem_for_output_block(wl, a_out, b_out, psi=None):
+    """oracle.heff.Problem restricted to the operator blocks that write σ block (a_out, b_out) of a
+    (large) seeded workload: for every term only the L block whose applied output sector is a_out and
+    the R block whose applied output sector is b_out are generated (host generator, workloads.fill_op_host),
+    so `sigma_blockwise` of the restricted problem equals the full σ on that block and is zero elsewhere."""
+    import workloads as wlmod
+    from oracle import heff
+    need = {}
+    for t in wl.terms:
+        for idx, trans, out in ((t.L, t.trans_L, a_out), (t.R, t.trans_R, b_out)):
+            if idx is None:
+                continue
+            spec = wl.ops[idx]
+            for (r, c, _, _, _) in wlmod.op_block_table(wl.sectors(spec.half), spec.dq):
+                if (c if trans else r) == out:
+                    need.setdefault(idx, set()).add((r, c))
+    ops = []
+    for i, spec in enumerate(wl.ops):
+        blocks = wlmod.fill_op_host(wl, i, only_blocks=need[i]) if i in need else {}
+        ops.append({"half": spec.half, "dq": tuple(spec.dq), "parity": spec.parity, "blocks": blocks})
+    terms = [(t.L, t.R, t.coef, t.trans_L, t.trans_R) for t in wl.terms]
+    return heff.Problem(wl.n_charges, list(wl.sectors_A), list(wl.sectors_B), tuple(wl.target), ops, terms,
+                        wlmod.fill_psi_host(wl) if psi is None else psi, wl.name + f"_out{a_out}_{b_out}")

@@ -303,3 +303,44 @@ def lattice_workload(kind, n_half, M, seed, name=None, width2=None, keep=None):
     sectors = [(q, d) for q, d in zip(qs, dims)]
     wl = Workload(name or f"{kind}_n{n_half}_M{M}", seed, len(target), sectors, list(sectors), target)
     return _family_builder(wl, shifts[0], shifts[1], keep=keep)
+
+
+# ----------------------------------------------------------------------------
+# the BASELINE.json configs by name (configs[0] is real physics and comes from
+# the oracle's DMRG, see tests/_gpu.config1_problem)
+# ----------------------------------------------------------------------------
+def config3():
+    """configs[2]: 8×8 spinless torus, mode-rotated, D = 2048 (M = 4096), K = 2146."""
+    return lattice_workload("spinless", 32, 4096, seed=3, name="config3_spinless8x8_rotated_D2048")
+
+
+def config4():
+    """configs[3]: 6×6 Hubbard torus, mode-rotated, D = 4096 (M = 16384), K = 2702."""
+    return lattice_workload("hubbard", 18, 16384, seed=4, name="config4_hubbard6x6_rotated_D4096")
+
+
+def config4_realspace():
+    """configs[3], real-space variant: on-site U gives no cross-cut two-body
+    term, so only H_A, H_B and the hopping of the 12 boundary sites × 2 spins cross the cut:
+    K = 2 + 12·2·2 = 50.  Built as the F0 + thinned F1/F2 families of the rotated list."""
+    keep = lambda fam, i: fam == "F1" and i < 24
+    return lattice_workload("hubbard", 18, 16384, seed=4, name="config4_hubbard6x6_realspace_D4096", keep=keep)
+
+
+def config5_keep(fam, i):
+    """Executed subset of configs[4]: every F1/F2 pair, every 12th F3 and F4 pair (same
+    family proportions as a stratified sample of the 10 586-pair list)."""
+    return fam in ("F1", "F2") or i % 12 == 0
+
+
+def config5():
+    """configs[4]: 12×12 spinless torus, mode-rotated, D = 8192 (M = 16384).  The full list
+    (K = 10 586, ≈ 1.05 TB of operators stored once) cannot fit; the executed subset keeps
+    K_exec pairs (≈ 115 GB) of which ``config5_staged_ops`` are bound to pinned host memory."""
+    return lattice_workload("spinless", 72, 16384, seed=5, name="config5_spinless12x12_rotated_D8192_subset",
+                            keep=config5_keep)
+
+
+def config5_staged_ops(wl):
+    """Every 7th stored operator streams from pinned host memory (≈ 14 % of the bytes)."""
+    return [i for i in range(len(wl.ops)) if i % 7 == 3]
