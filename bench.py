@@ -33,9 +33,9 @@ UNIT = "TFLOP/s"
 def make_workload(name):
     import workloads as wlmod
     if name == "4":
-        return wlmod.lattice_workload("hubbard", 18, 16384, seed=4, name="config4_hubbard6x6_rotated_D4096")
+        return wlmod.config4()
     if name == "3":
-        return wlmod.lattice_workload("spinless", 32, 4096, seed=3, name="config3_spinless8x8_rotated_D2048")
+        return wlmod.config3()
     if name == "3b":
         return wlmod.lattice_workload("spinless", 32, 8192, seed=3, name="shape3b_spinless8x8_rotated_D4096")
     if name == "2":
@@ -119,6 +119,23 @@ class ClockSampler:
         sm.sort()
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(smax) if smax else None,
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def max_over_ranks(ms, world, device=None):
+    """Max of a per-rank duration over all ranks (replicas run independently; the job is as slow
+    as its slowest rank).  Works on any initialised backend (nccl on GPUs, gloo in the CPU tests)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_tflops(flops_per_rank_step, world, ms_step):
+    """Whole-job throughput of `world` independent replicas ("replicas only", weak scaling)."""
+    return world * flops_per_rank_step / ms_step / 1e9
 
 
 def time_oracle(pb, steps, warmup):
@@ -215,12 +232,9 @@ def run_ours(args):
     prof_ms, prof_n = h.profile_read()
     h.profile(False)
     clk = clocks.stop()
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, world, "cuda")
     ms_step = ms_total / args.steps
-    value = world * h.flops_alg / ms_step / 1e9
+    value = aggregate_tflops(h.flops_alg, world, ms_step)
 
     # ---- e2e: the same matvec through the C-ABI call with HOST buffers ---------------------------
     ph = torch.empty(n, dtype=torch.float64).pin_memory()
@@ -237,10 +251,7 @@ def run_ours(args):
     e3.record(dp.stream)
     barrier()
     ms_e2e = e2.elapsed_time(e3) / args.steps
-    if world > 1:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = max_over_ranks(ms_e2e, world, "cuda")
 
     # ---- the FP64 ceiling of this box, live: register-only DMMA loop (burst) -------------------
     sink = torch.zeros(16, dtype=torch.float64, device="cuda")
