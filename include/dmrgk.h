@@ -123,7 +123,7 @@ enum {
 typedef struct dmrgk_heff_opts {
     int64_t t_chunk_bytes;  /* cap on the L_k·ψ intermediate workspace per chunk of pairs
                                (0 = default 4 GiB); pairs are processed chunk by chunk       */
-    int64_t ring_bytes;     /* staging ring for pinned operators, split in two halves
+    int64_t ring_bytes;     /* staging ring for pinned operators, split in three parts
                                (0 = no ring: binding a pinned operator is then an error)     */
     int32_t kernel;         /* 0 = DMMA tensor-core kernel (product path),
                                1 = scalar check kernel (same task lists; debugging aid)     */
@@ -164,11 +164,15 @@ int32_t dmrgk_heff_apply_host(dmrgk_heff* h, const double* psi_host, double* sig
 int32_t dmrgk_heff_diag(dmrgk_heff* h, double* diag_dev, void* workspace_dev, void* stream_main,
                         void* stream_copy);
 
-/* Measurement aid: with enable != 0 every later heff_apply brackets each of its
- * kernel launches with a CUDA event pair on stream_main; enable (either value) zeroes the sums.
- * profile_read synchronises on the recorded events and returns the accumulated device time in ms
- * and the launch counts since the last enable, as ms[3] / launches[3] =
- * {phase-1 GEMM (a5), phase-2 GEMM (a6), split-k reduce (a7)}.  Either pointer may be NULL. */
+/* Measurement aid.  enable = 1: every later heff_apply brackets its whole GEMM region
+ * (first phase-1 launch … last reduce) with one CUDA event pair on stream_main; the launches keep
+ * their normal overlap (phase 1 of chunk c+1 runs concurrently with phase 2 of chunk c).
+ * enable = 2 (diagnostic): apply runs every launch on stream_main, serialised, each inside its own
+ * event pair.  enable = 0 switches profiling off.  Every call zeroes the sums.
+ * profile_read synchronises on the recorded events and returns the accumulated device time in ms and
+ * the launch counts since the last enable, as ms[4] / launches[4] = {phase-1 GEMM (a5), phase-2 GEMM
+ * (a6), split-k reduce (a7), whole-apply span}; ms[0..2] are only filled in mode 2, launches[3]
+ * counts applies.  Either pointer may be NULL. */
 int32_t dmrgk_heff_profile(dmrgk_heff* h, int32_t enable);
 int32_t dmrgk_heff_profile_read(dmrgk_heff* h, double* ms, int64_t* launches);
 

@@ -13,9 +13,12 @@
 
 namespace dmrgk {
 
-constexpr int BM = TILE_M, BN = TILE_N, BK = 16;
+constexpr int BM = TILE_M, BN = TILE_N, BK = TILE_K;
 constexpr int NTHREADS = 128;           // 4 warps as 2×2, each a 32×32 warp tile = 4×4 DMMA frags
 constexpr int STAGES = 3;
+constexpr int NCOPY = BK / 4;            // 16-byte copies per thread per operand per stage
+constexpr int KM_CPR = BK / 2;           // 16-byte chunks per row of a K-major tile
+constexpr int KM_RPP = NTHREADS / KM_CPR;  // rows covered by one pass of the CTA
 // Shared tile layouts (doubles).  K-major operand tile: [64 rows][BK] with row stride 20
 // (20·2 words ≡ 8 mod 32 → the 4 rows × 4 k of a half-warp LDS.64 hit 16 distinct bank pairs).
 // MN-major operand tile: [BK rows][64] with row stride 68 (68·2 ≡ 8 mod 32, same argument with
@@ -63,15 +66,15 @@ __device__ __forceinline__ void make_plan(OpPlan& p, const char* base, int ld, b
                                           int tid) {
     p.safe = base;
     if (!mn_major) {
-        const int row = tid >> 3, ch = tid & 7;            // copies j: rows row + 16 j, chunk ch
+        const int row = tid / KM_CPR, ch = tid % KM_CPR;   // copies j: rows row + KM_RPP·j, chunk ch
         p.ptr = base + (int64_t(o0 + row) * ld + ch * 2) * 8;
-        p.step_j = int64_t(16) * ld * 8;
+        p.step_j = int64_t(KM_RPP) * ld * 8;
         p.step_k = BK * 8;
         p.dst = (row * KM_STRIDE + ch * 2) * 8;
-        p.dst_step = 16 * KM_STRIDE * 8;
+        p.dst_step = KM_RPP * KM_STRIDE * 8;
         int m = 0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) m |= ((o0 + row + 16 * j) < ext) << j;
+        for (int j = 0; j < NCOPY; ++j) m |= ((o0 + row + KM_RPP * j) < ext) << j;
         p.mask = m;
         p.krow = -64;
     } else {
@@ -81,7 +84,7 @@ __device__ __forceinline__ void make_plan(OpPlan& p, const char* base, int ld, b
         p.step_k = int64_t(BK) * ld * 8;
         p.dst = (row * MN_STRIDE + ch * 2) * 8;
         p.dst_step = 4 * MN_STRIDE * 8;
-        p.mask = (o0 + ch * 2) < ext ? 15 : 0;
+        p.mask = (o0 + ch * 2) < ext ? ((1 << NCOPY) - 1) : 0;
         p.krow = row;
     }
 }
@@ -89,7 +92,7 @@ __device__ __forceinline__ void make_plan(OpPlan& p, const char* base, int ld, b
 // Issue the four copies of one operand for a k-tile with `rem` contraction elements left (≥ 1).
 __device__ __forceinline__ void issue_plan(OpPlan& p, uint32_t smem_operand, int rem) {
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
+    for (int j = 0; j < NCOPY; ++j) {
         const bool ok = ((p.mask >> j) & 1) && (p.krow + 4 * j) < rem;
         const char* src = ok ? p.ptr + j * p.step_j : p.safe;
         const int n = ok ? 16 : 0;   // src-size 0 → 16 bytes of zeros
@@ -157,8 +160,8 @@ __device__ __forceinline__ void mma_layout(int nfm, int nfn, int nks, const doub
                                            int wn, int g, int t4, double (&acc)[4][4][2]) {
     const double* pa = sA + (wm * 32 + g) * (AM ? 1 : KM_STRIDE) + t4 * (AM ? MN_STRIDE : 1);
     const double* pb = sB + (wn * 32 + g) * (BN_ ? 1 : KM_STRIDE) + t4 * (BN_ ? MN_STRIDE : 1);
-    if (nfm == 4 && nfn == 4 && nks == 4) {
-        mma_ktile<4, 4, AM, BN_, true>(pa, pb, 4, acc);
+    if (nfm == 4 && nfn == 4 && nks == BK / 4) {
+        mma_ktile<4, 4, AM, BN_, true>(pa, pb, BK / 4, acc);
     } else {
         switch (nfm) {
             case 1: mma_ktile_n<1, AM, BN_>(nfn, pa, pb, nks, acc); break;

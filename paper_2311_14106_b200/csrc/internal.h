@@ -131,7 +131,7 @@ struct Unit {
     int32_t ncols_st;   // columns to store (padded ld of the C block); columns ≥ ncols get zeros
     int32_t seg_begin, seg_end;
     uint32_t mode;      // UNIT_ACCUM | selector << UNIT_C_SEL_SHIFT
-    int32_t nkt;        // Σ over the unit's segments of ceil(klen/16)
+    int32_t nkt;        // Σ over the unit's segments of ceil(klen/TILE_K)
 };  // 56 B
 
 // Fixed-order reduction of split-k partial tiles into σ: C[r, c] += Σ_s P[s][r·64 + c].
@@ -157,6 +157,7 @@ struct DiagBlock {
 };
 
 constexpr int TILE_M = 64, TILE_N = 64;
+constexpr int TILE_K = 16;   // contraction depth of one pipeline stage (k-tile); Unit::nkt counts these
 
 // kernel launchers (heff_kernels.cu)
 int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
@@ -179,7 +180,7 @@ struct Chunk {
     int64_t p1_segs = 0, p2_segs = 0;
     int64_t d_block0 = 0, d_blocks = 0;
     std::vector<StageCopy> copies;
-    int ring_half = -1;
+    int ring_part = -1;   // which third of the staging ring holds this chunk's pinned operators
 };
 
 }  // namespace dmrgk
@@ -191,8 +192,8 @@ struct dmrgk_heff {
     int64_t n_tasks = 0;
     double flops_alg = 0, flops_exec = 0;
     int64_t op_bytes = 0;
-    int64_t t_bytes = 0, partial_bytes = 0, ring_bytes = 0, ring_half_bytes = 0, workspace_bytes = 0;
-    bool done_recorded[2] = {false, false};
+    int64_t t_bytes = 0, partial_bytes = 0, ring_bytes = 0, ring_part_bytes = 0, workspace_bytes = 0;
+    bool done_recorded[3] = {false, false, false};
     std::vector<dmrgk::Chunk> chunks;
     // device metadata (library-owned)
     dmrgk::Unit* units_dev = nullptr;
@@ -202,14 +203,20 @@ struct dmrgk_heff {
     dmrgk::DiagTask* dtasks_dev = nullptr;
     int64_t n_dblocks = 0;
     double* ident_dev = nullptr;       // identity block for IDENT_L / IDENT_R factors
-    cudaEvent_t ev_copy[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
+    cudaEvent_t ev_copy[3] = {nullptr, nullptr, nullptr}, ev_done[3] = {nullptr, nullptr, nullptr};
+    // phase 1 of chunk c+1 runs on a library-owned side stream concurrently with phase 2 of chunk c
+    // (T is double-buffered), so the tail of one launch is filled by the CTAs of the other
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_p1[2] = {nullptr, nullptr}, ev_p2[2] = {nullptr, nullptr};
+    cudaEvent_t ev_span[2] = {nullptr, nullptr};
+    bool span_open = false;
     int64_t n_launches = 0;
     bool has_pinned = false;
     // optional per-kernel timing (dmrgk_heff_profile): event pairs around every launch of apply
-    bool prof_on = false;
+    bool prof_on = false, prof_serial = false;
     std::vector<cudaEvent_t> prof_ev;      // pool, two per launch
-    std::vector<int> prof_kind;            // per recorded pair: 0 phase 1, 1 phase 2, 2 reduce
+    std::vector<int> prof_kind;            // per recorded pair: 0 phase 1, 1 phase 2, 2 reduce, 3 whole-apply span
     size_t prof_used = 0;                  // pairs recorded since the last read
-    double prof_ms[3] = {0, 0, 0};
-    int64_t prof_launches[3] = {0, 0, 0};
+    double prof_ms[4] = {0, 0, 0, 0};
+    int64_t prof_launches[4] = {0, 0, 0, 0};
 };

@@ -59,10 +59,16 @@ void dmrgk_heff_destroy(dmrgk_heff* h) {
     cudaFree(h->dblocks_dev);
     cudaFree(h->dtasks_dev);
     cudaFree(h->ident_dev);
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < 3; ++i) {
         if (h->ev_copy[i]) cudaEventDestroy(h->ev_copy[i]);
         if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
     }
+    for (int i = 0; i < 2; ++i) {
+        if (h->ev_p1[i]) cudaEventDestroy(h->ev_p1[i]);
+        if (h->ev_p2[i]) cudaEventDestroy(h->ev_p2[i]);
+    }
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->side) cudaStreamDestroy(h->side);
     for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
     delete h;
 }
@@ -83,7 +89,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     if (o.split_waves <= 0) o.split_waves = 8;
     if (o.ring_bytes < 0 || (o.kernel != 0 && o.kernel != 1))
         return fail(DMRGK_EINVAL, "heff_create: bad options");
-    const int64_t ring_half = (o.ring_bytes / 2) / 128 * 128;
+    const int64_t ring_part = (o.ring_bytes / 3) / 128 * 128;   // three parts: see dmrgk_heff_apply
 
     const dmrgk_space *SA = layout->A, *SB = layout->B;
     const std::vector<Block>& pb = layout->blocks;
@@ -106,9 +112,9 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
         for (const dmrgk_op* op : {(const dmrgk_op*)L[k], (const dmrgk_op*)R[k]}) {
             if (!op || op->n_padded == 0) continue;
             if (!op->dev && !op->pinned) return fail(DMRGK_ESTATE, "heff_create: pair %lld has an unbound operator", (long long)k);
-            if (op->pinned && ring_half == 0) return fail(DMRGK_ESTATE, "heff_create: pair %lld has a pinned operator but ring_bytes = 0", (long long)k);
-            if (op->pinned && op->n_padded * 8 > ring_half)
-                return fail(DMRGK_ENOMEM, "heff_create: pinned operator of %lld bytes exceeds half the ring (%lld)", (long long)(op->n_padded * 8), (long long)ring_half);
+            if (op->pinned && ring_part == 0) return fail(DMRGK_ESTATE, "heff_create: pair %lld has a pinned operator but ring_bytes = 0", (long long)k);
+            if (op->pinned && op->n_padded * 8 > ring_part)
+                return fail(DMRGK_ENOMEM, "heff_create: pinned operator of %lld bytes exceeds a third of the ring (%lld)", (long long)(op->n_padded * 8), (long long)ring_part);
         }
     }
 
@@ -148,7 +154,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     int64_t k0 = 0;
     while (k0 < K) {
         Chunk ch;
-        ch.ring_half = int(h->chunks.size() & 1);
+        ch.ring_part = int(h->chunks.size() % 3);
         std::vector<Task> tasks;
         std::unordered_map<const dmrgk_op*, int64_t> staged;   // pinned op → ring offset (bytes)
         int64_t ring_used = 0, t_bytes = 0;
@@ -234,7 +240,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 mine.push_back(t);
             }
             const bool nonempty = !tasks.empty() || !staged.empty();
-            if (nonempty && (t_bytes + tb > o.t_chunk_bytes || ring_used + need > ring_half)) break;
+            if (nonempty && (t_bytes + tb > o.t_chunk_bytes || ring_used + need > ring_part)) break;
             // accept pair k into the chunk
             for (const dmrgk_op* op : {(const dmrgk_op*)L[k], (const dmrgk_op*)R[k]})
                 if (op && op->pinned && op->n_padded && !staged.count(op)) {
@@ -290,7 +296,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 segs.push_back(t.s1);   // a staged A still lacks the ring base (added below)
                 t.s2.A = (unsigned long long)t_off[i];
                 const int ldt = pb[t.ib].ld;
-                const int64_t nkt = (t.m + 15) / 16;
+                const int64_t nkt = (t.m + TILE_K - 1) / TILE_K;
                 for (int i0 = 0; i0 < t.mo; i0 += TILE_M)
                     for (int j0 = 0; j0 < ldt; j0 += TILE_N) {
                         Unit u;
@@ -327,12 +333,12 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             int64_t total_cost = 0;
             for (size_t ob = 0; ob < pb.size(); ++ob) {
                 int64_t nkt = 0;
-                for (int i : by_ob[ob]) nkt += (tasks[i].n + 15) / 16;
+                for (int i : by_ob[ob]) nkt += (tasks[i].n + TILE_K - 1) / TILE_K;
                 for (int i0 = 0; i0 < pb[ob].rows; i0 += TILE_M)
                     for (int j0 = 0; j0 < pb[ob].ld; j0 += TILE_N)
                         total_cost += cost_of(std::min(TILE_M, pb[ob].rows - i0), std::min(TILE_N, pb[ob].ld - j0), nkt);
             }
-            const int64_t target = std::max<int64_t>(64 * 16, total_cost / std::max<int64_t>(1, slots * o.split_waves));
+            const int64_t target = std::max<int64_t>(64 * 256 / TILE_K, total_cost / std::max<int64_t>(1, slots * o.split_waves));
             struct U2 {
                 int64_t cost;
                 Unit u;
@@ -345,7 +351,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 std::vector<int64_t> prefix(1, 0);
                 for (int i : by_ob[ob]) {
                     segs.push_back(tasks[i].s2);
-                    prefix.push_back(prefix.back() + (tasks[i].n + 15) / 16);
+                    prefix.push_back(prefix.back() + (tasks[i].n + TILE_K - 1) / TILE_K);
                 }
                 const int ns = int(by_ob[ob].size());
                 const int64_t nkt = prefix.back();
@@ -453,19 +459,24 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     bool any_pinned = false;
     for (const Chunk& c : h->chunks) any_pinned |= !c.copies.empty();
     h->has_pinned = any_pinned;
-    h->ring_bytes = any_pinned ? 2 * ring_half : 0;
-    h->ring_half_bytes = ring_half;
-    h->workspace_bytes = std::max<int64_t>(128, h->t_bytes + h->partial_bytes + h->ring_bytes);
-    const unsigned long long part_base = (unsigned long long)h->t_bytes;
+    h->ring_bytes = any_pinned ? 3 * ring_part : 0;
+    h->ring_part_bytes = ring_part;
+    // workspace layout: [T buffer 0 | T buffer 1 | partial tiles | ring part 0 | 1 | 2]
+    h->workspace_bytes = std::max<int64_t>(128, 2 * h->t_bytes + h->partial_bytes + h->ring_bytes);
+    const unsigned long long part_base = (unsigned long long)(2 * h->t_bytes);
     const unsigned long long ring_base = part_base + (unsigned long long)h->partial_bytes;
 
     // rebase: chunk-local segment indices → global, partial offsets → workspace, ring offsets
-    for (const Chunk& c : h->chunks) {
-        const unsigned long long ring = ring_base + (unsigned long long)(c.ring_half) * ring_half;
+    for (size_t ci = 0; ci < h->chunks.size(); ++ci) {
+        const Chunk& c = h->chunks[ci];
+        const unsigned long long ring = ring_base + (unsigned long long)(c.ring_part) * ring_part;
+        const unsigned long long tbuf = (unsigned long long)(ci & 1) * (unsigned long long)h->t_bytes;
         for (int64_t i = c.p1_unit0; i < c.p1_unit0 + c.p1_units; ++i) {
             units[i].seg_begin += int32_t(c.p1_seg0);
             units[i].seg_end += int32_t(c.p1_seg0);
+            units[i].C += tbuf;                                   // phase 1 writes T buffer ci mod 2
         }
+        for (int64_t sgi = c.p2_seg0; sgi < c.p2_seg0 + c.p2_segs; ++sgi) segs[sgi].A += tbuf;   // phase 2 reads it
         for (int64_t i = c.p2_unit0; i < c.p2_unit0 + c.p2_units; ++i) {
             units[i].seg_begin += int32_t(c.p2_seg0);
             units[i].seg_end += int32_t(c.p2_seg0);
@@ -493,12 +504,19 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     if (s == DMRGK_OK) s = upload(dblocks, &h->dblocks_dev);
     if (s == DMRGK_OK) s = upload(dtasks, &h->dtasks_dev);
     if (s != DMRGK_OK) return bail(s);
-    if (any_pinned)
-        for (int i = 0; i < 2; ++i) {
-            cudaError_t e = cudaEventCreateWithFlags(&h->ev_copy[i], cudaEventDisableTiming);
-            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming);
-            if (e != cudaSuccess) return bail(fail(DMRGK_ECUDA, "heff_create: event: %s", cudaGetErrorString(e)));
+    {
+        cudaError_t e = cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming);
+        for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+            e = cudaEventCreateWithFlags(&h->ev_p1[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_p2[i], cudaEventDisableTiming);
         }
+        for (int i = 0; i < 3 && e == cudaSuccess && any_pinned; ++i) {
+            e = cudaEventCreateWithFlags(&h->ev_copy[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) return bail(fail(DMRGK_ECUDA, "heff_create: stream/event: %s", cudaGetErrorString(e)));
+    }
     *out = h;
     return DMRGK_OK;
 }
@@ -523,20 +541,23 @@ namespace dmrgk {
 
 // Stage the pinned operators of chunk c into its ring half on the copy stream, ordered after the
 // last compute that read that half and before the compute that needs it (a3).
-static int32_t stage_chunk(dmrgk_heff* h, const Chunk& c, char* ws, cudaStream_t main, cudaStream_t copy) {
+static int32_t stage_chunk(dmrgk_heff* h, const Chunk& c, char* ws, cudaStream_t main, cudaStream_t copy,
+                           cudaStream_t side = nullptr) {
     if (c.copies.empty()) return DMRGK_OK;
-    const int hf = c.ring_half;
-    char* ring = ws + h->t_bytes + h->partial_bytes + int64_t(hf) * h->ring_half_bytes;
+    const int hf = c.ring_part;
+    char* ring = ws + 2 * h->t_bytes + h->partial_bytes + int64_t(hf) * h->ring_part_bytes;
     if (h->done_recorded[hf]) DMRGK_CUDA(cudaStreamWaitEvent(copy, h->ev_done[hf], 0));
     for (const StageCopy& sc : c.copies)
         DMRGK_CUDA(cudaMemcpyAsync(ring + sc.ring_off * 8, sc.src_host, size_t(sc.n) * 8, cudaMemcpyHostToDevice, copy));
     DMRGK_CUDA(cudaEventRecord(h->ev_copy[hf], copy));
     DMRGK_CUDA(cudaStreamWaitEvent(main, h->ev_copy[hf], 0));
+    if (side) DMRGK_CUDA(cudaStreamWaitEvent(side, h->ev_copy[hf], 0));
     return DMRGK_OK;
 }
 
 // Profiling (dmrgk_heff_profile): an event pair around one launch; the pool grows on demand.
-static int32_t prof_begin(dmrgk_heff* h, int kind, cudaStream_t main) {
+static int32_t prof_begin(dmrgk_heff* h, int kind, cudaStream_t st, size_t* slot) {
+    *slot = 0;
     if (!h->prof_on) return DMRGK_OK;
     while (h->prof_ev.size() < 2 * (h->prof_used + 1)) {
         cudaEvent_t e;
@@ -544,14 +565,14 @@ static int32_t prof_begin(dmrgk_heff* h, int kind, cudaStream_t main) {
         h->prof_ev.push_back(e);
     }
     if (h->prof_kind.size() <= h->prof_used) h->prof_kind.resize(h->prof_used + 1);
-    h->prof_kind[h->prof_used] = kind;
-    DMRGK_CUDA(cudaEventRecord(h->prof_ev[2 * h->prof_used], main));
+    *slot = h->prof_used++;
+    h->prof_kind[*slot] = kind;
+    DMRGK_CUDA(cudaEventRecord(h->prof_ev[2 * *slot], st));
     return DMRGK_OK;
 }
-static int32_t prof_end(dmrgk_heff* h, cudaStream_t main) {
+static int32_t prof_end(dmrgk_heff* h, size_t slot, cudaStream_t st) {
     if (!h->prof_on) return DMRGK_OK;
-    DMRGK_CUDA(cudaEventRecord(h->prof_ev[2 * h->prof_used + 1], main));
-    ++h->prof_used;
+    DMRGK_CUDA(cudaEventRecord(h->prof_ev[2 * slot + 1], st));
     return DMRGK_OK;
 }
 // Fold the recorded pairs into the running sums (synchronises on the last event).
@@ -569,8 +590,8 @@ static int32_t prof_collect(dmrgk_heff* h) {
 
 static int32_t chunk_done(dmrgk_heff* h, const Chunk& c, cudaStream_t main) {
     if (c.copies.empty()) return DMRGK_OK;
-    DMRGK_CUDA(cudaEventRecord(h->ev_done[c.ring_half], main));
-    h->done_recorded[c.ring_half] = true;
+    DMRGK_CUDA(cudaEventRecord(h->ev_done[c.ring_part], main));
+    h->done_recorded[c.ring_part] = true;
     return DMRGK_OK;
 }
 
@@ -598,28 +619,48 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
     bases.b[BASE_PSI] = (unsigned long long)(uintptr_t)psi_dev;
     bases.b[BASE_SIGMA] = (unsigned long long)(uintptr_t)sigma_dev;
     DMRGK_CUDA(cudaMemsetAsync(sigma_dev, 0, size_t(n) * 8, main));
-    // copies of chunk c+1 are enqueued before the compute of chunk c so that they overlap it
+    // Stream choreography (all ordering by events; `side` is library-owned and non-blocking):
+    //   side : p1(0)            p1(1)              p1(2) …      phase 1 of chunk c → T buffer c mod 2
+    //   main :        p2(0) r(0)       p2(1) r(1) …             phase 2 + reduce of chunk c
+    // p2(c) waits for p1(c); p1(c+2) waits for p2(c) (T buffer re-use); p1(c+1) overlaps p2(c), so
+    // the CTAs of one grid fill the tail of the other.  Everything side does is awaited by main
+    // before apply's last launch, so the caller only ever has to order against `main`.
+    // Copies of chunk c+1 are enqueued before the compute of chunk c so that they overlap it.
     const size_t nc = h->chunks.size();
-    if (nc) DMRGK_TRY(stage_chunk(h, h->chunks[0], (char*)workspace_dev, main, copy));
+    const bool serial = h->prof_on && h->prof_serial;   // diagnostic mode: one stream, per-launch events
+    cudaStream_t side = serial ? main : h->side;
+    DMRGK_CUDA(cudaEventRecord(h->ev_fork, main));
+    DMRGK_CUDA(cudaStreamWaitEvent(side, h->ev_fork, 0));
+    size_t span_slot = 0, slot = 0;
+    DMRGK_TRY(prof_begin(h, 3, main, &span_slot));
+    if (nc) DMRGK_TRY(stage_chunk(h, h->chunks[0], (char*)workspace_dev, main, copy, side));
     for (size_t c = 0; c < nc; ++c) {
         const Chunk& ch = h->chunks[c];
         if (ch.p1_units) {
-            DMRGK_TRY(prof_begin(h, 0, main));
-            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, main));
-            DMRGK_TRY(prof_end(h, main));
+            if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(side, h->ev_p2[c & 1], 0));
+            if (serial) DMRGK_TRY(prof_begin(h, 0, side, &slot));
+            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, side));
+            if (serial) DMRGK_TRY(prof_end(h, slot, side));
+            DMRGK_CUDA(cudaEventRecord(h->ev_p1[c & 1], side));
+            DMRGK_CUDA(cudaStreamWaitEvent(main, h->ev_p1[c & 1], 0));
         }
-        if (ch.p2_units) {
-            DMRGK_TRY(prof_begin(h, 1, main));
-            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, main));
-            DMRGK_TRY(prof_end(h, main));
-        }
-        if (ch.r_units) {
-            DMRGK_TRY(prof_begin(h, 2, main));
-            DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, main));
-            DMRGK_TRY(prof_end(h, main));
-        }
+        if (serial && ch.p2_units) DMRGK_TRY(prof_begin(h, 1, main, &slot));
+        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, main));
+        if (serial && ch.p2_units) DMRGK_TRY(prof_end(h, slot, main));
+        if (serial && ch.r_units) DMRGK_TRY(prof_begin(h, 2, main, &slot));
+        DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, main));
+        if (serial && ch.r_units) DMRGK_TRY(prof_end(h, slot, main));
+        DMRGK_CUDA(cudaEventRecord(h->ev_p2[c & 1], main));
         DMRGK_TRY(chunk_done(h, ch, main));
-        if (c + 1 < nc) DMRGK_TRY(stage_chunk(h, h->chunks[c + 1], (char*)workspace_dev, main, copy));
+        if (c + 1 < nc) DMRGK_TRY(stage_chunk(h, h->chunks[c + 1], (char*)workspace_dev, main, copy, side));
+    }
+    DMRGK_TRY(prof_end(h, span_slot, main));
+    if (h->prof_on && !serial) {
+        for (const Chunk& ch : h->chunks) {
+            h->prof_launches[0] += ch.p1_units > 0;
+            h->prof_launches[1] += ch.p2_units > 0;
+            h->prof_launches[2] += ch.r_units > 0;
+        }
     }
     return DMRGK_OK;
 }
@@ -628,7 +669,8 @@ int32_t dmrgk_heff_profile(dmrgk_heff* h, int32_t enable) {
     if (!h) return fail(DMRGK_EINVAL, "heff_profile: heff is NULL");
     if (h->prof_used) DMRGK_TRY(prof_collect(h));
     h->prof_on = enable != 0;
-    for (int i = 0; i < 3; ++i) {
+    h->prof_serial = enable == 2;
+    for (int i = 0; i < 4; ++i) {
         h->prof_ms[i] = 0.0;
         h->prof_launches[i] = 0;
     }
@@ -638,7 +680,7 @@ int32_t dmrgk_heff_profile(dmrgk_heff* h, int32_t enable) {
 int32_t dmrgk_heff_profile_read(dmrgk_heff* h, double* ms, int64_t* launches) {
     if (!h) return fail(DMRGK_EINVAL, "heff_profile_read: heff is NULL");
     DMRGK_TRY(prof_collect(h));
-    for (int i = 0; i < 3; ++i) {
+    for (int i = 0; i < 4; ++i) {
         if (ms) ms[i] = h->prof_ms[i];
         if (launches) launches[i] = h->prof_launches[i];
     }

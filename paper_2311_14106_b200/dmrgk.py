@@ -309,15 +309,16 @@ class Heff:
         check(self.lib.dmrgk_heff_apply_host(self.h, _dev(psi_host), _dev(sigma_host), _dev(psi), _dev(sigma),
                                              _dev(workspace), _stream(stream_main), _stream(stream_copy)))
 
-    def profile(self, enable=True):
-        check(self.lib.dmrgk_heff_profile(self.h, int(bool(enable))))
+    def profile(self, enable=1):
+        """0 off, 1 whole-apply span with normal overlap, 2 serialised per-launch timing."""
+        check(self.lib.dmrgk_heff_profile(self.h, int(enable)))
 
     def profile_read(self):
-        """({"p1","p2","reduce"} → ms, same → launch counts) accumulated since profile()."""
-        ms = np.zeros(3, np.float64)
-        ln = np.zeros(3, np.int64)
+        """({"p1","p2","reduce","apply"} → ms, same → launch counts) accumulated since profile()."""
+        ms = np.zeros(4, np.float64)
+        ln = np.zeros(4, np.int64)
         check(self.lib.dmrgk_heff_profile_read(self.h, ms.ctypes.data, ln.ctypes.data))
-        names = ("p1", "p2", "reduce")
+        names = ("p1", "p2", "reduce", "apply")
         return dict(zip(names, ms.tolist())), dict(zip(names, ln.tolist()))
 
     def diag(self, diag, workspace, stream_main=None, stream_copy=None):

@@ -184,12 +184,12 @@ def test_staged_operators_bit_identical_to_resident():
     pinned = [i for i in range(len(wl.ops)) if i % 3 == 1]
     stg = problem.from_workload(wl, pinned=pinned, ring_bytes=256 << 20, t_chunk_bytes=1 << 20)
     assert stg.heff.n_chunks == res.heff.n_chunks > 2
-    for _ in range(2):      # second call re-uses the ring halves
+    for _ in range(2):      # second call re-uses the ring parts
         got = stg.apply(stg.psi_fill(wl.seed, wlmod.PSI_STREAM))
         torch.cuda.synchronize()
         assert torch.equal(got, ref)
     assert torch.equal(stg.diag(), res.diag())
-    small = problem.from_workload(wl, pinned=pinned, ring_bytes=1300000, t_chunk_bytes=1 << 20)
+    small = problem.from_workload(wl, pinned=pinned, ring_bytes=2000000, t_chunk_bytes=1 << 20)
     assert small.heff.n_chunks >= res.heff.n_chunks
     first = small.apply(psi).clone()
     again = small.apply(psi)
