@@ -267,6 +267,40 @@ def run_ours(args):
     sm_max = clk.get("sm_max_mhz") or 1965.0
     peak = n_sm * 128 * sm_max * 1e6 / 1e12     # 64 DFMA-equivalents/clk/SM
 
+    # ---- a8 vector kernels alone: achieved HBM GB/s against MEASURED_PEAKS.json hbm_gbs ------------
+    def time_vec(fn, reps=10):
+        fn()
+        torch.cuda.synchronize()
+        v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        v0.record(dp.stream)
+        for _ in range(reps):
+            fn()
+        v1.record(dp.stream)
+        torch.cuda.synchronize()
+        return v0.elapsed_time(v1) / reps
+    mv = min(8, args.m_max)
+    scratch = torch.empty(dmrgk.vec_scratch_bytes(mv + 1), dtype=torch.uint8, device="cuda")
+    outv = torch.zeros(64, dtype=torch.float64, device="cuda")
+    coefv = torch.full((64,), 0.125, dtype=torch.float64, device="cuda")
+    yv = dp.new_vector()
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        hbm_peak, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
+    t_dot = time_vec(lambda: dmrgk.vec_multi_dot(dp.ctx, n, mv, dp.V, n, psi, outv, scratch, dp.stream))
+    t_axpy = time_vec(lambda: dmrgk.vec_multi_axpy(dp.ctx, n, mv, dp.V, n, coefv, -1.0, 1.0, yv, dp.stream))
+    t_res = time_vec(lambda: dmrgk.vec_residual(dp.ctx, n, mv, dp.V, dp.W, n, coefv, yv, outv, scratch, dp.stream))
+    gbs = lambda nvec, ms: nvec * n * 8 / ms / 1e6
+    vec = {"n_doubles": int(n), "m": mv, "peak_gbs": hbm_peak, "peak_source": hbm_src,
+           "multi_dot": {"ms": t_dot, "gbs": gbs(mv + 1, t_dot), "frac": gbs(mv + 1, t_dot) / hbm_peak},
+           "multi_axpy": {"ms": t_axpy, "gbs": gbs(mv + 2, t_axpy), "frac": gbs(mv + 2, t_axpy) / hbm_peak},
+           "residual": {"ms": t_res, "gbs": gbs(2 * mv + 1, t_res), "frac": gbs(2 * mv + 1, t_res) / hbm_peak}}
+
+    # dram__bytes_read.sum + dram__bytes_write.sum per GEMM launch from the committed ncu --set full
+    # capture of this workload (profiles/r1_v3_summary.md); other workloads have no capture
+    traffic = 12.78e9 if args.config == "4" else None
+
     # device time of the GEMM region of the applies (phase-1/phase-2 launches overlap on two streams, so
     # per-launch durations are not additive; the span from the first to the last launch of each apply
     # is what is timed, and it includes the split-k reduce launches)
@@ -294,7 +328,10 @@ def run_ours(args):
                                     "MEASURED_PEAKS.json); in-run register-only DMMA probe below corroborates",
                      "dmma_probe_tflops": dmma_probe, "launches": int(gemm_n), "avg_launch_ms": gemm_ms / max(gemm_n, 1),
                      "kernel_ms_per_step": gemm_ms / args.steps, "reduce_launches": int(prof_n["reduce"]),
-                     "traffic": None},
+                     "traffic": traffic, "traffic_note": "average over the 48 GEMM launches of one apply (ncu, cold cache); "
+                     "algorithmic bytes per launch = 4.2e9 (operators read once per task + psi + sigma); the excess is the T "
+                     "round trip and tile re-reads that miss L2 - 0.93 TB/s in total, 14 % of HBM, not the bound"},
+        "vector_kernels": vec,
         "clocks": clk,
     }
     if rank == 0 and world == 1 and not args.no_cpu:
