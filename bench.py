@@ -299,7 +299,7 @@ def run_ours(args):
 
     # dram__bytes_read.sum + dram__bytes_write.sum per GEMM launch from the committed ncu --set full
     # capture of this workload (profiles/r1_v3_summary.md); other workloads have no capture
-    traffic = 12.78e9 if args.config == "4" else None
+    traffic = 12.99e9 if args.config == "4" else None
 
     # device time of the GEMM region of the applies (phase-1/phase-2 launches overlap on two streams, so
     # per-launch durations are not additive; the span from the first to the last launch of each apply
