@@ -244,6 +244,8 @@ def run_ours(args):
     for _ in range(2):
         h.apply_host(ph, sh, pdev, sdev, dp.workspace, dp.stream, dp.copy_stream)
     barrier()
+    clocks_e2e = ClockSampler(local)
+    clocks_e2e.start()
     e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e2.record(dp.stream)
     for _ in range(args.steps):
@@ -251,6 +253,7 @@ def run_ours(args):
     e3.record(dp.stream)
     barrier()
     ms_e2e = e2.elapsed_time(e3) / args.steps
+    clk_e2e = clocks_e2e.stop()
     ms_e2e = max_over_ranks(ms_e2e, world, "cuda")
 
     # ---- the FP64 ceiling of this box, live: register-only DMMA loop (burst) -------------------
@@ -320,7 +323,7 @@ def run_ours(args):
         "pct_of_fp64_peak": 100.0 * value / world / peak,
         "e2e": {"value": world * h.flops_alg / ms_e2e / 1e9, "unit": UNIT, "ms_per_step": ms_e2e,
                 "what": "dmrgk_heff_apply_host: pinned ψ H2D, apply, σ D2H",
-                "h2d_bytes_per_step": int(n * 8), "d2h_bytes_per_step": int(n * 8)},
+                "h2d_bytes_per_step": int(n * 8), "d2h_bytes_per_step": int(n * 8), "clocks": clk_e2e},
         "gpu_launches": int(launches),
         "roofline": {"bound": "tensor", "kernel": "heff_gemm_dmma_kernel (a5 + a6)", "achieved": achieved,
                      "peak": peak, "unit": "TFLOP/s", "frac": (achieved / peak) if achieved else None,

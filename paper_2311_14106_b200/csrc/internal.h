@@ -206,7 +206,9 @@ struct dmrgk_heff {
     cudaEvent_t ev_copy[3] = {nullptr, nullptr, nullptr}, ev_done[3] = {nullptr, nullptr, nullptr};
     // phase 1 of chunk c+1 runs on a library-owned side stream concurrently with phase 2 of chunk c
     // (T is double-buffered), so the tail of one launch is filled by the CTAs of the other
-    cudaStream_t side = nullptr;
+    cudaStream_t side = nullptr;       // phase 1 (lowest priority)
+    cudaStream_t side_hi = nullptr;    // phase 2 + reduce (greatest priority: its CTAs are dispatched first)
+    cudaEvent_t ev_join = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_p1[2] = {nullptr, nullptr}, ev_p2[2] = {nullptr, nullptr};
     cudaEvent_t ev_span[2] = {nullptr, nullptr};
     bool span_open = false;

@@ -68,7 +68,9 @@ void dmrgk_heff_destroy(dmrgk_heff* h) {
         if (h->ev_p2[i]) cudaEventDestroy(h->ev_p2[i]);
     }
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->ev_join) cudaEventDestroy(h->ev_join);
     if (h->side) cudaStreamDestroy(h->side);
+    if (h->side_hi) cudaStreamDestroy(h->side_hi);
     for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
     delete h;
 }
@@ -505,8 +507,12 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     if (s == DMRGK_OK) s = upload(dtasks, &h->dtasks_dev);
     if (s != DMRGK_OK) return bail(s);
     {
-        cudaError_t e = cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking);
+        int prio_lo = 0, prio_hi = 0;
+        cudaError_t e = cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&h->side, cudaStreamNonBlocking, prio_lo);
+        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&h->side_hi, cudaStreamNonBlocking, prio_hi);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming);
         for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
             e = cudaEventCreateWithFlags(&h->ev_p1[i], cudaEventDisableTiming);
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_p2[i], cudaEventDisableTiming);
@@ -542,7 +548,7 @@ namespace dmrgk {
 // Stage the pinned operators of chunk c into its ring half on the copy stream, ordered after the
 // last compute that read that half and before the compute that needs it (a3).
 static int32_t stage_chunk(dmrgk_heff* h, const Chunk& c, char* ws, cudaStream_t main, cudaStream_t copy,
-                           cudaStream_t side = nullptr) {
+                           cudaStream_t side = nullptr, cudaStream_t side2 = nullptr) {
     if (c.copies.empty()) return DMRGK_OK;
     const int hf = c.ring_part;
     char* ring = ws + 2 * h->t_bytes + h->partial_bytes + int64_t(hf) * h->ring_part_bytes;
@@ -552,6 +558,7 @@ static int32_t stage_chunk(dmrgk_heff* h, const Chunk& c, char* ws, cudaStream_t
     DMRGK_CUDA(cudaEventRecord(h->ev_copy[hf], copy));
     DMRGK_CUDA(cudaStreamWaitEvent(main, h->ev_copy[hf], 0));
     if (side) DMRGK_CUDA(cudaStreamWaitEvent(side, h->ev_copy[hf], 0));
+    if (side2) DMRGK_CUDA(cudaStreamWaitEvent(side2, h->ev_copy[hf], 0));
     return DMRGK_OK;
 }
 
@@ -619,40 +626,49 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
     bases.b[BASE_PSI] = (unsigned long long)(uintptr_t)psi_dev;
     bases.b[BASE_SIGMA] = (unsigned long long)(uintptr_t)sigma_dev;
     DMRGK_CUDA(cudaMemsetAsync(sigma_dev, 0, size_t(n) * 8, main));
-    // Stream choreography (all ordering by events; `side` is library-owned and non-blocking):
-    //   side : p1(0)            p1(1)              p1(2) …      phase 1 of chunk c → T buffer c mod 2
-    //   main :        p2(0) r(0)       p2(1) r(1) …             phase 2 + reduce of chunk c
-    // p2(c) waits for p1(c); p1(c+2) waits for p2(c) (T buffer re-use); p1(c+1) overlaps p2(c), so
-    // the CTAs of one grid fill the tail of the other.  Everything side does is awaited by main
-    // before apply's last launch, so the caller only ever has to order against `main`.
+    // Stream choreography (all ordering by events; s1 and s2 are library-owned, non-blocking):
+    //   s1 (lowest priority)  : p1(0)            p1(1)              p1(2) …   phase 1 of chunk c → T buffer c mod 2
+    //   s2 (greatest priority):        p2(0) r(0)       p2(1) r(1) …          phase 2 + reduce of chunk c
+    // p2(c) waits for p1(c); p1(c+2) waits for p2(c) (T buffer re-use); p1(c+1) overlaps p2(c).  s2's
+    // priority makes the block scheduler dispatch the few long stacked-k units of p2(c) first and fill
+    // the remaining slots — and the tail — with the many short units of p1(c+1).  The caller's stream
+    // forks into s1/s2 after the memset of σ and joins them before apply returns, so the caller only
+    // ever has to order against `main`.
     // Copies of chunk c+1 are enqueued before the compute of chunk c so that they overlap it.
     const size_t nc = h->chunks.size();
     const bool serial = h->prof_on && h->prof_serial;   // diagnostic mode: one stream, per-launch events
-    cudaStream_t side = serial ? main : h->side;
-    DMRGK_CUDA(cudaEventRecord(h->ev_fork, main));
-    DMRGK_CUDA(cudaStreamWaitEvent(side, h->ev_fork, 0));
+    cudaStream_t s1 = serial ? main : h->side, s2 = serial ? main : h->side_hi;
     size_t span_slot = 0, slot = 0;
     DMRGK_TRY(prof_begin(h, 3, main, &span_slot));
-    if (nc) DMRGK_TRY(stage_chunk(h, h->chunks[0], (char*)workspace_dev, main, copy, side));
+    DMRGK_CUDA(cudaEventRecord(h->ev_fork, main));
+    if (!serial) {
+        DMRGK_CUDA(cudaStreamWaitEvent(s1, h->ev_fork, 0));
+        DMRGK_CUDA(cudaStreamWaitEvent(s2, h->ev_fork, 0));
+    }
+    if (nc) DMRGK_TRY(stage_chunk(h, h->chunks[0], (char*)workspace_dev, main, copy, s1, s2));
     for (size_t c = 0; c < nc; ++c) {
         const Chunk& ch = h->chunks[c];
         if (ch.p1_units) {
-            if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(side, h->ev_p2[c & 1], 0));
-            if (serial) DMRGK_TRY(prof_begin(h, 0, side, &slot));
-            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, side));
-            if (serial) DMRGK_TRY(prof_end(h, slot, side));
-            DMRGK_CUDA(cudaEventRecord(h->ev_p1[c & 1], side));
-            DMRGK_CUDA(cudaStreamWaitEvent(main, h->ev_p1[c & 1], 0));
+            if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(s1, h->ev_p2[c & 1], 0));
+            if (serial) DMRGK_TRY(prof_begin(h, 0, s1, &slot));
+            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, s1));
+            if (serial) DMRGK_TRY(prof_end(h, slot, s1));
+            DMRGK_CUDA(cudaEventRecord(h->ev_p1[c & 1], s1));
+            DMRGK_CUDA(cudaStreamWaitEvent(s2, h->ev_p1[c & 1], 0));
         }
-        if (serial && ch.p2_units) DMRGK_TRY(prof_begin(h, 1, main, &slot));
-        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, main));
-        if (serial && ch.p2_units) DMRGK_TRY(prof_end(h, slot, main));
-        if (serial && ch.r_units) DMRGK_TRY(prof_begin(h, 2, main, &slot));
-        DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, main));
-        if (serial && ch.r_units) DMRGK_TRY(prof_end(h, slot, main));
-        DMRGK_CUDA(cudaEventRecord(h->ev_p2[c & 1], main));
-        DMRGK_TRY(chunk_done(h, ch, main));
-        if (c + 1 < nc) DMRGK_TRY(stage_chunk(h, h->chunks[c + 1], (char*)workspace_dev, main, copy, side));
+        if (serial && ch.p2_units) DMRGK_TRY(prof_begin(h, 1, s2, &slot));
+        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, s2));
+        if (serial && ch.p2_units) DMRGK_TRY(prof_end(h, slot, s2));
+        if (serial && ch.r_units) DMRGK_TRY(prof_begin(h, 2, s2, &slot));
+        DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, s2));
+        if (serial && ch.r_units) DMRGK_TRY(prof_end(h, slot, s2));
+        DMRGK_CUDA(cudaEventRecord(h->ev_p2[c & 1], s2));
+        DMRGK_TRY(chunk_done(h, ch, s2));
+        if (c + 1 < nc) DMRGK_TRY(stage_chunk(h, h->chunks[c + 1], (char*)workspace_dev, main, copy, s1, s2));
+    }
+    if (!serial) {
+        DMRGK_CUDA(cudaEventRecord(h->ev_join, s2));      // s2 has waited for every p1 launch of s1
+        DMRGK_CUDA(cudaStreamWaitEvent(main, h->ev_join, 0));
     }
     DMRGK_TRY(prof_end(h, span_slot, main));
     if (h->prof_on && !serial) {
