@@ -122,7 +122,9 @@ enum {
 
 typedef struct dmrgk_heff_opts {
     int64_t t_chunk_bytes;  /* cap on the L_k·ψ intermediate workspace per chunk of pairs
-                               (0 = default 4 GiB); pairs are processed chunk by chunk       */
+                               (0 = default: about 1/16 of the total, clamped to
+                               [512 MiB, 4 GiB]); pairs are processed chunk by chunk and the
+                               workspace holds two such buffers                             */
     int64_t ring_bytes;     /* staging ring for pinned operators, split in three parts
                                (0 = no ring: binding a pinned operator is then an error)     */
     int32_t kernel;         /* 0 = DMMA tensor-core kernel (product path),

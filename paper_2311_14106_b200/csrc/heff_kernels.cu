@@ -327,24 +327,36 @@ heff_gemm_scalar_kernel(const Unit* __restrict__ units, const Seg* __restrict__ 
     }
 }
 
-// a7: fixed-order sum of split-k partial tiles, σ_tile += Σ_s P_s (s ascending).
+// a7: fixed-order sum of split-k partial tiles, σ_tile += Σ_s P_s (s ascending).  Eight CTAs per tile
+// (one 8-row slab each, one double2 per thread) so that even a handful of output tiles fills the GPU;
+// the partial loads of four splits are issued together, the additions stay in split order.
+constexpr int RED_SLABS = BM / 8;
 __global__ void __launch_bounds__(256)
 heff_reduce_kernel(const RUnit* __restrict__ runits, Bases bases) {
-    const RUnit u = runits[blockIdx.x];
-    double* C = reinterpret_cast<double*>(bases.b[BASE_SIGMA] + u.C);
-    const double* P = reinterpret_cast<const double*>(bases.b[BASE_WS] + u.P);
-    const int half_cols = u.cols >> 1;   // cols is even (multiple of 16 or tile width 64)
-    for (int e = threadIdx.x; e < u.rows * half_cols; e += 256) {
-        const int r = e / half_cols, c = (e % half_cols) * 2;
-        double2* p = reinterpret_cast<double2*>(C + int64_t(r) * u.ldc + c);
-        double2 v = *p;
-        for (int s = 0; s < u.n_split; ++s) {
-            const double2 q = *reinterpret_cast<const double2*>(P + int64_t(s) * (BM * BN) + r * BN + c);
-            v.x += q.x;
-            v.y += q.y;
+    const RUnit u = runits[blockIdx.x / RED_SLABS];
+    const int r = (blockIdx.x % RED_SLABS) * 8 + (threadIdx.x >> 5);
+    const int c = (threadIdx.x & 31) * 2;
+    if (r >= u.rows || c >= u.cols) return;   // cols is even (multiple of 16 or the tile width 64)
+    double2* p = reinterpret_cast<double2*>(reinterpret_cast<double*>(bases.b[BASE_SIGMA] + u.C) + int64_t(r) * u.ldc + c);
+    const double2* P = reinterpret_cast<const double2*>(reinterpret_cast<const double*>(bases.b[BASE_WS] + u.P) + r * BN + c);
+    double2 v = *p;
+    int s = 0;
+    for (; s + 4 <= u.n_split; s += 4) {
+        double2 q[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) q[j] = P[int64_t(s + j) * (BM * BN / 2)];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            v.x += q[j].x;
+            v.y += q[j].y;
         }
-        *p = v;
     }
+    for (; s < u.n_split; ++s) {
+        const double2 q = P[int64_t(s) * (BM * BN / 2)];
+        v.x += q.x;
+        v.y += q.y;
+    }
+    *p = v;
 }
 
 // a4: diag(H_eff)[i, j] += Σ_t alpha_t · L_t[i, i] · R_t[j, j] over the block's diagonal tasks.
@@ -405,7 +417,7 @@ int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev
 
 int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cudaStream_t st) {
     if (n <= 0) return DMRGK_OK;
-    heff_reduce_kernel<<<unsigned(n), 256, 0, st>>>(runits_dev, bases);
+    heff_reduce_kernel<<<unsigned(n * RED_SLABS), 256, 0, st>>>(runits_dev, bases);
     count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;

@@ -87,7 +87,6 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     dmrgk_heff_opts o;
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
-    if (o.t_chunk_bytes <= 0) o.t_chunk_bytes = int64_t(4) << 30;
     if (o.split_waves <= 0) o.split_waves = 8;
     if (o.ring_bytes < 0 || (o.kernel != 0 && o.kernel != 1))
         return fail(DMRGK_EINVAL, "heff_create: bad options");
@@ -153,6 +152,98 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     const int64_t slots = int64_t(ctx->n_sm) * 3;
     int64_t max_t_bytes = 0, max_partial_tiles = 0;
 
+    // Tasks of pair k (every ψ block whose L and R blocks exist and whose output block is in the layout)
+    // and the bytes of their T intermediates.  Enumerated once for all pairs: the total decides the
+    // default chunk size, the chunk loop below then only groups the pairs.
+    auto tasks_of_pair = [&](int64_t k, std::vector<Task>& mine) -> int64_t {
+        const uint32_t f = flags[k];
+        int64_t tb = 0;
+        for (int ib = 0; ib < int(pb.size()); ++ib) {
+            const int a = pb[ib].r_idx, b = pb[ib].c_idx;
+            Task t;
+            memset(&t, 0, sizeof(t));
+            t.k = int32_t(k);
+            t.ib = ib;
+            t.m = pb[ib].rows;
+            t.n = pb[ib].cols;
+            int ao, bo;
+            // L applied to sector a
+            if (!L[k]) {
+                ao = a;
+                t.mo = t.m;
+                t.s1.A = (unsigned long long)(uintptr_t)h->ident_dev;
+                t.s1.lda = ident_ld;
+                t.s1.flags = BASE_ABS << SEG_A_SEL_SHIFT;
+            } else {
+                const int bi = (f & DMRGK_TRANS_L) ? L[k]->by_row[a] : L[k]->by_col[a];
+                if (bi < 0) continue;
+                const Block& lb = L[k]->blocks[bi];
+                ao = (f & DMRGK_TRANS_L) ? lb.c_idx : lb.r_idx;
+                t.mo = (f & DMRGK_TRANS_L) ? lb.cols : lb.rows;
+                t.s1.lda = lb.ld;
+                t.s1.flags = (f & DMRGK_TRANS_L) ? SEG_A_MMAJOR : 0u;
+                if (L[k]->dev) {
+                    t.s1.A = (unsigned long long)(uintptr_t)(L[k]->dev + lb.off);
+                    t.s1.flags |= BASE_ABS << SEG_A_SEL_SHIFT;
+                } else {
+                    t.s1.A = (unsigned long long)(lb.off * 8);   // ring offset added below
+                    t.s1.flags |= BASE_WS << SEG_A_SEL_SHIFT;
+                }
+            }
+            if (!R[k]) {
+                bo = b;
+                t.no = t.n;
+                t.s2.B = (unsigned long long)(uintptr_t)h->ident_dev;
+                t.s2.ldb = ident_ld;
+                t.s2.flags = BASE_ABS << SEG_B_SEL_SHIFT;
+            } else {
+                const int bi = (f & DMRGK_TRANS_R) ? R[k]->by_row[b] : R[k]->by_col[b];
+                if (bi < 0) continue;
+                const Block& rb = R[k]->blocks[bi];
+                bo = (f & DMRGK_TRANS_R) ? rb.c_idx : rb.r_idx;
+                t.no = (f & DMRGK_TRANS_R) ? rb.cols : rb.rows;
+                t.s2.ldb = rb.ld;
+                t.s2.flags = (f & DMRGK_TRANS_R) ? SEG_B_NMAJOR : 0u;
+                if (R[k]->dev) {
+                    t.s2.B = (unsigned long long)(uintptr_t)(R[k]->dev + rb.off);
+                    t.s2.flags |= BASE_ABS << SEG_B_SEL_SHIFT;
+                } else {
+                    t.s2.B = (unsigned long long)(rb.off * 8);
+                    t.s2.flags |= BASE_WS << SEG_B_SEL_SHIFT;
+                }
+            }
+            const int ob = layout->by_a[ao];
+            if (ob < 0 || pb[ob].c_idx != bo) continue;
+            t.ob = ob;
+            const int par = L[k] ? L[k]->parity : (R[k] ? R[k]->parity : 0);
+            t.alpha = coef[k] * ((par && SA->parity(a)) ? -1.0 : 1.0);
+            t.diag = (ob == ib);
+            // phase-1 B operand = ψ block (N-major), phase-2 A operand = T (K-major, set per chunk)
+            t.s1.B = (unsigned long long)(pb[ib].off * 8);
+            t.s1.ldb = pb[ib].ld;
+            t.s1.klen = t.m;
+            t.s1.flags |= SEG_B_NMAJOR | (BASE_PSI << SEG_B_SEL_SHIFT);
+            t.s2.lda = pb[ib].ld;
+            t.s2.klen = t.n;
+            t.s2.flags |= BASE_WS << SEG_A_SEL_SHIFT;
+            tb += int64_t(t.mo) * pb[ib].ld * 8;
+            mine.push_back(t);
+        }
+        return tb;
+    };
+    std::vector<std::vector<Task>> pair_tasks(static_cast<size_t>(K));
+    std::vector<int64_t> pair_tb(static_cast<size_t>(K), 0);
+    int64_t total_tb = 0;
+    for (int64_t k = 0; k < K; ++k) {
+        pair_tb[k] = tasks_of_pair(k, pair_tasks[k]);
+        total_tb += pair_tb[k];
+    }
+    if (opts == nullptr || opts->t_chunk_bytes <= 0) {
+        // default: about 16 chunks so that phase 1 of one chunk overlaps phase 2 of the previous one
+        // (dmrgk_heff_apply), between 512 MiB (launches stay long against their tails) and 4 GiB
+        o.t_chunk_bytes = std::min<int64_t>(int64_t(4) << 30, std::max<int64_t>(int64_t(512) << 20, total_tb / 16));
+    }
+
     int64_t k0 = 0;
     while (k0 < K) {
         Chunk ch;
@@ -167,80 +258,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             int64_t need = 0;
             for (const dmrgk_op* op : {(const dmrgk_op*)L[k], (const dmrgk_op*)R[k]})
                 if (op && op->pinned && op->n_padded && !staged.count(op)) need += round_up(op->n_padded * 8, 128);
-            // T bytes of this pair
-            int64_t tb = 0;
-            std::vector<Task> mine;
-            for (int ib = 0; ib < int(pb.size()); ++ib) {
-                const int a = pb[ib].r_idx, b = pb[ib].c_idx;
-                Task t;
-                memset(&t, 0, sizeof(t));
-                t.k = int32_t(k);
-                t.ib = ib;
-                t.m = pb[ib].rows;
-                t.n = pb[ib].cols;
-                int ao, bo;
-                // L applied to sector a
-                if (!L[k]) {
-                    ao = a;
-                    t.mo = t.m;
-                    t.s1.A = (unsigned long long)(uintptr_t)h->ident_dev;
-                    t.s1.lda = ident_ld;
-                    t.s1.flags = BASE_ABS << SEG_A_SEL_SHIFT;
-                } else {
-                    const int bi = (f & DMRGK_TRANS_L) ? L[k]->by_row[a] : L[k]->by_col[a];
-                    if (bi < 0) continue;
-                    const Block& lb = L[k]->blocks[bi];
-                    ao = (f & DMRGK_TRANS_L) ? lb.c_idx : lb.r_idx;
-                    t.mo = (f & DMRGK_TRANS_L) ? lb.cols : lb.rows;
-                    t.s1.lda = lb.ld;
-                    t.s1.flags = (f & DMRGK_TRANS_L) ? SEG_A_MMAJOR : 0u;
-                    if (L[k]->dev) {
-                        t.s1.A = (unsigned long long)(uintptr_t)(L[k]->dev + lb.off);
-                        t.s1.flags |= BASE_ABS << SEG_A_SEL_SHIFT;
-                    } else {
-                        t.s1.A = (unsigned long long)(lb.off * 8);   // ring offset added below
-                        t.s1.flags |= BASE_WS << SEG_A_SEL_SHIFT;
-                    }
-                }
-                if (!R[k]) {
-                    bo = b;
-                    t.no = t.n;
-                    t.s2.B = (unsigned long long)(uintptr_t)h->ident_dev;
-                    t.s2.ldb = ident_ld;
-                    t.s2.flags = BASE_ABS << SEG_B_SEL_SHIFT;
-                } else {
-                    const int bi = (f & DMRGK_TRANS_R) ? R[k]->by_row[b] : R[k]->by_col[b];
-                    if (bi < 0) continue;
-                    const Block& rb = R[k]->blocks[bi];
-                    bo = (f & DMRGK_TRANS_R) ? rb.c_idx : rb.r_idx;
-                    t.no = (f & DMRGK_TRANS_R) ? rb.cols : rb.rows;
-                    t.s2.ldb = rb.ld;
-                    t.s2.flags = (f & DMRGK_TRANS_R) ? SEG_B_NMAJOR : 0u;
-                    if (R[k]->dev) {
-                        t.s2.B = (unsigned long long)(uintptr_t)(R[k]->dev + rb.off);
-                        t.s2.flags |= BASE_ABS << SEG_B_SEL_SHIFT;
-                    } else {
-                        t.s2.B = (unsigned long long)(rb.off * 8);
-                        t.s2.flags |= BASE_WS << SEG_B_SEL_SHIFT;
-                    }
-                }
-                const int ob = layout->by_a[ao];
-                if (ob < 0 || pb[ob].c_idx != bo) continue;
-                t.ob = ob;
-                const int par = L[k] ? L[k]->parity : (R[k] ? R[k]->parity : 0);
-                t.alpha = coef[k] * ((par && SA->parity(a)) ? -1.0 : 1.0);
-                t.diag = (ob == ib);
-                // phase-1 B operand = ψ block (N-major), phase-2 A operand = T (K-major, set per chunk)
-                t.s1.B = (unsigned long long)(pb[ib].off * 8);
-                t.s1.ldb = pb[ib].ld;
-                t.s1.klen = t.m;
-                t.s1.flags |= SEG_B_NMAJOR | (BASE_PSI << SEG_B_SEL_SHIFT);
-                t.s2.lda = pb[ib].ld;
-                t.s2.klen = t.n;
-                t.s2.flags |= BASE_WS << SEG_A_SEL_SHIFT;
-                tb += int64_t(t.mo) * pb[ib].ld * 8;
-                mine.push_back(t);
-            }
+            const int64_t tb = pair_tb[k];
+            std::vector<Task>& mine = pair_tasks[k];
             const bool nonempty = !tasks.empty() || !staged.empty();
             if (nonempty && (t_bytes + tb > o.t_chunk_bytes || ring_used + need > ring_part)) break;
             // accept pair k into the chunk
