@@ -16,6 +16,7 @@ Tiers:
   T3  heff.py      the same sum block by block (one dense product per step);
                    also the timed CPU baseline
       davidson.py  the Davidson iteration, step by step
+      renorm.py    renormalisation O′ = Φ† O Φ of block operators
 
 Parity pins: every function here is pinned by ``tests/test_oracle_*.py``
 (anticommutators, brute-force bit-string action, free-fermion closed forms,

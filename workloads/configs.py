@@ -344,3 +344,44 @@ def config5():
 def config5_staged_ops(wl):
     """Every 7th stored operator streams from pinned host memory (≈ 14 % of the bytes)."""
     return [i for i in range(len(wl.ops)) if i % 7 == 3]
+
+
+# ----------------------------------------------------------------------------
+# renormalisation inputs (SURVEY §8(f) NEXT-1): the kept basis Φ of half A
+# ----------------------------------------------------------------------------
+PHI_STREAM = 13
+
+
+def renorm_basis(wl, M_new=None, half="A"):
+    """Sector list of the kept (new) basis of one half of ``wl`` and the block table of Φ.
+
+    The new basis keeps M_new states (default M/d with d = 2 spinless, 4 Hubbard: the bond
+    dimension D behind the enlarged dimension M = d·D, reading r9), distributed over the same
+    charges by the workload's own sector law (largest-remainder rounding, capped by the enlarged
+    dims).  Returns (sectors_new, phi_table) with phi_table = [(enl_idx, new_idx, rows, cols, off)],
+    off counting unpadded elements block after block in enlarged-sector order; sectors that keep no
+    state are dropped from the new space."""
+    sectors = wl.sectors(half)
+    M = sum(d for _, d in sectors)
+    d_loc = 2 if wl.n_charges == 1 else 4
+    M_new = M // d_loc if M_new is None else M_new
+    w = [float(d) for _, d in sectors]
+    dims = gaussian_sectors(M_new, w, [d for _, d in sectors]) if M_new < M else [d for _, d in sectors]
+    sectors_new, table, off = [], [], 0
+    for ei, ((q, de), dn) in enumerate(zip(sectors, dims)):
+        if dn <= 0 or de <= 0:
+            continue
+        table.append((ei, len(sectors_new), de, dn, off))
+        sectors_new.append((q, dn))
+        off += de * dn
+    return sectors_new, table
+
+
+def fill_phi_host(wl, phi_table, stream=PHI_STREAM):
+    """Φ blocks {(enl_idx, new_idx): ndarray}: normal12 / sqrt(rows) (synthetic: not orthonormal,
+    which the products do not need)."""
+    out = {}
+    for (ei, ni, rows, cols, off) in phi_table:
+        idx = off + np.arange(rows * cols, dtype=np.uint64).reshape(rows, cols)
+        out[(ei, ni)] = normal12(wl.seed, stream, idx) / math.sqrt(rows)
+    return out
