@@ -230,6 +230,47 @@ int32_t dmrgk_davidson_solve(dmrgk_davidson* d, double* theta, double* resnorm, 
 /* Current subspace size m. */
 int32_t dmrgk_davidson_query(const dmrgk_davidson* d, int32_t* m, int32_t* n_apply);
 
+/* ---- renormalisation step ("the renormalization step",
+ *      PAPER.md:142 Fig. 7 "Ren_l", "Ren_r"):  O′ = Φᵀ O Φ  for every operator kept -------------- */
+/* Φ: the kept basis of one half, a charge-block-diagonal map from the NEW space (kept states) into
+ * the ENLARGED space: one block (dim_enl(q) × dim_new(q)) for every enlarged sector (in enlarged
+ * order) whose charge is also a sector of the new space, both dims > 0.  Same packed layout rules as
+ * operators (ld = round_up(cols, 16), zero padding, offsets multiples of 16 doubles). */
+typedef struct dmrgk_iso dmrgk_iso;
+int32_t dmrgk_iso_create(dmrgk_ctx* ctx, const dmrgk_space* enlarged, const dmrgk_space* kept,
+                         dmrgk_iso** out);
+void dmrgk_iso_destroy(dmrgk_iso* phi);
+int32_t dmrgk_iso_query(const dmrgk_iso* phi, int64_t* n_blocks, int64_t* n_elems, int64_t* n_padded);
+/* enl_idx / new_idx: sector indices in the enlarged / kept space. */
+int32_t dmrgk_iso_blocks(const dmrgk_iso* phi, int32_t* enl_idx, int32_t* new_idx, int32_t* rows,
+                         int32_t* cols, int32_t* ld, int64_t* offset);
+int32_t dmrgk_iso_pack(const dmrgk_iso* phi, const double* unpadded_host, double* packed_host);
+int32_t dmrgk_iso_bind_device(dmrgk_iso* phi, const double* arena_dev);
+
+typedef struct dmrgk_renorm dmrgk_renorm;
+typedef struct dmrgk_renorm_opts {
+    int64_t t_chunk_bytes;  /* cap on the O·Φ intermediate per chunk of operators (0 = default 4 GiB) */
+    int32_t kernel;         /* 0 = DMMA kernel, 1 = scalar check kernel                               */
+    int32_t reserved[5];
+} dmrgk_renorm_opts;
+/* Plans out[i] = Φᵀ in[i] Φ for n_ops operators: in[i] lives on the enlarged space of Φ, out[i] on the
+ * kept space with the same charge shift and parity; per stored block
+ *     out[i][q+δ, q] = Φ[q+δ]ᵀ · in[i][q+δ, q] · Φ[q]
+ * as two grouped GEMMs (T = in·Φ, then Φᵀ·T) on the same FP64 tensor-core kernel as heff_apply.
+ * Blocks whose row or column sector keeps no state are skipped.  Every in[i], out[i] and Φ must be
+ * bound to DEVICE arenas; the arenas bound to out[i] are WRITTEN by dmrgk_renorm_apply (all blocks
+ * including their zero padding).  Errors: DMRGK_ESHAPE (wrong space), DMRGK_ECHARGE (shift or parity
+ * of in[i] and out[i] differ), DMRGK_ESTATE (unbound / pinned-only operand), DMRGK_EINVAL. */
+int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
+                            dmrgk_op* const* in, dmrgk_op* const* out,
+                            const dmrgk_renorm_opts* opts, dmrgk_renorm** plan);
+void dmrgk_renorm_destroy(dmrgk_renorm* plan);
+/* flops = Σ_blocks 2·e′·e·n + 2·n′·e′·n (e, e′: enlarged dims; n, n′: kept dims). */
+int32_t dmrgk_renorm_query(const dmrgk_renorm* plan, int64_t* n_tasks, double* flops,
+                           int64_t* workspace_bytes, int64_t* n_launches_per_apply);
+/* Enqueues the products on `stream` and returns (asynchronous). */
+int32_t dmrgk_renorm_apply(dmrgk_renorm* plan, void* workspace_dev, void* stream);
+
 /* ---- harness kernels (outside the hot path): seeded inputs and FP64 pipe probes ----------- */
 /* Counter-based values, bit-identical to workloads/rng.py normal12(seed, stream, index): fills the
  * packed arena of an operator / a ψ layout from the UNPADDED element index of each entry, times
@@ -239,6 +280,9 @@ int32_t dmrgk_op_fill_normal(const dmrgk_op* op, double* arena_dev, uint64_t see
                              int32_t scale_mode, int32_t symmetric, void* stream);
 int32_t dmrgk_layout_fill_normal(const dmrgk_layout* l, double* arena_dev, uint64_t seed,
                                  uint64_t stream_id, void* stream);
+/* Φ blocks: normal12 / sqrt(rows of the block) (workloads.fill_phi_host). */
+int32_t dmrgk_iso_fill_normal(const dmrgk_iso* phi, double* arena_dev, uint64_t seed, uint64_t stream_id,
+                              void* stream);
 /* Register-only FP64 pipe probes: every warp of a full grid issues `iters` rounds of 16 independent
  * mma.sync.m8n8k4.f64 (kind 0) or 32 independent fma.rn.f64 per lane (kind 1).  Returns the flops
  * issued in *flops; the caller times the stream with events. */

@@ -32,7 +32,7 @@ __host__ __device__ inline double normal12(unsigned long long base, unsigned lon
 __global__ void fill_normal_kernel(const DevBlock* __restrict__ table, double* __restrict__ arena,
                                    unsigned long long base, int scale_mode, int symmetric) {
     const DevBlock b = table[blockIdx.y];
-    const double scale = scale_mode ? 1.0 / sqrt((double)b.cols) : 1.0;
+    const double scale = scale_mode == 1 ? 1.0 / sqrt((double)b.cols) : scale_mode == 2 ? 1.0 / sqrt((double)b.rows) : 1.0;
     const long long total = (long long)b.rows * b.ld;
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
          e += (long long)gridDim.x * blockDim.x) {
@@ -122,6 +122,14 @@ int32_t dmrgk_layout_fill_normal(const dmrgk_layout* l, double* arena_dev, uint6
     if (!aligned128(arena_dev)) return fail(DMRGK_EALIGN, "layout_fill_normal: arena not 128-byte aligned");
     DMRGK_CUDA(cudaSetDevice(l->ctx->device));
     return fill(l->dev_table, l->blocks, arena_dev, seed, stream_id, 0, 0, (cudaStream_t)stream);
+}
+
+int32_t dmrgk_iso_fill_normal(const dmrgk_iso* phi, double* arena_dev, uint64_t seed, uint64_t stream_id,
+                              void* stream) {
+    if (!phi) return fail(DMRGK_EINVAL, "iso_fill_normal: phi is NULL");
+    if (!aligned128(arena_dev)) return fail(DMRGK_EALIGN, "iso_fill_normal: arena not 128-byte aligned");
+    DMRGK_CUDA(cudaSetDevice(phi->ctx->device));
+    return fill(phi->dev_table, phi->blocks, arena_dev, seed, stream_id, 2, 0, (cudaStream_t)stream);
 }
 
 int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* sink_dev, double* flops,

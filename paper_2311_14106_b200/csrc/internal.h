@@ -93,6 +93,16 @@ struct dmrgk_op {
     dmrgk::DevBlock* dev_table = nullptr;
 };
 
+struct dmrgk_iso {
+    dmrgk_ctx* ctx;
+    const dmrgk_space *enl, *kept;
+    std::vector<dmrgk::Block> blocks;     // r_idx = enlarged sector, c_idx = kept sector
+    std::vector<int32_t> by_enl;          // enlarged sector → block index or −1
+    int64_t n_elems = 0, n_padded = 0;
+    const double* dev = nullptr;
+    dmrgk::DevBlock* dev_table = nullptr;
+};
+
 namespace dmrgk {
 
 // ---- a2: device-side work descriptions ---------------------------------------------------------
@@ -184,6 +194,19 @@ struct Chunk {
 };
 
 }  // namespace dmrgk
+
+struct dmrgk_renorm {
+    dmrgk_ctx* ctx;
+    int kernel = 0;
+    int64_t n_tasks = 0, t_bytes = 0, workspace_bytes = 0, n_launches = 0;
+    double flops = 0;
+    struct RChunk {
+        int64_t p1_unit0 = 0, p1_units = 0, p2_unit0 = 0, p2_units = 0;
+    };
+    std::vector<RChunk> chunks;
+    dmrgk::Unit* units_dev = nullptr;
+    dmrgk::Seg* segs_dev = nullptr;
+};
 
 struct dmrgk_heff {
     dmrgk_ctx* ctx;

@@ -1,0 +1,236 @@
+// renorm.cu — renormalisation step O′ = Φᵀ O Φ of block operators (
+// PAPER.md:60 §II.A "the renormalization step", Fig. 7 "Ren_l", "Ren_r").
+//
+// Per stored block of operator i:   out_i[q+δ, q] = Φ[q+δ]ᵀ · in_i[q+δ, q] · Φ[q]
+//   phase 1:  T = in_i[q+δ, q] · Φ[q]          A = operator block (K-major), B = Φ[q] (N-major)
+//   phase 2:  out = Φ[q+δ]ᵀ · T                A = Φ[q+δ] (M-major),        B = T (N-major)
+// Both phases are work lists for the grouped FP64 tensor-core kernel of heff_kernels.cu (one segment
+// per unit, output written directly — every output tile has exactly one producer, so nothing is
+// accumulated).  Operators are processed in chunks so that T fits its workspace.
+#include "internal.h"
+#include <algorithm>
+#include <cstring>
+#include <new>
+
+using namespace dmrgk;
+
+namespace {
+
+struct RTask {
+    const Block *ob, *pc, *pr;   // operator block, Φ[q] (column sector), Φ[q+δ] (row sector)
+    const double *in, *out;      // device arenas of in_i / out_i
+    const Block* outb;           // output block of out_i
+};
+
+int64_t tile_cost(int rows, int cols, int64_t nkt) { return int64_t((rows + 7) / 8) * ((cols + 7) / 8) * nkt; }
+
+template <class T>
+int32_t upload(const std::vector<T>& v, T** out) {
+    *out = nullptr;
+    if (v.empty()) return DMRGK_OK;
+    DMRGK_CUDA(cudaMalloc(out, v.size() * sizeof(T)));
+    DMRGK_CUDA(cudaMemcpy(*out, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return DMRGK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+void dmrgk_renorm_destroy(dmrgk_renorm* r) {
+    if (!r) return;
+    cudaFree(r->units_dev);
+    cudaFree(r->segs_dev);
+    delete r;
+}
+
+int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops, dmrgk_op* const* in,
+                            dmrgk_op* const* out, const dmrgk_renorm_opts* opts, dmrgk_renorm** plan) {
+    if (!plan) return fail(DMRGK_EINVAL, "renorm_create: plan is NULL");
+    *plan = nullptr;
+    if (!ctx || !phi) return fail(DMRGK_EINVAL, "renorm_create: NULL ctx or phi");
+    if (n_ops < 0 || (n_ops > 0 && (!in || !out))) return fail(DMRGK_EINVAL, "renorm_create: bad operator arrays");
+    if (phi->n_padded && !phi->dev) return fail(DMRGK_ESTATE, "renorm_create: phi is not bound to a device arena");
+    dmrgk_renorm_opts o;
+    memset(&o, 0, sizeof(o));
+    if (opts) o = *opts;
+    if (o.t_chunk_bytes <= 0) o.t_chunk_bytes = int64_t(4) << 30;
+    if (o.kernel != 0 && o.kernel != 1) return fail(DMRGK_EINVAL, "renorm_create: bad options");
+    for (int64_t i = 0; i < n_ops; ++i) {
+        if (!in[i] || !out[i]) return fail(DMRGK_EINVAL, "renorm_create: operator %lld is NULL", (long long)i);
+        if (in[i]->space != phi->enl) return fail(DMRGK_ESHAPE, "renorm_create: in[%lld] is not on phi's enlarged space", (long long)i);
+        if (out[i]->space != phi->kept) return fail(DMRGK_ESHAPE, "renorm_create: out[%lld] is not on phi's kept space", (long long)i);
+        if (in[i]->dq[0] != out[i]->dq[0] || in[i]->dq[1] != out[i]->dq[1] || in[i]->parity != out[i]->parity)
+            return fail(DMRGK_ECHARGE, "renorm_create: in[%lld] and out[%lld] differ in charge shift or parity", (long long)i, (long long)i);
+        if ((in[i]->n_padded && !in[i]->dev) || (out[i]->n_padded && !out[i]->dev))
+            return fail(DMRGK_ESTATE, "renorm_create: operator %lld is not bound to a device arena", (long long)i);
+    }
+    DMRGK_CUDA(cudaSetDevice(ctx->device));
+    dmrgk_renorm* r = new (std::nothrow) dmrgk_renorm;
+    if (!r) return fail(DMRGK_ENOMEM, "renorm_create: out of host memory");
+    r->ctx = ctx;
+    r->kernel = o.kernel;
+
+    std::vector<Unit> units;
+    std::vector<Seg> segs;
+    int64_t max_t = 0;
+    int64_t i0 = 0;
+    while (i0 < n_ops) {
+        // ---- one chunk: operators [i0, i1) whose T intermediates fit o.t_chunk_bytes ----
+        std::vector<RTask> tasks;
+        int64_t t_bytes = 0, i1 = i0;
+        for (; i1 < n_ops; ++i1) {
+            std::vector<RTask> mine;
+            int64_t tb = 0;
+            for (const Block& ob : in[i1]->blocks) {
+                const int pc = phi->by_enl[ob.c_idx], pr = phi->by_enl[ob.r_idx];
+                if (pc < 0 || pr < 0) continue;
+                const Block& bc = phi->blocks[pc];
+                const Block& br = phi->blocks[pr];
+                const int oi = out[i1]->by_col[bc.c_idx];
+                if (oi < 0 || out[i1]->blocks[oi].r_idx != br.c_idx) {
+                    dmrgk_renorm_destroy(r);
+                    return fail(DMRGK_ESHAPE, "renorm_create: out[%lld] has no block for kept sectors (%d, %d)", (long long)i1, br.c_idx, bc.c_idx);
+                }
+                mine.push_back({&ob, &bc, &br, in[i1]->dev, out[i1]->dev, &out[i1]->blocks[oi]});
+                tb += int64_t(ob.rows) * bc.ld * 8;
+            }
+            if (!tasks.empty() && t_bytes + tb > o.t_chunk_bytes) break;
+            tasks.insert(tasks.end(), mine.begin(), mine.end());
+            t_bytes += tb;
+        }
+        i0 = i1;
+        max_t = std::max(max_t, t_bytes);
+        dmrgk_renorm::RChunk ch;
+        struct CU {
+            int64_t cost;
+            Unit u;
+        };
+        std::vector<CU> p1, p2;
+        int64_t t_off = 0;
+        for (const RTask& t : tasks) {
+            const int e_r = t.ob->rows, e_c = t.ob->cols, n_c = t.pc->cols, n_r = t.pr->cols;
+            const int ldt = t.pc->ld;
+            r->flops += 2.0 * e_r * e_c * n_c + 2.0 * n_r * e_r * n_c;
+            ++r->n_tasks;
+            // phase 1: T (e_r × n_c, ld ldt) = O (K-major) · Φ[q] (N-major)
+            Seg s1;
+            memset(&s1, 0, sizeof(s1));
+            s1.A = (unsigned long long)(uintptr_t)(t.in + t.ob->off);
+            s1.lda = t.ob->ld;
+            s1.B = (unsigned long long)(uintptr_t)(phi->dev + t.pc->off);
+            s1.ldb = t.pc->ld;
+            s1.klen = e_c;
+            s1.flags = SEG_B_NMAJOR | (BASE_ABS << SEG_A_SEL_SHIFT) | (BASE_ABS << SEG_B_SEL_SHIFT);
+            const int32_t si1 = int32_t(segs.size());
+            segs.push_back(s1);
+            const int64_t nkt1 = (e_c + TILE_K - 1) / TILE_K;
+            for (int r0 = 0; r0 < e_r; r0 += TILE_M)
+                for (int c0 = 0; c0 < ldt; c0 += TILE_N) {
+                    Unit u;
+                    memset(&u, 0, sizeof(u));
+                    u.C = (unsigned long long)(t_off + (int64_t(r0) * ldt + c0) * 8);
+                    u.alpha = 1.0;
+                    u.ldc = ldt;
+                    u.i0 = r0;
+                    u.j0 = c0;
+                    u.mrows = e_r;
+                    u.ncols = n_c;
+                    u.ncols_st = ldt;
+                    u.seg_begin = si1;
+                    u.seg_end = si1 + 1;
+                    u.mode = BASE_WS << UNIT_C_SEL_SHIFT;
+                    u.nkt = int32_t(nkt1);
+                    p1.push_back({tile_cost(std::min(TILE_M, e_r - r0), std::min(TILE_N, ldt - c0), nkt1), u});
+                }
+            // phase 2: out (n_r × n_c) = Φ[q+δ]ᵀ (M-major) · T (N-major)
+            Seg s2;
+            memset(&s2, 0, sizeof(s2));
+            s2.A = (unsigned long long)(uintptr_t)(phi->dev + t.pr->off);
+            s2.lda = t.pr->ld;
+            s2.B = (unsigned long long)t_off;
+            s2.ldb = ldt;
+            s2.klen = e_r;
+            s2.flags = SEG_A_MMAJOR | SEG_B_NMAJOR | (BASE_ABS << SEG_A_SEL_SHIFT) | (BASE_WS << SEG_B_SEL_SHIFT);
+            const int32_t si2 = int32_t(segs.size());
+            segs.push_back(s2);
+            const int64_t nkt2 = (e_r + TILE_K - 1) / TILE_K;
+            const int ldo = t.outb->ld;
+            for (int r0 = 0; r0 < n_r; r0 += TILE_M)
+                for (int c0 = 0; c0 < ldo; c0 += TILE_N) {
+                    Unit u;
+                    memset(&u, 0, sizeof(u));
+                    u.C = (unsigned long long)(uintptr_t)(t.out + t.outb->off + int64_t(r0) * ldo + c0);
+                    u.alpha = 1.0;
+                    u.ldc = ldo;
+                    u.i0 = r0;
+                    u.j0 = c0;
+                    u.mrows = n_r;
+                    u.ncols = n_c;
+                    u.ncols_st = ldo;
+                    u.seg_begin = si2;
+                    u.seg_end = si2 + 1;
+                    u.mode = BASE_ABS << UNIT_C_SEL_SHIFT;
+                    u.nkt = int32_t(nkt2);
+                    p2.push_back({tile_cost(std::min(TILE_M, n_r - r0), std::min(TILE_N, ldo - c0), nkt2), u});
+                }
+            t_off += int64_t(e_r) * ldt * 8;
+        }
+        auto by_cost = [](const CU& a, const CU& b) { return a.cost > b.cost; };
+        std::stable_sort(p1.begin(), p1.end(), by_cost);
+        std::stable_sort(p2.begin(), p2.end(), by_cost);
+        ch.p1_unit0 = int64_t(units.size());
+        for (const CU& x : p1) units.push_back(x.u);
+        ch.p1_units = int64_t(p1.size());
+        ch.p2_unit0 = int64_t(units.size());
+        for (const CU& x : p2) units.push_back(x.u);
+        ch.p2_units = int64_t(p2.size());
+        r->chunks.push_back(ch);
+    }
+    if (int64_t(segs.size()) > 0x7fffffffLL) {
+        dmrgk_renorm_destroy(r);
+        return fail(DMRGK_EINVAL, "renorm_create: too many segments");
+    }
+    r->t_bytes = round_up(max_t, 128);
+    r->workspace_bytes = std::max<int64_t>(128, r->t_bytes);
+    for (const auto& c : r->chunks) r->n_launches += (c.p1_units > 0) + (c.p2_units > 0);
+    int32_t s = upload(units, &r->units_dev);
+    if (s == DMRGK_OK) s = upload(segs, &r->segs_dev);
+    if (s != DMRGK_OK) {
+        dmrgk_renorm_destroy(r);
+        return s;
+    }
+    *plan = r;
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_renorm_query(const dmrgk_renorm* r, int64_t* n_tasks, double* flops, int64_t* workspace_bytes,
+                           int64_t* n_launches_per_apply) {
+    if (!r) return fail(DMRGK_EINVAL, "renorm_query: plan is NULL");
+    if (n_tasks) *n_tasks = r->n_tasks;
+    if (flops) *flops = r->flops;
+    if (workspace_bytes) *workspace_bytes = r->workspace_bytes;
+    if (n_launches_per_apply) *n_launches_per_apply = r->n_launches;
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_renorm_apply(dmrgk_renorm* r, void* workspace_dev, void* stream) {
+    if (!r) return fail(DMRGK_EINVAL, "renorm_apply: plan is NULL");
+    if (r->n_tasks == 0) return DMRGK_OK;
+    if (!workspace_dev) return fail(DMRGK_EINVAL, "renorm_apply: NULL workspace");
+    if (!aligned128(workspace_dev)) return fail(DMRGK_EALIGN, "renorm_apply: workspace must be 128-byte aligned");
+    DMRGK_CUDA(cudaSetDevice(r->ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    Bases bases;
+    bases.b[BASE_ABS] = 0;
+    bases.b[BASE_WS] = (unsigned long long)(uintptr_t)workspace_dev;
+    bases.b[BASE_PSI] = 0;
+    bases.b[BASE_SIGMA] = 0;
+    for (const auto& c : r->chunks) {
+        DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + c.p1_unit0, r->segs_dev, c.p1_units, bases, st));
+        DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + c.p2_unit0, r->segs_dev, c.p2_units, bases, st));
+    }
+    return DMRGK_OK;
+}
+
+}  // extern "C"

@@ -311,4 +311,85 @@ int32_t dmrgk_op_bind_pinned(dmrgk_op* op, const double* arena_pinned_host) {
     return DMRGK_OK;
 }
 
+// ---- Φ: kept basis of one half (renormalisation) ----------------------------
+int32_t dmrgk_iso_create(dmrgk_ctx* ctx, const dmrgk_space* enlarged, const dmrgk_space* kept, dmrgk_iso** out) {
+    if (!out) return fail(DMRGK_EINVAL, "iso_create: out is NULL");
+    *out = nullptr;
+    if (!ctx || !enlarged || !kept) return fail(DMRGK_EINVAL, "iso_create: NULL argument");
+    if (enlarged->n_charges != kept->n_charges)
+        return fail(DMRGK_ESHAPE, "iso_create: the two spaces have different numbers of charges");
+    dmrgk_iso* p = new (std::nothrow) dmrgk_iso;
+    if (!p) return fail(DMRGK_ENOMEM, "iso_create: out of host memory");
+    p->ctx = ctx;
+    p->enl = enlarged;
+    p->kept = kept;
+    p->by_enl.assign(enlarged->n(), -1);
+    int64_t off = 0, uoff = 0;
+    for (int e = 0; e < enlarged->n(); ++e) {
+        const int k = kept->find(enlarged->q[2 * e], enlarged->q[2 * e + 1]);
+        if (k < 0 || enlarged->dim[e] == 0 || kept->dim[k] == 0) continue;
+        if (kept->dim[k] > enlarged->dim[e]) {
+            delete p;
+            return fail(DMRGK_ESHAPE, "iso_create: kept sector %d holds %d states, its enlarged sector only %d", k,
+                        kept->dim[k], enlarged->dim[e]);
+        }
+        Block b;
+        b.r_idx = e;
+        b.c_idx = k;
+        b.rows = enlarged->dim[e];
+        b.cols = kept->dim[k];
+        b.ld = int32_t(round_up(b.cols, LD_PAD));
+        b.off = off;
+        b.uoff = uoff;
+        off += int64_t(b.rows) * b.ld;
+        uoff += int64_t(b.rows) * b.cols;
+        p->by_enl[e] = int32_t(p->blocks.size());
+        p->blocks.push_back(b);
+    }
+    p->n_elems = uoff;
+    p->n_padded = off;
+    int32_t s = upload_table(p->blocks, &p->dev_table);
+    if (s != DMRGK_OK) {
+        delete p;
+        return s;
+    }
+    *out = p;
+    return DMRGK_OK;
+}
+
+void dmrgk_iso_destroy(dmrgk_iso* phi) {
+    if (!phi) return;
+    if (phi->dev_table) cudaFree(phi->dev_table);
+    delete phi;
+}
+
+int32_t dmrgk_iso_query(const dmrgk_iso* phi, int64_t* n_blocks, int64_t* n_elems, int64_t* n_padded) {
+    if (!phi) return fail(DMRGK_EINVAL, "iso_query: phi is NULL");
+    if (n_blocks) *n_blocks = int64_t(phi->blocks.size());
+    if (n_elems) *n_elems = phi->n_elems;
+    if (n_padded) *n_padded = phi->n_padded;
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_iso_blocks(const dmrgk_iso* phi, int32_t* enl_idx, int32_t* new_idx, int32_t* rows, int32_t* cols,
+                         int32_t* ld, int64_t* offset) {
+    if (!phi) return fail(DMRGK_EINVAL, "iso_blocks: phi is NULL");
+    copy_table(phi->blocks, enl_idx, new_idx, rows, cols, ld, offset);
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_iso_pack(const dmrgk_iso* phi, const double* u, double* p) {
+    if (!phi || (phi->n_padded && (!u || !p))) return fail(DMRGK_EINVAL, "iso_pack: NULL argument");
+    pack_blocks(phi->blocks, phi->n_padded, u, p);
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_iso_bind_device(dmrgk_iso* phi, const double* arena_dev) {
+    if (!phi) return fail(DMRGK_EINVAL, "iso_bind_device: phi is NULL");
+    if (phi->n_padded && !arena_dev) return fail(DMRGK_EINVAL, "iso_bind_device: arena is NULL");
+    if (!aligned128(arena_dev)) return fail(DMRGK_EALIGN, "iso_bind_device: arena %p not 128-byte aligned", (const void*)arena_dev);
+    phi->dev = arena_dev;
+    return DMRGK_OK;
+}
+
 }  // extern "C"

@@ -27,6 +27,10 @@ class DmrgkError(RuntimeError):
         self.message = message
 
 
+class RenormOpts(C.Structure):
+    _fields_ = [("t_chunk_bytes", C.c_int64), ("kernel", C.c_int32), ("reserved", C.c_int32 * 5)]
+
+
 class HeffOpts(C.Structure):
     _fields_ = [("t_chunk_bytes", C.c_int64), ("ring_bytes", C.c_int64), ("kernel", C.c_int32),
                 ("split_waves", C.c_int32), ("reserved", C.c_int32 * 4)]
@@ -67,6 +71,17 @@ SIGNATURES = {
     "dmrgk_heff_diag": (_i32, [_p, _p, _p, _p, _p]),
     "dmrgk_heff_profile": (_i32, [_p, _i32]),
     "dmrgk_heff_profile_read": (_i32, [_p, _p, _p]),
+    "dmrgk_iso_create": (_i32, [_p, _p, _p, _pp]),
+    "dmrgk_iso_destroy": (None, [_p]),
+    "dmrgk_iso_query": (_i32, [_p, _pi64, _pi64, _pi64]),
+    "dmrgk_iso_blocks": (_i32, [_p, _p, _p, _p, _p, _p, _p]),
+    "dmrgk_iso_pack": (_i32, [_p, _p, _p]),
+    "dmrgk_iso_bind_device": (_i32, [_p, _p]),
+    "dmrgk_iso_fill_normal": (_i32, [_p, _p, _u64, _u64, _p]),
+    "dmrgk_renorm_create": (_i32, [_p, _p, _i64, _p, _p, _p, _pp]),
+    "dmrgk_renorm_destroy": (None, [_p]),
+    "dmrgk_renorm_query": (_i32, [_p, _pi64, _pf64, _pi64, _pi64]),
+    "dmrgk_renorm_apply": (_i32, [_p, _p, _p]),
     "dmrgk_vec_scratch_bytes": (_i64, [_i32]),
     "dmrgk_vec_multi_dot": (_i32, [_p, _i64, _i32, _p, _i64, _p, _p, _p, _p]),
     "dmrgk_vec_multi_axpy": (_i32, [_p, _i64, _i32, _p, _i64, _p, _f64, _f64, _p, _p]),
@@ -262,6 +277,67 @@ class Op(_Blocked):
     def __del__(self):
         if getattr(self, "h", None):
             self.lib.dmrgk_op_destroy(self.h)
+            self.h = None
+
+
+class Iso(_Blocked):
+    """dmrgk_iso: the kept basis Φ (kept space → enlarged space)."""
+    _query, _blocks = "dmrgk_iso_query", "dmrgk_iso_blocks"
+
+    def __init__(self, ctx, enlarged, kept):
+        self.ctx, self.lib, self.enlarged, self.kept = ctx, ctx.lib, enlarged, kept
+        h = C.c_void_p()
+        check(self.lib.dmrgk_iso_create(ctx.h, enlarged.h, kept.h, C.byref(h)))
+        self.h = h
+        self.n_blocks, self.n_elems, self.n_padded = self.query()
+        self._keep = None
+
+    def pack(self, unpadded):
+        u = np.ascontiguousarray(unpadded, dtype=np.float64)
+        assert u.size == self.n_elems
+        p = np.zeros(self.n_padded, np.float64)
+        check(self.lib.dmrgk_iso_pack(self.h, u.ctypes.data, p.ctypes.data))
+        return p
+
+    def bind_device(self, arena):
+        check(self.lib.dmrgk_iso_bind_device(self.h, _dev(arena)))
+        self._keep = arena
+
+    def fill_normal(self, arena, seed, stream_id, stream=None):
+        check(self.lib.dmrgk_iso_fill_normal(self.h, _dev(arena), seed, stream_id, _stream(stream)))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.dmrgk_iso_destroy(self.h)
+            self.h = None
+
+
+class Renorm:
+    """dmrgk_renorm: out[i] = Φᵀ in[i] Φ for lists of bound operators."""
+
+    def __init__(self, ctx, phi, ops_in, ops_out, t_chunk_bytes=0, kernel=0):
+        self.ctx, self.lib = ctx, ctx.lib
+        n = len(ops_in)
+        assert len(ops_out) == n
+        a_in = (C.c_void_p * max(n, 1))()
+        a_out = (C.c_void_p * max(n, 1))()
+        for i in range(n):
+            a_in[i], a_out[i] = ops_in[i].h, ops_out[i].h
+        opts = RenormOpts(int(t_chunk_bytes), int(kernel))
+        h = C.c_void_p()
+        check(self.lib.dmrgk_renorm_create(ctx.h, phi.h, n, a_in, a_out, C.byref(opts), C.byref(h)))
+        self.h = h
+        self._keep = (phi, list(ops_in), list(ops_out))
+        nt, wb, nl, fl = C.c_int64(), C.c_int64(), C.c_int64(), C.c_double()
+        check(self.lib.dmrgk_renorm_query(self.h, C.byref(nt), C.byref(fl), C.byref(wb), C.byref(nl)))
+        self.n_tasks, self.flops, self.workspace_bytes, self.n_launches = nt.value, fl.value, wb.value, nl.value
+
+    def apply(self, workspace, stream=None):
+        check(self.lib.dmrgk_renorm_apply(self.h, _dev(workspace), _stream(stream)))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.dmrgk_renorm_destroy(self.h)
             self.h = None
 
 

@@ -201,3 +201,59 @@ def from_host(n_charges, sectors_A, sectors_B, target, ops, terms, device=0, ctx
         dp.set_op_host(i, o["blocks"])
     dp.build(terms, **opts)
     return dp
+
+
+class RenormProblem:
+    """Device set-up of one renormalisation step (marshalling and memory only): the operators of one
+    half of a DeviceProblem as inputs, Φ, and freshly allocated output operators on the kept space."""
+
+    def __init__(self, dp, half, sectors_new, op_indices=None, **opts):
+        self.dp, self.ctx, self.device = dp, dp.ctx, dp.device
+        self.enl = dp.A if half == "A" else dp.B
+        self.kept = dmrgk.Space(self.ctx, self.enl.n_charges, sectors_new)
+        self.phi = dmrgk.Iso(self.ctx, self.enl, self.kept)
+        self.phi_arena = torch.zeros(max(self.phi.n_padded, 16), dtype=torch.float64, device=self.device)
+        self.phi.bind_device(self.phi_arena)
+        self.idx = [i for i, op in enumerate(dp.ops) if op.space is self.enl] if op_indices is None else list(op_indices)
+        self.ops_in = [dp.ops[i] for i in self.idx]
+        self.opts = opts
+        self.ops_out, self.out_views, self.plan, self.workspace = [], [], None, None
+
+    def set_phi_host(self, blocks):
+        self.phi_arena[:self.phi.n_padded].copy_(torch.from_numpy(self.phi.pack(_unpadded_from_blocks(self.phi.blocks(), blocks))))
+
+    def fill_phi(self, seed, stream_id):
+        if self.phi.n_padded:
+            self.phi.fill_normal(self.phi_arena, seed, stream_id, self.dp.stream)
+
+    def build(self, specs):
+        """specs: [(dq, parity)] of the operators in self.idx order."""
+        self.ops_out = [dmrgk.Op(self.ctx, self.kept, dq, parity) for (dq, parity) in specs]
+        total = int(sum(op.n_padded for op in self.ops_out))
+        self.out_arena = torch.full((max(total, 16),), float("nan"), dtype=torch.float64, device=self.device)
+        o = 0
+        for op in self.ops_out:
+            view = self.out_arena[o:o + op.n_padded] if op.n_padded else self.out_arena[0:16]
+            op.bind_device(view)
+            self.out_views.append(view)
+            o += op.n_padded
+        self.plan = dmrgk.Renorm(self.ctx, self.phi, self.ops_in, self.ops_out, **self.opts)
+        self.workspace = torch.empty(max(self.plan.workspace_bytes, 128), dtype=torch.uint8, device=self.device)
+        return self.plan
+
+    def apply(self):
+        self.plan.apply(self.workspace, self.dp.stream)
+
+    def read_out_blocks(self, j):
+        """D2H of output operator j as {(row_idx, col_idx): ndarray} plus a flag that its padding is zero."""
+        op = self.ops_out[j]
+        if not op.n_padded:
+            return {}, True
+        r, c, rows, cols, ld, off = op.blocks()
+        host = self.out_views[j].cpu().numpy()
+        out, pad_ok = {}, True
+        for b in range(len(r)):
+            blk = host[off[b]:off[b] + int(rows[b]) * int(ld[b])].reshape(int(rows[b]), int(ld[b]))
+            out[(int(r[b]), int(c[b]))] = blk[:, :cols[b]].copy()
+            pad_ok = pad_ok and not np.any(blk[:, cols[b]:] != 0.0)
+        return out, pad_ok

@@ -383,5 +383,5 @@ def fill_phi_host(wl, phi_table, stream=PHI_STREAM):
     out = {}
     for (ei, ni, rows, cols, off) in phi_table:
         idx = off + np.arange(rows * cols, dtype=np.uint64).reshape(rows, cols)
-        out[(ei, ni)] = normal12(wl.seed, stream, idx) / math.sqrt(rows)
+        out[(ei, ni)] = normal12(wl.seed, stream, idx) * (1.0 / math.sqrt(rows))
     return out
