@@ -363,6 +363,67 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_renorm(args):
+    """--op renorm: one step = the renormalisation O' = Phi^T O Phi of every enlarged-block operator of
+    the left half of the workload to D kept states; not the headline metric."""
+    import torch
+    import workloads as wlmod
+    from paper_2311_14106_b200 import dmrgk, problem
+    from oracle import renorm as orenorm
+    torch.cuda.set_device(0)
+    wl = make_workload(args.config)
+    dp = problem.from_workload(wl)
+    sectors_new, table = wlmod.renorm_basis(wl)
+    rp = problem.RenormProblem(dp, "A", sectors_new)
+    rp.fill_phi(wl.seed, wlmod.PHI_STREAM)
+    rp.build([(wl.ops[i].dq, wl.ops[i].parity) for i in rp.idx])
+    for _ in range(args.warmup):
+        rp.apply()
+    torch.cuda.synchronize()
+    clocks = ClockSampler(0)
+    clocks.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dmrgk.launch_count(reset=True)
+    e0.record(dp.stream)
+    for _ in range(args.steps):
+        rp.apply()
+    e1.record(dp.stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    launches = dmrgk.launch_count()
+    clk = clocks.stop()
+    n_sm = dp.ctx.query()[0]
+    peak = n_sm * 128 * (clk.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+    val = rp.plan.flops / ms / 1e9
+    out = {"metric": "renorm_fp64_tflops", "value": val, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": wl.name + "_renorm_left_half", "operators": len(rp.idx), "blocks": rp.plan.n_tasks,
+                      "M_enlarged": wl.M_A, "M_kept": sum(d for _, d in sectors_new), "flops_per_apply": rp.plan.flops,
+                      "in_bytes": int(sum(op.n_padded for op in rp.ops_in) * 8),
+                      "out_bytes": int(sum(op.n_padded for op in rp.ops_out) * 8),
+                      "l2": "operator arenas (>> 126 MB L2) are streamed once per step"},
+           "gpu_launches": int(launches),
+           "roofline": {"bound": "tensor", "kernel": "heff_gemm_dmma_kernel (renormalisation work lists)", "achieved": val,
+                        "peak": peak, "unit": "TFLOP/s", "frac": val / peak, "traffic": None,
+                        "launches": int(rp.plan.n_launches * args.steps)},
+           "clocks": clk}
+    if not args.no_cpu:
+        phi = wlmod.fill_phi_host(wl, table)
+        ids = rp.idx[::max(1, len(rp.idx) // 12)]
+        ops = [{"half": "A", "dq": tuple(wl.ops[i].dq), "parity": wl.ops[i].parity, "blocks": wlmod.fill_op_host(wl, i)} for i in ids]
+        fl = float(sum(orenorm.flops(o, phi) for o in ops))
+        reps, t0 = 0, time.perf_counter()
+        while reps < 2 or (time.perf_counter() - t0 < 10.0 and reps < 100):
+            for o in ops:
+                orenorm.renormalise_blockwise(o, wl.sectors_A, phi, sectors_new)
+            reps += 1
+        sec = (time.perf_counter() - t0) / reps
+        out["cpu_baseline"] = {"value": fl / sec / 1e12, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+                               "sample": f"oracle.renorm.renormalise_blockwise on {len(ids)} of {len(rp.idx)} operators, {fl:.3e} flop x {reps} repeats"}
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -372,9 +433,13 @@ def main():
     ap.add_argument("--config", default="4", choices=["2", "3", "3b", "4", "5", "5r"])
     ap.add_argument("--m-max", dest="m_max", type=int, default=16)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm"],
+                    help="davidson (default, the headline hot path) or renorm (NEXT-1 row, its own metric)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.op == "renorm":
+        run_renorm(args)
     else:
         run_ours(args)
 
