@@ -249,7 +249,8 @@ int32_t dmrgk_iso_bind_device(dmrgk_iso* phi, const double* arena_dev);
 
 typedef struct dmrgk_renorm dmrgk_renorm;
 typedef struct dmrgk_renorm_opts {
-    int64_t t_chunk_bytes;  /* cap on the O·Φ intermediate per chunk of operators (0 = default 4 GiB) */
+    int64_t t_chunk_bytes;  /* cap on the O·Φ intermediate per chunk of operators (0 = default: total/16
+                               in [256 MiB, 4 GiB]); the workspace holds two such buffers                */
     int32_t kernel;         /* 0 = DMMA kernel, 1 = scalar check kernel                               */
     int32_t reserved[5];
 } dmrgk_renorm_opts;
@@ -268,7 +269,8 @@ void dmrgk_renorm_destroy(dmrgk_renorm* plan);
 /* flops = Σ_blocks 2·e′·e·n + 2·n′·e′·n (e, e′: enlarged dims; n, n′: kept dims). */
 int32_t dmrgk_renorm_query(const dmrgk_renorm* plan, int64_t* n_tasks, double* flops,
                            int64_t* workspace_bytes, int64_t* n_launches_per_apply);
-/* Enqueues the products on `stream` and returns (asynchronous). */
+/* Enqueues the products and returns (asynchronous); all work is ordered after what `stream` holds at
+ * the call and joined back into `stream` (two library-owned streams overlap the two phases). */
 int32_t dmrgk_renorm_apply(dmrgk_renorm* plan, void* workspace_dev, void* stream);
 
 /* ---- harness kernels (outside the hot path): seeded inputs and FP64 pipe probes ----------- */

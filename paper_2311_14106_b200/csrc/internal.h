@@ -206,6 +206,10 @@ struct dmrgk_renorm {
     std::vector<RChunk> chunks;
     dmrgk::Unit* units_dev = nullptr;
     dmrgk::Seg* segs_dev = nullptr;
+    // same choreography as dmrgk_heff_apply: phase 1 of chunk c+1 (lowest-priority stream) overlaps
+    // phase 2 of chunk c (greatest-priority stream); T is double-buffered
+    cudaStream_t s1 = nullptr, s2 = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_p1[2] = {nullptr, nullptr}, ev_p2[2] = {nullptr, nullptr};
 };
 
 struct dmrgk_heff {

@@ -41,6 +41,14 @@ void dmrgk_renorm_destroy(dmrgk_renorm* r) {
     if (!r) return;
     cudaFree(r->units_dev);
     cudaFree(r->segs_dev);
+    for (int i = 0; i < 2; ++i) {
+        if (r->ev_p1[i]) cudaEventDestroy(r->ev_p1[i]);
+        if (r->ev_p2[i]) cudaEventDestroy(r->ev_p2[i]);
+    }
+    if (r->ev_fork) cudaEventDestroy(r->ev_fork);
+    if (r->ev_join) cudaEventDestroy(r->ev_join);
+    if (r->s1) cudaStreamDestroy(r->s1);
+    if (r->s2) cudaStreamDestroy(r->s2);
     delete r;
 }
 
@@ -54,7 +62,7 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
     dmrgk_renorm_opts o;
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
-    if (o.t_chunk_bytes <= 0) o.t_chunk_bytes = int64_t(4) << 30;
+    const bool default_chunk = o.t_chunk_bytes <= 0;
     if (o.kernel != 0 && o.kernel != 1) return fail(DMRGK_EINVAL, "renorm_create: bad options");
     for (int64_t i = 0; i < n_ops; ++i) {
         if (!in[i] || !out[i]) return fail(DMRGK_EINVAL, "renorm_create: operator %lld is NULL", (long long)i);
@@ -71,8 +79,18 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
     r->ctx = ctx;
     r->kernel = o.kernel;
 
+    if (default_chunk) {   // about 16 chunks, between 256 MiB and 4 GiB (see dmrgk_heff_create)
+        int64_t total = 0;
+        for (int64_t i = 0; i < n_ops; ++i)
+            for (const Block& ob : in[i]->blocks) {
+                const int pc = phi->by_enl[ob.c_idx], pr = phi->by_enl[ob.r_idx];
+                if (pc >= 0 && pr >= 0) total += int64_t(ob.rows) * phi->blocks[pc].ld * 8;
+            }
+        o.t_chunk_bytes = std::min<int64_t>(int64_t(4) << 30, std::max<int64_t>(int64_t(256) << 20, total / 16));
+    }
     std::vector<Unit> units;
     std::vector<Seg> segs;
+    std::vector<int64_t> seg0_of_chunk;
     int64_t max_t = 0;
     int64_t i0 = 0;
     while (i0 < n_ops) {
@@ -102,6 +120,7 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
         i0 = i1;
         max_t = std::max(max_t, t_bytes);
         dmrgk_renorm::RChunk ch;
+        seg0_of_chunk.push_back(int64_t(segs.size()));
         struct CU {
             int64_t cost;
             Unit u;
@@ -192,7 +211,31 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
         return fail(DMRGK_EINVAL, "renorm_create: too many segments");
     }
     r->t_bytes = round_up(max_t, 128);
-    r->workspace_bytes = std::max<int64_t>(128, r->t_bytes);
+    r->workspace_bytes = std::max<int64_t>(128, 2 * r->t_bytes);      // two T buffers
+    seg0_of_chunk.push_back(int64_t(segs.size()));
+    for (size_t c = 1; c < r->chunks.size(); c += 2) {                // odd chunks use the second buffer
+        const unsigned long long tbuf = (unsigned long long)r->t_bytes;
+        const auto& ch = r->chunks[c];
+        for (int64_t i = ch.p1_unit0; i < ch.p1_unit0 + ch.p1_units; ++i) units[i].C += tbuf;
+        for (int64_t sgi = seg0_of_chunk[c]; sgi < seg0_of_chunk[c + 1]; ++sgi)
+            if (((segs[sgi].flags >> SEG_B_SEL_SHIFT) & 3u) == BASE_WS) segs[sgi].B += tbuf;
+    }
+    {
+        int lo = 0, hi = 0;
+        cudaError_t e = cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&r->s1, cudaStreamNonBlocking, lo);
+        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&r->s2, cudaStreamNonBlocking, hi);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&r->ev_fork, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&r->ev_join, cudaEventDisableTiming);
+        for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+            e = cudaEventCreateWithFlags(&r->ev_p1[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&r->ev_p2[i], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) {
+            dmrgk_renorm_destroy(r);
+            return fail(DMRGK_ECUDA, "renorm_create: stream/event: %s", cudaGetErrorString(e));
+        }
+    }
     for (const auto& c : r->chunks) r->n_launches += (c.p1_units > 0) + (c.p2_units > 0);
     int32_t s = upload(units, &r->units_dev);
     if (s == DMRGK_OK) s = upload(segs, &r->segs_dev);
@@ -226,10 +269,20 @@ int32_t dmrgk_renorm_apply(dmrgk_renorm* r, void* workspace_dev, void* stream) {
     bases.b[BASE_WS] = (unsigned long long)(uintptr_t)workspace_dev;
     bases.b[BASE_PSI] = 0;
     bases.b[BASE_SIGMA] = 0;
-    for (const auto& c : r->chunks) {
-        DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + c.p1_unit0, r->segs_dev, c.p1_units, bases, st));
-        DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + c.p2_unit0, r->segs_dev, c.p2_units, bases, st));
+    DMRGK_CUDA(cudaEventRecord(r->ev_fork, st));
+    DMRGK_CUDA(cudaStreamWaitEvent(r->s1, r->ev_fork, 0));
+    DMRGK_CUDA(cudaStreamWaitEvent(r->s2, r->ev_fork, 0));
+    for (size_t c = 0; c < r->chunks.size(); ++c) {
+        const auto& ch = r->chunks[c];
+        if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(r->s1, r->ev_p2[c & 1], 0));     // T buffer re-use
+        DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p1_unit0, r->segs_dev, ch.p1_units, bases, r->s1));
+        DMRGK_CUDA(cudaEventRecord(r->ev_p1[c & 1], r->s1));
+        DMRGK_CUDA(cudaStreamWaitEvent(r->s2, r->ev_p1[c & 1], 0));
+        DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p2_unit0, r->segs_dev, ch.p2_units, bases, r->s2));
+        DMRGK_CUDA(cudaEventRecord(r->ev_p2[c & 1], r->s2));
     }
+    DMRGK_CUDA(cudaEventRecord(r->ev_join, r->s2));
+    DMRGK_CUDA(cudaStreamWaitEvent(st, r->ev_join, 0));
     return DMRGK_OK;
 }
 
