@@ -59,7 +59,8 @@ typedef struct dmrgk_heff dmrgk_heff;
 typedef struct dmrgk_davidson dmrgk_davidson;
 
 const char* dmrgk_last_error(void);
-/* Library version string, e.g. "dmrgk 0.1 sm_100a". */
+/* Library version string, "dmrgk <version> sm_100a src:<16 hex digits>": the hash identifies the sources
+ * and compiler flags the binary was built from (paper_2311_14106_b200/build.py source_hash). */
 const char* dmrgk_version(void);
 
 /* Number of CUDA kernels this library has launched in the calling process so far (every launch site

@@ -209,7 +209,7 @@ struct dmrgk_renorm {
     // same choreography as dmrgk_heff_apply: phase 1 of chunk c+1 (lowest-priority stream) overlaps
     // phase 2 of chunk c (greatest-priority stream); T is double-buffered
     cudaStream_t s1 = nullptr, s2 = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_p1[2] = {nullptr, nullptr}, ev_p2[2] = {nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_join1 = nullptr, ev_p1[2] = {nullptr, nullptr}, ev_p2[2] = {nullptr, nullptr};
 };
 
 struct dmrgk_heff {
@@ -235,7 +235,7 @@ struct dmrgk_heff {
     // (T is double-buffered), so the tail of one launch is filled by the CTAs of the other
     cudaStream_t side = nullptr;       // phase 1 (lowest priority)
     cudaStream_t side_hi = nullptr;    // phase 2 + reduce (greatest priority: its CTAs are dispatched first)
-    cudaEvent_t ev_join = nullptr;
+    cudaEvent_t ev_join = nullptr, ev_join1 = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_p1[2] = {nullptr, nullptr}, ev_p2[2] = {nullptr, nullptr};
     cudaEvent_t ev_span[2] = {nullptr, nullptr};
     bool span_open = false;

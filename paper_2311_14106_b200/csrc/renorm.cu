@@ -47,6 +47,7 @@ void dmrgk_renorm_destroy(dmrgk_renorm* r) {
     }
     if (r->ev_fork) cudaEventDestroy(r->ev_fork);
     if (r->ev_join) cudaEventDestroy(r->ev_join);
+    if (r->ev_join1) cudaEventDestroy(r->ev_join1);
     if (r->s1) cudaStreamDestroy(r->s1);
     if (r->s2) cudaStreamDestroy(r->s2);
     delete r;
@@ -227,6 +228,7 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
         if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&r->s2, cudaStreamNonBlocking, hi);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&r->ev_fork, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&r->ev_join, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&r->ev_join1, cudaEventDisableTiming);
         for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
             e = cudaEventCreateWithFlags(&r->ev_p1[i], cudaEventDisableTiming);
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&r->ev_p2[i], cudaEventDisableTiming);
@@ -272,18 +274,30 @@ int32_t dmrgk_renorm_apply(dmrgk_renorm* r, void* workspace_dev, void* stream) {
     DMRGK_CUDA(cudaEventRecord(r->ev_fork, st));
     DMRGK_CUDA(cudaStreamWaitEvent(r->s1, r->ev_fork, 0));
     DMRGK_CUDA(cudaStreamWaitEvent(r->s2, r->ev_fork, 0));
-    for (size_t c = 0; c < r->chunks.size(); ++c) {
-        const auto& ch = r->chunks[c];
-        if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(r->s1, r->ev_p2[c & 1], 0));     // T buffer re-use
-        DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p1_unit0, r->segs_dev, ch.p1_units, bases, r->s1));
-        DMRGK_CUDA(cudaEventRecord(r->ev_p1[c & 1], r->s1));
-        DMRGK_CUDA(cudaStreamWaitEvent(r->s2, r->ev_p1[c & 1], 0));
-        DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p2_unit0, r->segs_dev, ch.p2_units, bases, r->s2));
-        DMRGK_CUDA(cudaEventRecord(r->ev_p2[c & 1], r->s2));
+    // every exit path joins the library-owned streams back into the caller's stream (see dmrgk_heff_apply)
+    auto enqueue_chunks = [&]() -> int32_t {
+        for (size_t c = 0; c < r->chunks.size(); ++c) {
+            const auto& ch = r->chunks[c];
+            if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(r->s1, r->ev_p2[c & 1], 0));     // T buffer re-use
+            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p1_unit0, r->segs_dev, ch.p1_units, bases, r->s1));
+            DMRGK_CUDA(cudaEventRecord(r->ev_p1[c & 1], r->s1));
+            DMRGK_CUDA(cudaStreamWaitEvent(r->s2, r->ev_p1[c & 1], 0));
+            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p2_unit0, r->segs_dev, ch.p2_units, bases, r->s2));
+            DMRGK_CUDA(cudaEventRecord(r->ev_p2[c & 1], r->s2));
+        }
+        return DMRGK_OK;
+    };
+    const int32_t status = enqueue_chunks();
+    cudaError_t e = cudaEventRecord(r->ev_join, r->s2);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, r->ev_join, 0);
+    if (e == cudaSuccess) e = cudaEventRecord(r->ev_join1, r->s1);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, r->ev_join1, 0);
+    if (e != cudaSuccess) {
+        cudaStreamSynchronize(r->s1);
+        cudaStreamSynchronize(r->s2);
+        if (status == DMRGK_OK) return fail(DMRGK_ECUDA, "renorm_apply: join failed: %s", cudaGetErrorString(e));
     }
-    DMRGK_CUDA(cudaEventRecord(r->ev_join, r->s2));
-    DMRGK_CUDA(cudaStreamWaitEvent(st, r->ev_join, 0));
-    return DMRGK_OK;
+    return status;
 }
 
 }  // extern "C"

@@ -55,7 +55,10 @@ using namespace dmrgk;
 extern "C" {
 
 const char* dmrgk_last_error(void) { return g_err; }
-const char* dmrgk_version(void) { return "dmrgk 0.1 sm_100a"; }
+#ifndef DMRGK_SOURCE_HASH
+#define DMRGK_SOURCE_HASH "unstamped"
+#endif
+const char* dmrgk_version(void) { return "dmrgk 0.2 sm_100a src:" DMRGK_SOURCE_HASH; }
 int64_t dmrgk_launch_count(int32_t reset) {
     return reset ? g_launches.exchange(0) : g_launches.load();
 }
@@ -324,6 +327,17 @@ int32_t dmrgk_iso_create(dmrgk_ctx* ctx, const dmrgk_space* enlarged, const dmrg
     p->enl = enlarged;
     p->kept = kept;
     p->by_enl.assign(enlarged->n(), -1);
+    // every kept sector that holds states needs its enlarged counterpart: otherwise the renormalised
+    // blocks on that sector would have no producer and would silently keep stale values
+    for (int k = 0; k < kept->n(); ++k) {
+        if (kept->dim[k] == 0) continue;
+        const int e = enlarged->find(kept->q[2 * k], kept->q[2 * k + 1]);
+        if (e < 0 || enlarged->dim[e] == 0) {
+            delete p;
+            return fail(DMRGK_ESHAPE, "iso_create: kept sector %d (charge %d,%d; %d states) has no enlarged sector", k,
+                        kept->q[2 * k], kept->q[2 * k + 1], kept->dim[k]);
+        }
+    }
     int64_t off = 0, uoff = 0;
     for (int e = 0; e < enlarged->n(); ++e) {
         const int k = kept->find(enlarged->q[2 * e], enlarged->q[2 * e + 1]);

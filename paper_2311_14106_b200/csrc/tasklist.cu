@@ -69,6 +69,7 @@ void dmrgk_heff_destroy(dmrgk_heff* h) {
     }
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->ev_join) cudaEventDestroy(h->ev_join);
+    if (h->ev_join1) cudaEventDestroy(h->ev_join1);
     if (h->side) cudaStreamDestroy(h->side);
     if (h->side_hi) cudaStreamDestroy(h->side_hi);
     for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
@@ -116,6 +117,14 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             if (op->pinned && ring_part == 0) return fail(DMRGK_ESTATE, "heff_create: pair %lld has a pinned operator but ring_bytes = 0", (long long)k);
             if (op->pinned && op->n_padded * 8 > ring_part)
                 return fail(DMRGK_ENOMEM, "heff_create: pinned operator of %lld bytes exceeds a third of the ring (%lld)", (long long)(op->n_padded * 8), (long long)ring_part);
+        }
+        // both operators of a pair are staged into the SAME ring part: together they must fit it
+        {
+            int64_t need = 0;
+            if (L[k] && L[k]->pinned && !L[k]->dev) need += round_up(L[k]->n_padded * 8, 128);
+            if (R[k] && R[k]->pinned && !R[k]->dev && (const dmrgk_op*)R[k] != (const dmrgk_op*)L[k]) need += round_up(R[k]->n_padded * 8, 128);
+            if (need > ring_part)
+                return fail(DMRGK_ENOMEM, "heff_create: the pinned operators of pair %lld need %lld bytes together, more than a third of the ring (%lld)", (long long)k, (long long)need, (long long)ring_part);
         }
     }
 
@@ -532,6 +541,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
         if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&h->side_hi, cudaStreamNonBlocking, prio_hi);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_join1, cudaEventDisableTiming);
         for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
             e = cudaEventCreateWithFlags(&h->ev_p1[i], cudaEventDisableTiming);
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_p2[i], cudaEventDisableTiming);
@@ -664,6 +674,10 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
         DMRGK_CUDA(cudaStreamWaitEvent(s1, h->ev_fork, 0));
         DMRGK_CUDA(cudaStreamWaitEvent(s2, h->ev_fork, 0));
     }
+    // The chunk loop runs inside a lambda so that EVERY exit path — also a failed launch or event call
+    // half-way — joins the library-owned streams back into `main` and closes the profiling span: the
+    // caller only orders against `main` and may free ψ / σ / workspace right after an error return.
+    auto enqueue_chunks = [&]() -> int32_t {
     if (nc) DMRGK_TRY(stage_chunk(h, h->chunks[0], (char*)workspace_dev, main, copy, s1, s2));
     for (size_t c = 0; c < nc; ++c) {
         const Chunk& ch = h->chunks[c];
@@ -685,11 +699,27 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
         DMRGK_TRY(chunk_done(h, ch, s2));
         if (c + 1 < nc) DMRGK_TRY(stage_chunk(h, h->chunks[c + 1], (char*)workspace_dev, main, copy, s1, s2));
     }
+    return DMRGK_OK;
+    };
+    const int32_t status = enqueue_chunks();
     if (!serial) {
-        DMRGK_CUDA(cudaEventRecord(h->ev_join, s2));      // s2 has waited for every p1 launch of s1
-        DMRGK_CUDA(cudaStreamWaitEvent(main, h->ev_join, 0));
+        // on success s2 has already waited for every p1 launch of s1; after an error it may not have,
+        // so main waits for both streams explicitly
+        cudaError_t e = cudaEventRecord(h->ev_join, s2);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(main, h->ev_join, 0);
+        if (e == cudaSuccess) e = cudaEventRecord(h->ev_join1, s1);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(main, h->ev_join1, 0);
+        if (e != cudaSuccess) {
+            cudaStreamSynchronize(s1);                    // last resort: nothing may outlive the call
+            cudaStreamSynchronize(s2);
+            if (status == DMRGK_OK) return fail(DMRGK_ECUDA, "heff_apply: join failed: %s", cudaGetErrorString(e));
+        }
     }
-    DMRGK_TRY(prof_end(h, span_slot, main));
+    {
+        const int32_t ps = prof_end(h, span_slot, main);
+        if (status != DMRGK_OK) return status;
+        if (ps != DMRGK_OK) return ps;
+    }
     if (h->prof_on && !serial) {
         for (const Chunk& ch : h->chunks) {
             h->prof_launches[0] += ch.p1_units > 0;

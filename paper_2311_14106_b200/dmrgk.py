@@ -114,13 +114,30 @@ def load(path=None):
         raise FileNotFoundError(
             f"{path} not found: build it with `python -m paper_2311_14106_b200.build` "
             "(dmrgk has no CPU or PyTorch fallback)")
+    if path == LIB_PATH:
+        # a binary built from other sources than the ones beside it must not be loaded silently
+        # (mtimes mean nothing after a checkout or a copy): rebuild it, or fail
+        from . import build as _build
+        if _build.built_hash() != _build.source_hash():
+            _build.build()
     lib = C.CDLL(path)
     for name, (res, args) in SIGNATURES.items():
         fn = getattr(lib, name)
         fn.restype = res
         fn.argtypes = args
+    if path == LIB_PATH:
+        from . import build as _build
+        have = lib.dmrgk_version().decode().rsplit("src:", 1)[-1]
+        if have != _build.source_hash():
+            raise RuntimeError(f"{path} was built from sources {have}, the tree holds {_build.source_hash()}: "
+                               "rebuild with `python -m paper_2311_14106_b200.build --force`")
     _lib = lib
     return lib
+
+
+def source_hash():
+    """The source hash compiled into the loaded library (dmrgk_version)."""
+    return load().dmrgk_version().decode().rsplit("src:", 1)[-1]
 
 
 def last_error():

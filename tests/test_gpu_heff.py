@@ -198,6 +198,29 @@ def test_staged_operators_bit_identical_to_resident():
     assert float((first - ref).abs().max() / ref.abs().max()) <= 1e-13
 
 
+def test_staging_ring_too_small_for_a_pair_is_refused():
+    """Both operators of a pair are staged into the same ring part: a ring whose third holds either
+    operator alone but not the two together must be refused at create time (DMRGK_ENOMEM), not
+    overflowed at apply time."""
+    from paper_2311_14106_b200 import dmrgk, problem
+    wl = medium_spinless()
+    probe = problem.from_workload(wl)
+    pairs = [(t.L, t.R) for t in wl.terms if t.L is not None and t.R is not None]
+    L, R = max(pairs, key=lambda p: probe.ops[p[0]].n_padded + probe.ops[p[1]].n_padded)
+    nl, nr = probe.ops[L].n_padded * 8, probe.ops[R].n_padded * 8
+    third = (max(nl, nr) + nl + nr) // 2 // 128 * 128          # ≥ each alone, < both together
+    assert max(nl, nr) <= third < nl + nr
+    with pytest.raises(dmrgk.DmrgkError) as e:
+        problem.from_workload(wl, pinned=[L, R], ring_bytes=3 * third)
+    assert e.value.status == dmrgk.ENOMEM
+    ok = problem.from_workload(wl, pinned=[L, R], ring_bytes=3 * (nl + nr + 256))
+    psi = ok.psi_fill(wl.seed, wlmod.PSI_STREAM)
+    ref = probe.apply(probe.psi_fill(wl.seed, wlmod.PSI_STREAM))
+    got = ok.apply(psi)
+    torch.cuda.synchronize()
+    assert float((got - ref).abs().max() / ref.abs().max()) <= 1e-13
+
+
 def test_apply_host_end_to_end():
     wl = medium_config2()
     pb = heff.problem_from_workload(wl)

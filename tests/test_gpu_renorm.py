@@ -130,6 +130,10 @@ def test_errors():
     with pytest.raises(dmrgk.DmrgkError) as e:
         problem.RenormProblem(dp, "A", too_many)
     assert e.value.status == dmrgk.ESHAPE
+    orphan = list(sectors_new) + [((99,), 2)]           # a kept sector with no enlarged counterpart
+    with pytest.raises(dmrgk.DmrgkError) as e:
+        problem.RenormProblem(dp, "A", orphan)
+    assert e.value.status == dmrgk.ESHAPE and "no enlarged sector" in e.value.message
 
 
 def test_config4_half_sampled_operators():
