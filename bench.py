@@ -561,6 +561,41 @@ def run_renorm(args):
     print(json.dumps(out), flush=True)
 
 
+def run_loop_probe(args):
+    """--op loop_probe: the k-tile-loop skeletons of csrc/probe_gemm.cu (harness, not the product path)
+    and the register-only pipe probes in all shapes — the ceilings design decisions are judged against."""
+    import torch
+    from paper_2311_14106_b200 import dmrgk
+    torch.cuda.set_device(0)
+    ctx = dmrgk.Ctx(0)
+    st = torch.cuda.current_stream()
+    buf = (torch.rand(1 << 23, dtype=torch.float64, device="cuda") - 0.5) * 1e-3      # 64 MiB, L2-resident
+    sink = torch.zeros(16, dtype=torch.float64, device="cuda")
+    out = {"op": "loop_probe", "source_hash": dmrgk.source_hash(), "n_sm": ctx.query()[0]}
+    cs = ClockSampler(0)
+    cs.start()
+    for kind, name in ((0, "cp.async 64x64 (round-1 loop)"), (1, "cp.async.bulk + mbarrier 64x64"),
+                       (2, "cp.async.bulk + mbarrier 128x64")):
+        dmrgk.probe_gemm_loop(ctx, kind, 2000, buf, sink, st)
+        best = 0.0
+        for _ in range(5):
+            box = {}
+            ms = timed(st, lambda: box.setdefault("f", dmrgk.probe_gemm_loop(ctx, kind, 20000, buf, sink, st)))
+            best = max(best, box["f"] / ms / 1e9)
+        out[f"gemm_loop_kind{kind}"] = {"what": name, "tflops": best}
+    for kind, name in ((0, "DMMA 4 CTAs x 8 warps / SM"), (2, "DMMA 1 x 4 warps / SM"), (3, "DMMA 2 x 4 warps / SM"),
+                       (4, "DMMA 3 x 4 warps / SM"), (1, "DFMA 4 x 8 warps / SM")):
+        dmrgk.probe_fp64(ctx, kind, 20000, sink, st)
+        best = 0.0
+        for _ in range(3):
+            box = {}
+            ms = timed(st, lambda: box.setdefault("f", dmrgk.probe_fp64(ctx, kind, 200000, sink, st)))
+            best = max(best, box["f"] / ms / 1e9)
+        out[f"pipe_probe_kind{kind}"] = {"what": name, "tflops": best}
+    out["clocks"] = cs.stop()
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -572,13 +607,15 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-extras", dest="no_extras", action="store_true",
                     help="skip the extra rows (renormalisation, configs 3 and 2) of the default config-4 line")
-    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm"],
+    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "loop_probe"],
                     help="davidson (default, the headline hot path) or renorm (NEXT-1 row, its own metric)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
     elif args.op == "renorm":
         run_renorm(args)
+    elif args.op == "loop_probe":
+        run_loop_probe(args)
     else:
         run_ours(args)
 

@@ -287,10 +287,18 @@ int32_t dmrgk_layout_fill_normal(const dmrgk_layout* l, double* arena_dev, uint6
 int32_t dmrgk_iso_fill_normal(const dmrgk_iso* phi, double* arena_dev, uint64_t seed, uint64_t stream_id,
                               void* stream);
 /* Register-only FP64 pipe probes: every warp of a full grid issues `iters` rounds of 16 independent
- * mma.sync.m8n8k4.f64 (kind 0) or 32 independent fma.rn.f64 per lane (kind 1).  Returns the flops
- * issued in *flops; the caller times the stream with events. */
+ * mma.sync.m8n8k4.f64 (kind 0: 4 CTAs × 8 warps per SM; kinds 2, 3, 4: 1, 2, 3 CTAs × 4 warps per SM)
+ * or 32 independent fma.rn.f64 per lane (kind 1).  Returns the flops issued in *flops; the caller
+ * times the stream with events. */
 int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* sink_dev,
                          double* flops, void* stream);
+/* Skeletons of the k-tile loop of the grouped GEMM kernel (csrc/probe_gemm.cu): every CTA of a full
+ * grid (3 per SM) runs `ktiles` dense k-tiles of 16 with operand tiles streamed from buf_dev (≥ 1 MiB,
+ * any finite values).  kind 0: 64×64 tile staged by cp.async from every thread (the round-1 loop);
+ * kind 1: 64×64 tile staged by cp.async.bulk from one elected thread with full/empty mbarriers;
+ * kind 2: 128×64 tile, otherwise as kind 1.  Returns the flops issued in *flops. */
+int32_t dmrgk_probe_gemm_loop(dmrgk_ctx* ctx, int32_t kind, int32_t ktiles, const double* buf_dev,
+                              int64_t buf_doubles, double* sink_dev, double* flops, void* stream);
 
 #ifdef __cplusplus
 }

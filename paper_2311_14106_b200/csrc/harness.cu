@@ -136,8 +136,14 @@ int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* si
                          void* stream) {
     if (!ctx || !sink_dev || iters < 0) return fail(DMRGK_EINVAL, "probe_fp64: bad argument");
     DMRGK_CUDA(cudaSetDevice(ctx->device));
-    const int blocks = ctx->n_sm * 4, threads = 256;
-    if (kind == 0) {
+    int blocks = ctx->n_sm * 4, threads = 256;
+    if (kind == 0 || (kind >= 2 && kind <= 4)) {
+        // kind 0: 4 CTAs × 8 warps per SM; kinds 2-4: 1, 2, 3 CTAs × 4 warps per SM (3 × 4 is the
+        // residency of the GEMM kernel) — the DMMA rate a box shows depends on the shape
+        if (kind >= 2) {
+            blocks = ctx->n_sm * (kind - 1);
+            threads = 128;
+        }
         probe_dmma_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(iters, sink_dev);
         count_launch();
         if (flops) *flops = double(blocks) * (threads / 32) * double(iters) * 16.0 * 512.0;
@@ -146,7 +152,7 @@ int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* si
         count_launch();
         if (flops) *flops = double(blocks) * threads * double(iters) * 32.0 * 2.0;
     } else {
-        return fail(DMRGK_EINVAL, "probe_fp64: kind must be 0 (DMMA) or 1 (DFMA)");
+        return fail(DMRGK_EINVAL, "probe_fp64: kind must be 0, 2, 3, 4 (DMMA shapes) or 1 (DFMA)");
     }
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;

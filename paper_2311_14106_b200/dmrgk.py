@@ -99,6 +99,7 @@ SIGNATURES = {
     "dmrgk_op_fill_normal": (_i32, [_p, _p, _u64, _u64, _i32, _i32, _p]),
     "dmrgk_layout_fill_normal": (_i32, [_p, _p, _u64, _u64, _p]),
     "dmrgk_probe_fp64": (_i32, [_p, _i32, _i64, _p, _pf64, _p]),
+    "dmrgk_probe_gemm_loop": (_i32, [_p, _i32, _i32, _p, _i64, _p, _pf64, _p]),
 }
 
 _lib = None
@@ -495,6 +496,13 @@ def vec_residual(ctx, n, m, V, W, stride, coef, r, out, scratch, stream=None):
 
 def vec_precond(ctx, n, r, diag, theta_dev, t, stream=None):
     check(ctx.lib.dmrgk_vec_precond(ctx.h, n, _dev(r), _dev(diag), _dev(theta_dev), _dev(t), _stream(stream)))
+
+
+def probe_gemm_loop(ctx, kind, ktiles, buf, sink, stream=None):
+    fl = C.c_double()
+    check(ctx.lib.dmrgk_probe_gemm_loop(ctx.h, kind, ktiles, _dev(buf), buf.numel(), _dev(sink), C.byref(fl),
+                                        _stream(stream)))
+    return fl.value
 
 
 def probe_fp64(ctx, kind, iters, sink, stream=None):
