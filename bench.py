@@ -255,7 +255,7 @@ def read_traffic_table(workload, kernel_hash):
     return None, f"no ncu capture of workload {workload} with kernel sources {kernel_hash} in profiles/traffic.csv"
 
 
-def davidson_bench(dp, wl, args, world, local, steps, warmup, profile=True):
+def davidson_bench(dp, wl, args, world, local, steps, warmup, make_davidson=None):
     """W warm-up + K timed Davidson steps (each exactly one H_eff apply) on a built problem."""
     import torch
     import torch.distributed as dist
@@ -263,7 +263,8 @@ def davidson_bench(dp, wl, args, world, local, steps, warmup, profile=True):
     from paper_2311_14106_b200 import dmrgk
     h = dp.heff
     psi = dp.psi_fill(wl.seed, wlmod.PSI_STREAM)
-    dav = dp.davidson(m_max=args.m_max, tol=0.0, max_iter=1 << 30)     # tol 0: never stops early
+    make_davidson = make_davidson or dp.davidson
+    dav = make_davidson(m_max=args.m_max, tol=0.0, max_iter=1 << 30)     # tol 0: never stops early
     dav.start(psi)
 
     def barrier():
@@ -317,6 +318,8 @@ def run_ours(args):
     dmrgk.load()
 
     wl = make_workload(args.config)
+    if args.shard == "k" and world > 1:
+        return run_sharded(args, wl, rank, world, local)
     staged = wlmod.config5_staged_ops(wl) if args.config == "5" else []
     dp = problem.from_workload(wl, device=local, pinned=staged, **({"ring_bytes": 6 << 30} if staged else {}))
     torch.cuda.synchronize()
@@ -461,6 +464,44 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sharded(args, wl, rank, world, local):
+    """--shard k at N > 1: the operator-pair list is split over the ranks (balanced
+    by flops and bytes), ψ is replicated, every apply is followed by ONE NCCL all-reduce (sum) of the
+    ψ-sized σ over NVLink, the Davidson iteration runs replicated.  Total work is fixed ⇒ "strong"
+    scaling; value = flops of the WHOLE list ÷ max-over-ranks step time.  UNMEASURED on hardware in this
+    build (one GPU per call); covered by tests/test_shard.py."""
+    import torch
+    import torch.distributed as dist
+    from paper_2311_14106_b200 import dmrgk, shard
+    sp = shard.ShardedProblem(wl, rank, world, device=local)
+    torch.cuda.synchronize()
+    flops_total = float(shard.term_costs(wl)[0].sum())
+    r = davidson_bench(sp.dp, sp.wl, args, world, local, args.steps, args.warmup, make_davidson=sp.davidson)
+    ms_step = r["ms_step"]
+    n = sp.dp.layout.n_padded
+    sm_max = r["clocks"].get("sm_max_mhz") or 1965.0
+    peak = sp.dp.ctx.query()[0] * 128 * sm_max * 1e6 / 1e12
+    gemm_ms = max_over_ranks(r["prof_ms"]["apply"], world, "cuda")
+    out = {"metric": METRIC, "value": flops_total / ms_step / 1e9, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": wl.name, "parallelism": f"k-sharded x{world}: pair list split by flops and bytes, psi replicated, "
+                      "one NCCL all-reduce (sum) of sigma per apply", "K_pairs": len(wl.terms),
+                      "pairs_per_rank": [len(s) for s in sp.shards], "flops_per_rank": [st["flops"] for st in sp.stats],
+                      "op_bytes_per_rank": [st["bytes"] for st in sp.stats], "flops_alg_per_apply": flops_total,
+                      "allreduce_bytes_per_apply": int(n * 8), "source_hash": dmrgk.source_hash(),
+                      "l2": "operator arenas (>> 126 MB L2) are streamed once per step; no flush needed"},
+           "gpu_launches": r["launches"], "theta_last": r["theta"], "resnorm_last": r["rho"],
+           "roofline": {"bound": "tensor", "kernel": "heff_gemm_dmma_kernel (a5 + a6), slowest rank", "peak": peak * world,
+                        "achieved": flops_total * args.steps / gemm_ms / 1e9 if gemm_ms > 0 else None, "unit": "TFLOP/s",
+                        "frac": (flops_total * args.steps / gemm_ms / 1e9) / (peak * world) if gemm_ms > 0 else None,
+                        "peak_source": f"of derived: {world} x 148 SMs x 128 FP64 flop/clk x {sm_max:.0f} MHz", "traffic": None},
+           "e2e": None, "clocks": r["clocks"]}
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    dist.destroy_process_group()
+
+
 def cpu_baseline_from_device(dp, wl, args, budget_s=25.0):
     """The oracle (oracle.heff.sigma_blockwise, NumPy/BLAS, as it stands) on the host cores, on a
     stratified sample of the operator pairs (every CPU_EVERY-th pair ≈ 5 %) with all ψ
@@ -575,7 +616,8 @@ def run_loop_probe(args):
     cs = ClockSampler(0)
     cs.start()
     for kind, name in ((0, "cp.async 64x64 (round-1 loop)"), (1, "cp.async.bulk + mbarrier 64x64"),
-                       (2, "cp.async.bulk + mbarrier 128x64")):
+                       (2, "cp.async.bulk + mbarrier 128x64"), (3, "cp.async producer warp + mbarrier 128x64, 2 CTAs/SM"),
+                       (4, "cp.async.bulk + mbarrier 128x64, 2 CTAs/SM, 4 stages"), (5, "cp.async.bulk + mbarrier 64x64, 2 CTAs/SM")):
         dmrgk.probe_gemm_loop(ctx, kind, 2000, buf, sink, st)
         best = 0.0
         for _ in range(5):
@@ -607,6 +649,9 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-extras", dest="no_extras", action="store_true",
                     help="skip the extra rows (renormalisation, configs 3 and 2) of the default config-4 line")
+    ap.add_argument("--shard", default="none", choices=["none", "k"],
+                    help="N > 1 only: 'none' = independent replicas (the scope of BASELINE.json), 'k' = split the operator-pair "
+                         "list over the ranks and all-reduce sigma (SURVEY §8(f) NEXT-2)")
     ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "loop_probe"],
                     help="davidson (default, the headline hot path) or renorm (NEXT-1 row, its own metric)")
     args = ap.parse_args()

@@ -230,6 +230,14 @@ int32_t dmrgk_davidson_solve(dmrgk_davidson* d, double* theta, double* resnorm, 
                              int32_t* n_apply);
 /* Current subspace size m. */
 int32_t dmrgk_davidson_query(const dmrgk_davidson* d, int32_t* m, int32_t* n_apply);
+/* Multi-GPU k-sharding hook (the sum over operator pairs
+ * is split over the GPUs, ψ is replicated, σ is the sum of the ranks' partial results).  When set, fn
+ * is called right after every H_eff apply of the driver with the freshly written W vector (device
+ * pointer, n_padded doubles) and the main stream; it must turn the vector into the SUM over all ranks
+ * in stream order (e.g. an NCCL all-reduce) and return 0.  Every rank then iterates on identical
+ * data.  fn = NULL removes the hook.  The library itself never communicates. */
+typedef int32_t (*dmrgk_allreduce_fn)(double* vec_dev, int64_t n, void* stream, void* user);
+int32_t dmrgk_davidson_set_allreduce(dmrgk_davidson* d, dmrgk_allreduce_fn fn, void* user);
 
 /* ---- renormalisation step ("the renormalization step",
  *      PAPER.md:142 Fig. 7 "Ren_l", "Ren_r"):  O′ = Φᵀ O Φ  for every operator kept -------------- */
@@ -296,7 +304,8 @@ int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* si
  * grid (3 per SM) runs `ktiles` dense k-tiles of 16 with operand tiles streamed from buf_dev (≥ 1 MiB,
  * any finite values).  kind 0: 64×64 tile staged by cp.async from every thread (the round-1 loop);
  * kind 1: 64×64 tile staged by cp.async.bulk from one elected thread with full/empty mbarriers;
- * kind 2: 128×64 tile, otherwise as kind 1.  Returns the flops issued in *flops. */
+ * kind 2: 128×64 tile, otherwise as kind 1; kind 3: 128×64 tile, cp.async from a dedicated producer warp
+ * (2 CTAs per SM); kinds 4, 5: kinds 2, 1 at 2 CTAs per SM.  Returns the flops issued in *flops. */
 int32_t dmrgk_probe_gemm_loop(dmrgk_ctx* ctx, int32_t kind, int32_t ktiles, const double* buf_dev,
                               int64_t buf_doubles, double* sink_dev, double* flops, void* stream);
 

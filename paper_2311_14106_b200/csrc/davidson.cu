@@ -37,6 +37,8 @@ struct dmrgk_davidson {
     int m = 0, n_apply = 0;
     bool started = false, converged = false;
     double theta = 0.0, rho = 0.0;
+    dmrgk_allreduce_fn reduce = nullptr;   // k-sharding hook: makes W_j the sum over all ranks
+    void* reduce_user = nullptr;
 };
 
 namespace {
@@ -92,6 +94,17 @@ void jacobi_lowest(std::vector<double>& A, int m, double* theta, std::vector<dou
 int32_t read_back(dmrgk_davidson* d, int count) {
     DMRGK_CUDA(cudaMemcpyAsync(d->host + 64, d->out, size_t(count) * 8, cudaMemcpyDeviceToHost, d->main));
     DMRGK_CUDA(cudaStreamSynchronize(d->main));
+    return DMRGK_OK;
+}
+
+// w = H v on this rank's share of the pair list, then the all-reduce hook (if any) completes it
+int32_t apply_h(dmrgk_davidson* d, const double* v, double* w) {
+    DMRGK_TRY(dmrgk_heff_apply(d->h, v, w, d->ws, d->main, d->copy));
+    if (d->reduce) {
+        const int32_t s = d->reduce(w, d->n, (void*)d->main, d->reduce_user);
+        if (s != 0) return fail(DMRGK_ESTATE, "davidson: the all-reduce hook failed (%d)", s);
+    }
+    d->n_apply += 1;
     return DMRGK_OK;
 }
 
@@ -195,8 +208,7 @@ int32_t dmrgk_davidson_start(dmrgk_davidson* d, const double* x0_dev) {
     if (!(d->host[64] > 0.0) || !std::isfinite(d->host[64]))
         return fail(DMRGK_EINVAL, "davidson_start: start vector has norm² = %g", d->host[64]);
     DMRGK_TRY(dmrgk_vec_scal_dev(d->ctx, d->n, d->out, 3, x0_dev, d->V, d->main));
-    DMRGK_TRY(dmrgk_heff_apply(d->h, d->V, d->W, d->ws, d->main, d->copy));
-    d->n_apply = 1;
+    DMRGK_TRY(apply_h(d, d->V, d->W));
     DMRGK_TRY(extend_G(d));
     d->m = 1;
     d->started = true;
@@ -249,8 +261,7 @@ int32_t dmrgk_davidson_step(dmrgk_davidson* d, double* theta, double* resnorm, i
     double* v = d->V + int64_t(d->m) * d->n;
     double* w = d->W + int64_t(d->m) * d->n;
     DMRGK_TRY(dmrgk_vec_scal_dev(d->ctx, d->n, d->out, 3, d->t, v, d->main));
-    DMRGK_TRY(dmrgk_heff_apply(d->h, v, w, d->ws, d->main, d->copy));
-    d->n_apply += 1;
+    DMRGK_TRY(apply_h(d, v, w));
     DMRGK_TRY(extend_G(d));
     d->m += 1;
     return DMRGK_OK;
@@ -291,6 +302,13 @@ int32_t dmrgk_davidson_solve(dmrgk_davidson* d, double* theta, double* resnorm, 
     if (resnorm) *resnorm = rn;
     if (n_apply) *n_apply = d->n_apply;
     if (!conv) return fail(DMRGK_ENOTCONV, "davidson_solve: ‖r‖ = %.3e > tol = %.3e after %d applies", rn, d->tol, d->n_apply);
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_davidson_set_allreduce(dmrgk_davidson* d, dmrgk_allreduce_fn fn, void* user) {
+    if (!d) return fail(DMRGK_EINVAL, "davidson_set_allreduce: solver is NULL");
+    d->reduce = fn;
+    d->reduce_user = user;
     return DMRGK_OK;
 }
 

@@ -11,6 +11,9 @@
 //           mbarriers instead of __syncthreads, dense 128-byte shared rows with the 32-byte-group XOR
 //           swizzle already present in global memory (panel layout)
 //   kind 2: as kind 1 with a 128×64 CTA tile, 2×2 warps of 64×32 (8×4 fragments), 3 stages
+//   kind 3: 128×64 tile, row-major source, cp.async issued by a dedicated fifth (producer) warp and
+//           signalled through mbarriers; 160 threads, 2 CTAs per SM
+//   kind 4: kind 2 at 2 CTAs per SM with 4 stages;   kind 5: kind 1 at 2 CTAs per SM
 #include "internal.h"
 
 namespace dmrgk {
@@ -126,8 +129,8 @@ probe_loop_cpasync(const double* __restrict__ buf, long long span_tiles, int kti
 // sits at row·16 + (k ^ ((row & 3) << 2)) — the swizzle is in the global panel, the copy is verbatim.
 // Lane (g, t4) of a fragment reads row (…+g), k = 4·ks + t4 → offset 4·(ks ^ (g & 3)) + t4: the 16 lanes
 // of a half-warp hit 16 distinct 8-byte banks.
-template <int FM, int STAGES>
-__global__ void __launch_bounds__(NTHREADS, 3)
+template <int FM, int STAGES, int MINB>
+__global__ void __launch_bounds__(NTHREADS, MINB)
 probe_loop_bulk(const double* __restrict__ buf, long long span_tiles, int ktiles, double* sink) {
     constexpr int BM = FM * 16;                      // 2 warps along M, FM fragments of 8 rows each
     constexpr int A_DOUBLES = BM * BK, B_DOUBLES = 64 * BK, STAGE_DOUBLES = A_DOUBLES + B_DOUBLES;
@@ -209,6 +212,87 @@ probe_loop_bulk(const double* __restrict__ buf, long long span_tiles, int ktiles
     if (sum == 123.456) sink[0] = sum;
 }
 
+// ---- kind 3: cp.async issued by a dedicated PRODUCER WARP, full/empty mbarriers --------------------
+// Keeps the row-major global layout (tile rows are `ld` apart; here ld = 16) and the padded shared
+// strides of kind 0, but the four compute warps carry no loader state: a fifth warp issues every
+// 16-byte cp.async of the stage (48 per lane for a 128×64 tile pair) and lets the copies arrive on the
+// stage's full barrier (cp.async.mbarrier.arrive.noinc).  160 threads, 2 CTAs per SM.
+constexpr int K3_STRIDE = 20, K3_STAGES = 3, K3_A = 128 * K3_STRIDE, K3_B = 64 * K3_STRIDE;
+constexpr int K3_STAGE = K3_A + K3_B, K3_SMEM = K3_STAGES * K3_STAGE * 8;
+
+__global__ void __launch_bounds__(160, 2)
+probe_loop_producer_warp(const double* __restrict__ buf, long long span_tiles, int ktiles, double* sink) {
+    extern __shared__ __align__(128) double smem[];
+    __shared__ __align__(8) unsigned long long bars[2 * K3_STAGES];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const double* A = buf + (long long)(blockIdx.x % 32) * span_tiles * 2048;
+    const double* B = buf + (long long)(32 + (blockIdx.x / 32) % 32) * span_tiles * 2048;
+    const uint32_t sbase = smem_u32(smem), bar0 = smem_u32(bars);
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < K3_STAGES; ++s) {
+            mbar_init(bar0 + s * 8, 32);                     // full[s]: one deferred arrive per producer lane
+            mbar_init(bar0 + (K3_STAGES + s) * 8, 4);        // empty[s]: one arrive per consumer warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == 4) {
+        // producer: lane owns chunk ch = lane & 7 of rows (lane >> 3) + 4·j
+        const int r0 = lane >> 3, ch = lane & 7;
+        for (int kt = 0; kt < ktiles; ++kt) {
+            const int s = kt % K3_STAGES;
+            if (kt >= K3_STAGES) mbar_wait(bar0 + (K3_STAGES + s) * 8, ((kt / K3_STAGES) - 1) & 1);
+            const long long t = kt % span_tiles;
+            const double* srcA = A + t * 2048 + r0 * 16 + ch * 2;
+            const double* srcB = B + t * 1024 + r0 * 16 + ch * 2;
+            const uint32_t dA = sbase + (s * K3_STAGE + r0 * K3_STRIDE + ch * 2) * 8;
+            const uint32_t dB = dA + K3_A * 8;
+#pragma unroll 8
+            for (int j = 0; j < 32; ++j)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dA + j * 4 * K3_STRIDE * 8), "l"(srcA + j * 64));
+#pragma unroll 8
+            for (int j = 0; j < 16; ++j)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dB + j * 4 * K3_STRIDE * 8), "l"(srcB + j * 64));
+            asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar0 + s * 8) : "memory");
+        }
+        asm volatile("cp.async.wait_all;\n" ::: "memory");
+        return;
+    }
+    const int wm = warp >> 1, wn = warp & 1, g = lane >> 2, t4 = lane & 3;
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    for (int it = 0; it < ktiles; ++it) {
+        const int s = it % K3_STAGES;
+        mbar_wait(bar0 + s * 8, (it / K3_STAGES) & 1);
+        const double* pa = smem + s * K3_STAGE + (wm * 64 + g) * K3_STRIDE + t4;
+        const double* pb = smem + s * K3_STAGE + K3_A + (wn * 32 + g) * K3_STRIDE + t4;
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks) {
+            double af[8], bf[4];
+#pragma unroll
+            for (int f = 0; f < 8; ++f) af[f] = pa[f * 8 * K3_STRIDE + ks * 4];
+#pragma unroll
+            for (int f = 0; f < 4; ++f) bf[f] = pb[f * 8 * K3_STRIDE + ks * 4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar0 + (K3_STAGES + s) * 8);
+    }
+    double sum = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) sum += acc[i][j][0] + acc[i][j][1];
+    if (sum == 123.456) sink[0] = sum;
+}
+
 }  // namespace pg
 }  // namespace dmrgk
 
@@ -224,24 +308,42 @@ extern "C" int32_t dmrgk_probe_gemm_loop(dmrgk_ctx* ctx, int32_t kind, int32_t k
     // 64 spans (32 for A, 32 for B) of span_tiles tiles each; a tile is ≤ 2048 doubles
     const long long span_tiles = buf_doubles / (64LL * 2048);
     if (span_tiles < 1) return fail(DMRGK_EINVAL, "probe_gemm_loop: buffer too small (need ≥ 1 MiB)");
-    int bm = 64;
+    int bm = 64, ctas = 3;
     if (kind == 0) {
         DMRGK_CUDA(cudaFuncSetAttribute(pg::probe_loop_cpasync, cudaFuncAttributeMaxDynamicSharedMemorySize, pg::K0_SMEM));
         pg::probe_loop_cpasync<<<grid, pg::NTHREADS, pg::K0_SMEM, st>>>(buf_dev, span_tiles, ktiles, sink_dev);
-    } else if (kind == 1) {
+    } else if (kind == 1 || kind == 5) {
         constexpr int smem = 4 * (64 + 64) * 16 * 8;
-        DMRGK_CUDA(cudaFuncSetAttribute(pg::probe_loop_bulk<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        pg::probe_loop_bulk<4, 4><<<grid, pg::NTHREADS, smem, st>>>(buf_dev, span_tiles, ktiles, sink_dev);
-    } else if (kind == 2) {
-        constexpr int smem = 3 * (128 + 64) * 16 * 8;
-        DMRGK_CUDA(cudaFuncSetAttribute(pg::probe_loop_bulk<8, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        pg::probe_loop_bulk<8, 3><<<grid, pg::NTHREADS, smem, st>>>(buf_dev, span_tiles, ktiles, sink_dev);
+        if (kind == 1) {
+            DMRGK_CUDA(cudaFuncSetAttribute(pg::probe_loop_bulk<4, 4, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            pg::probe_loop_bulk<4, 4, 3><<<grid, pg::NTHREADS, smem, st>>>(buf_dev, span_tiles, ktiles, sink_dev);
+        } else {
+            ctas = 2;
+            DMRGK_CUDA(cudaFuncSetAttribute(pg::probe_loop_bulk<4, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            pg::probe_loop_bulk<4, 4, 2><<<ctx->n_sm * 2, pg::NTHREADS, smem, st>>>(buf_dev, span_tiles, ktiles, sink_dev);
+        }
+    } else if (kind == 2 || kind == 4) {
         bm = 128;
+        if (kind == 2) {
+            constexpr int smem = 3 * (128 + 64) * 16 * 8;
+            DMRGK_CUDA(cudaFuncSetAttribute(pg::probe_loop_bulk<8, 3, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            pg::probe_loop_bulk<8, 3, 3><<<grid, pg::NTHREADS, smem, st>>>(buf_dev, span_tiles, ktiles, sink_dev);
+        } else {
+            ctas = 2;
+            constexpr int smem = 4 * (128 + 64) * 16 * 8;
+            DMRGK_CUDA(cudaFuncSetAttribute(pg::probe_loop_bulk<8, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            pg::probe_loop_bulk<8, 4, 2><<<ctx->n_sm * 2, pg::NTHREADS, smem, st>>>(buf_dev, span_tiles, ktiles, sink_dev);
+        }
+    } else if (kind == 3) {
+        bm = 128;
+        ctas = 2;
+        DMRGK_CUDA(cudaFuncSetAttribute(pg::probe_loop_producer_warp, cudaFuncAttributeMaxDynamicSharedMemorySize, pg::K3_SMEM));
+        pg::probe_loop_producer_warp<<<ctx->n_sm * 2, 160, pg::K3_SMEM, st>>>(buf_dev, span_tiles, ktiles, sink_dev);
     } else {
-        return fail(DMRGK_EINVAL, "probe_gemm_loop: kind must be 0, 1 or 2");
+        return fail(DMRGK_EINVAL, "probe_gemm_loop: kind must be 0 … 5");
     }
     count_launch();
     DMRGK_CUDA(cudaGetLastError());
-    if (flops) *flops = double(grid) * double(ktiles) * 2.0 * bm * 64 * 16;
+    if (flops) *flops = double(ctx->n_sm) * ctas * double(ktiles) * 2.0 * bm * 64 * 16;
     return DMRGK_OK;
 }

@@ -96,6 +96,7 @@ SIGNATURES = {
     "dmrgk_davidson_step": (_i32, [_p, _pf64, _pf64, _pi32]),
     "dmrgk_davidson_solve": (_i32, [_p, _pf64, _pf64, _p, _pi32]),
     "dmrgk_davidson_query": (_i32, [_p, _pi32, _pi32]),
+    "dmrgk_davidson_set_allreduce": (_i32, [_p, _p, _p]),
     "dmrgk_op_fill_normal": (_i32, [_p, _p, _u64, _u64, _i32, _i32, _p]),
     "dmrgk_layout_fill_normal": (_i32, [_p, _p, _u64, _u64, _p]),
     "dmrgk_probe_fp64": (_i32, [_p, _i32, _i64, _p, _pf64, _p]),
@@ -454,6 +455,16 @@ class Davidson:
         m, na = C.c_int32(), C.c_int32()
         check(self.lib.dmrgk_davidson_query(self.h, C.byref(m), C.byref(na)))
         return m.value, na.value
+
+    def set_allreduce(self, fn):
+        """fn(device pointer, n doubles) -> 0: called after every apply of the driver (k-sharding hook)."""
+        if fn is None:
+            self._reduce_cb = None
+            check(self.lib.dmrgk_davidson_set_allreduce(self.h, None, None))
+            return
+        proto = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)
+        self._reduce_cb = proto(lambda ptr, n, stream, user: int(fn(int(ptr), int(n))))
+        check(self.lib.dmrgk_davidson_set_allreduce(self.h, C.cast(self._reduce_cb, C.c_void_p), None))
 
     def __del__(self):
         if getattr(self, "h", None):

@@ -85,7 +85,7 @@ class DeviceProblem:
             self.ops[i].bind_pinned(t)
             self.pinned_arenas.append(t)
             out[i] = t
-        self.pinned_views = dict(getattr(self, "pinned_views", {}), **out)
+        self.pinned_views.update(out)
         return out
 
     def set_op_host(self, i, blocks):
@@ -159,10 +159,13 @@ class DeviceProblem:
         self.heff.diag(out, self.workspace, self.stream, self.copy_stream)
         return out
 
-    def davidson(self, m_max=16, tol=1e-9, max_iter=500):
-        """Allocates the basis, the diagonal and the extended workspace; returns a dmrgk.Davidson."""
+    def davidson(self, m_max=16, tol=1e-9, max_iter=500, diag_hook=None):
+        """Allocates the basis, the diagonal and the extended workspace; returns a dmrgk.Davidson.
+        ``diag_hook`` (k-sharding): applied to the diagonal of this rank's share (the all-reduce)."""
         n = self.layout.n_padded
         self.diag_vec = self.diag()
+        if diag_hook is not None:
+            diag_hook(self.diag_vec)
         self.V = torch.empty(m_max * n, dtype=torch.float64, device=self.device)
         self.W = torch.empty(m_max * n, dtype=torch.float64, device=self.device)
         wb = (self.heff.workspace_bytes + 127) // 128 * 128
@@ -175,7 +178,7 @@ def from_workload(wl, device=0, pinned=(), ctx=None, **opts):
     """A seeded ``workloads.Workload`` on the device: operators filled by the library's fill kernel
     with the same counter-based stream ids as ``workloads.fill_op_host``."""
     import time
-    from workloads import op_stream_id   # input recipe only (no arithmetic of the method)
+    from workloads import op_stream_of   # input recipe only (no arithmetic of the method)
     t0 = time.perf_counter()
     dp = DeviceProblem(wl.n_charges, wl.sectors_A, wl.sectors_B, wl.target, device, ctx)
     dp.create_ops([(s.half, s.dq, s.parity) for s in wl.ops])
@@ -188,10 +191,10 @@ def from_workload(wl, device=0, pinned=(), ctx=None, **opts):
         if i in pinned:
             if dp.ops[i].n_padded:
                 tmp = torch.empty(dp.ops[i].n_padded, dtype=torch.float64, device=dp.device)
-                dp.fill_op(i, wl.seed, op_stream_id(i), mode, s.symmetric, arena=tmp)
+                dp.fill_op(i, wl.seed, op_stream_of(wl, i), mode, s.symmetric, arena=tmp)
                 staged[i][:dp.ops[i].n_padded].copy_(tmp)
         else:
-            dp.fill_op(i, wl.seed, op_stream_id(i), mode, s.symmetric)
+            dp.fill_op(i, wl.seed, op_stream_of(wl, i), mode, s.symmetric)
     torch.cuda.synchronize(dp.device)
     t2 = time.perf_counter()
     dp.build([(t.L, t.R, t.coef, t.trans_L, t.trans_R) for t in wl.terms], **opts)

@@ -31,6 +31,12 @@ def op_stream_id(op_index):
     return OP_STREAM0 + op_index
 
 
+def op_stream_of(wl, op_index):
+    """RNG stream of stored operator ``op_index`` of ``wl`` (its own if pinned by sub_workload)."""
+    s = wl.ops[op_index].stream
+    return s if s >= 0 else op_stream_id(op_index)
+
+
 @dataclass
 class OpSpec:
     half: str            # "A" or "B"
@@ -39,6 +45,8 @@ class OpSpec:
     symmetric: bool = False   # dq == 0 and every diagonal block symmetrised
     scale_mode: str = "rsqrt_cols"   # "one" (config 2) or "rsqrt_cols" (configs 3-5)
     tag: str = ""
+    stream: int = -1     # RNG stream of the values; −1 = op_stream_id(position in wl.ops).  Set when an
+                         # operator keeps its values while moving to another position (sub_workload)
 
 
 @dataclass
@@ -132,7 +140,7 @@ def fill_op_host(wl, op_index, only_blocks=None):
     """
     spec = wl.ops[op_index]
     sectors = wl.sectors(spec.half)
-    stream = op_stream_id(op_index)
+    stream = op_stream_of(wl, op_index)
     out = {}
     for (ri, ci, rows, cols, off) in op_block_table(sectors, spec.dq):
         if only_blocks is not None and (ri, ci) not in only_blocks:
@@ -344,6 +352,29 @@ def config5():
 def config5_staged_ops(wl):
     """Every 7th stored operator streams from pinned host memory (≈ 14 % of the bytes)."""
     return [i for i in range(len(wl.ops)) if i % 7 == 3]
+
+
+def sub_workload(wl, term_ids, name=None):
+    """The workload restricted to the operator pairs ``term_ids`` (a shard of the k list):
+    same sectors and target, only the stored operators those pairs touch, re-indexed, each keeping the
+    RNG stream it has in ``wl`` so that its values are unchanged.  Σ over a partition of the pair list
+    of the shards' σ equals the σ of ``wl`` (k-additivity)."""
+    import copy
+    term_ids = list(term_ids)
+    used = sorted({i for k in term_ids for i in (wl.terms[k].L, wl.terms[k].R) if i is not None})
+    new_index = {old: new for new, old in enumerate(used)}
+    sub = Workload(name or f"{wl.name}_sub{len(term_ids)}", wl.seed, wl.n_charges, list(wl.sectors_A),
+                   list(wl.sectors_B), tuple(wl.target), hermitian=False)
+    for old in used:
+        spec = copy.copy(wl.ops[old])
+        spec.stream = op_stream_of(wl, old)
+        sub.ops.append(spec)
+    for k in term_ids:
+        t = copy.copy(wl.terms[k])
+        t.L = None if t.L is None else new_index[t.L]
+        t.R = None if t.R is None else new_index[t.R]
+        sub.terms.append(t)
+    return sub
 
 
 # ----------------------------------------------------------------------------
