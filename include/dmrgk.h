@@ -22,13 +22,19 @@
  *  - Streams are cudaStream_t passed as void* (NULL = legacy default stream).
  *  - ASYNCHRONY: heff_apply, heff_diag and the vec_* calls enqueue work and return; the
  *    davidson_* calls and *_host calls synchronise the stream (they read scalars back).
- *  - LAYOUT: a block (rows × cols) is row-major with leading dimension ld = round_up(cols, 16)
- *    doubles; the padding columns must be zero (pack/fill write zeros; every kernel of the library
- *    preserves zeros there).  A block-sparse object is one packed arena plus a block table; block
- *    offsets (in doubles) are multiples of 16.  ψ, σ, diag(H_eff) and all Davidson vectors share the
- *    layout of dmrgk_layout, so vector kernels run over the flat padded arena.
- *    The "unpadded" form used by pack/unpack and by the seeded fill is: block after block in table
- *    order, each block rows×cols row-major with no padding.
+ *  - LAYOUT ("panel layout"): a block (rows × cols) occupies rows_pad·ld doubles with
+ *    ld = round_up(cols, 16), rows_pad = round_up(rows, 4).  It is stored as ld/16 column PANELS one
+ *    after the other; a panel holds rows_pad rows of 16 doubles (128 bytes each), and inside a row the
+ *    four 32-byte groups are XOR-swizzled with the row index: element (r, c) sits at
+ *        ((c / 16)·rows_pad + r)·16 + ((c mod 16) xor ((r mod 4)·4))          doubles from the block origin,
+ *    so a (rows ≤ 64) × 16-column operand tile is ONE contiguous chunk for a bulk copy and its
+ *    shared-memory image is read without bank conflicts.  Padding rows and columns must be zero
+ *    (pack/fill write zeros; every kernel of the library preserves zeros there).  A block-sparse object
+ *    is one packed arena plus a block table; block offsets (in doubles) are multiples of 64.  ψ, σ,
+ *    diag(H_eff) and all Davidson vectors share the layout of dmrgk_layout, so vector kernels run over
+ *    the flat padded arena.  Callers never index the packed form themselves: *_pack / *_unpack and
+ *    dmrgk_block_unpack translate to and from the "unpadded" form — block after block in table order,
+ *    each block rows×cols row-major with no padding — which is also what the seeded fill indexes.
  */
 #ifndef DMRGK_H
 #define DMRGK_H
@@ -91,7 +97,7 @@ void dmrgk_layout_destroy(dmrgk_layout* l);
 int32_t dmrgk_layout_query(const dmrgk_layout* l, int64_t* n_blocks, int64_t* n_elems,
                            int64_t* n_padded);
 /* Block table; each output array has n_blocks entries (any may be NULL).  offset is in doubles
- * into the packed arena. */
+ * into the packed arena; block i occupies dmrgk_block_size(rows[i], cols[i]) doubles from there. */
 int32_t dmrgk_layout_blocks(const dmrgk_layout* l, int32_t* a_idx, int32_t* b_idx, int32_t* rows,
                             int32_t* cols, int32_t* ld, int64_t* offset);
 /* Host-side test aids: unpadded ↔ packed (host pointers; pack zero-fills the padding). */
@@ -107,6 +113,13 @@ int32_t dmrgk_op_query(const dmrgk_op* op, int64_t* n_blocks, int64_t* n_elems, 
 int32_t dmrgk_op_blocks(const dmrgk_op* op, int32_t* row_idx, int32_t* col_idx, int32_t* rows,
                         int32_t* cols, int32_t* ld, int64_t* offset);
 int32_t dmrgk_op_pack(const dmrgk_op* op, const double* unpadded_host, double* packed_host);
+int32_t dmrgk_op_unpack(const dmrgk_op* op, const double* packed_host, double* unpadded_host);
+/* One block in isolation (host test aids; no handle needed): the number of doubles a rows×cols block
+ * occupies, its dense row-major form from its packed form, and whether all its padding is zero
+ * (returns 0 if so, 1 if not). */
+int64_t dmrgk_block_size(int32_t rows, int32_t cols);
+int32_t dmrgk_block_unpack(int32_t rows, int32_t cols, const double* packed_host, double* dense_host);
+int32_t dmrgk_block_padding_is_zero(int32_t rows, int32_t cols, const double* packed_host);
 /* Resident operator: packed arena in device memory (n_padded doubles, 128-B aligned). */
 int32_t dmrgk_op_bind_device(dmrgk_op* op, const double* arena_dev);
 /* Staged operator ("H2D IO"): packed arena in PINNED host memory;
@@ -244,7 +257,7 @@ int32_t dmrgk_davidson_set_allreduce(dmrgk_davidson* d, dmrgk_allreduce_fn fn, v
 /* Φ: the kept basis of one half, a charge-block-diagonal map from the NEW space (kept states) into
  * the ENLARGED space: one block (dim_enl(q) × dim_new(q)) for every enlarged sector (in enlarged
  * order) whose charge is also a sector of the new space, both dims > 0.  Same packed layout rules as
- * operators (ld = round_up(cols, 16), zero padding, offsets multiples of 16 doubles). */
+ * operators (panel layout, zero padding). */
 typedef struct dmrgk_iso dmrgk_iso;
 int32_t dmrgk_iso_create(dmrgk_ctx* ctx, const dmrgk_space* enlarged, const dmrgk_space* kept,
                          dmrgk_iso** out);

@@ -33,12 +33,16 @@ __global__ void fill_normal_kernel(const DevBlock* __restrict__ table, double* _
                                    unsigned long long base, int scale_mode, int symmetric) {
     const DevBlock b = table[blockIdx.y];
     const double scale = scale_mode == 1 ? 1.0 / sqrt((double)b.cols) : scale_mode == 2 ? 1.0 / sqrt((double)b.rows) : 1.0;
-    const long long total = (long long)b.rows * b.ld;
+    const long long total = (long long)b.rows_pad * b.ld;      // every stored double, padding included
+    const long long panel = (long long)b.rows_pad * 16;
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
          e += (long long)gridDim.x * blockDim.x) {
-        const int r = int(e / b.ld), c = int(e % b.ld);
+        // inverse of panel_off: storage position e → element (r, c)
+        const int p = int(e / panel), rem = int(e % panel);
+        const int r = rem >> 4, pos = rem & 15;
+        const int c = p * 16 + (pos ^ ((r & 3) << 2));
         double v = 0.0;
-        if (c < b.cols) {
+        if (r < b.rows && c < b.cols) {
             double gv = normal12(base, (unsigned long long)(b.uoff + (long long)r * b.cols + c));
             if (symmetric && b.square_diag) {
                 const double gt = normal12(base, (unsigned long long)(b.uoff + (long long)c * b.cols + r));
@@ -59,7 +63,7 @@ static int32_t fill(const DevBlock* table, const std::vector<Block>& blocks, dou
     for (size_t b0 = 0; b0 < blocks.size(); b0 += 65535) {
         const unsigned nb = unsigned(std::min<size_t>(65535, blocks.size() - b0));
         int64_t biggest = 0;
-        for (size_t i = b0; i < b0 + nb; ++i) biggest = std::max<int64_t>(biggest, int64_t(blocks[i].rows) * blocks[i].ld);
+        for (size_t i = b0; i < b0 + nb; ++i) biggest = std::max<int64_t>(biggest, blocks[i].size());
         const unsigned gx = unsigned(std::max<int64_t>(1, std::min<int64_t>(1024, (biggest + 255) / 256)));
         fill_normal_kernel<<<dim3(gx, nb), 256, 0, st>>>(table + b0, arena, base, scale_mode, symmetric);
         count_launch();

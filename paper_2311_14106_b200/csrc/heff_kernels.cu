@@ -6,38 +6,56 @@
 // list of segments (phase 1: one segment, T_k = c_k s · L_k ψ; phase 2: every task of the output
 // block, σ += [T_1 … T_n]·[R_1 … R_n]ᵀ — the stacked-k form, so accumulators never leave registers
 // between tasks).  FP64 tensor cores on sm_100a are reached through mma.sync.m8n8k4.f64 (SASS
-// DMMA.8x8x4; tcgen05.mma has no f64 kind), so accumulators live in registers, operands are staged
-// global→shared by cp.async in a multi-stage ring that runs across segment boundaries, and every
-// fragment load is one conflict-free LDS.64 per lane (padded tile strides, see smem layout below).
+// DMMA.8x8x4; tcgen05.mma has no f64 kind), so accumulators live in registers.
+//
+// Staging (round 2): operand tiles are fetched by the TMA unit.  Every block is stored in the panel
+// layout (internal.h), in which a ≤64×16 K-major tile — and each 16×16 piece of an MN-major one — is
+// one contiguous chunk, already swizzled; ONE elected thread per k-tile issues 1–8 cp.async.bulk
+// copies (SASS UBLKCP) that complete on the stage's `full` mbarrier, the four compute warps wait on
+// it, run LDS.64 + DMMA only, and release the stage through its `empty` mbarrier.  There is no
+// __syncthreads and no per-thread address arithmetic in the k-loop.  The producer role rotates over
+// the warps (tile t is fetched by lane 0 of warp t mod 4).  2 CTAs per SM: with the warps decoupled
+// by mbarriers the DMMA pipe runs fastest at two resident warps per scheduler (profiles/r2_tma_summary.md).
 #include "internal.h"
 
 namespace dmrgk {
 
 constexpr int BM = TILE_M, BN = TILE_N, BK = TILE_K;
 constexpr int NTHREADS = 128;           // 4 warps as 2×2, each a 32×32 warp tile = 4×4 DMMA frags
-constexpr int STAGES = 3;
-constexpr int NCOPY = BK / 4;            // 16-byte copies per thread per operand per stage
-constexpr int KM_CPR = BK / 2;           // 16-byte chunks per row of a K-major tile
-constexpr int KM_RPP = NTHREADS / KM_CPR;  // rows covered by one pass of the CTA
-// Shared tile layouts (doubles).  K-major operand tile: [64 rows][BK] with row stride 20
-// (20·2 words ≡ 8 mod 32 → the 4 rows × 4 k of a half-warp LDS.64 hit 16 distinct bank pairs).
-// MN-major operand tile: [BK rows][64] with row stride 68 (68·2 ≡ 8 mod 32, same argument with
-// the roles of row and k exchanged).
-constexpr int KM_STRIDE = BK + 4;       // 20
-constexpr int MN_STRIDE = BM + 4;       // 68
-constexpr int OPER_DOUBLES = (BM * KM_STRIDE > BK * MN_STRIDE) ? BM * KM_STRIDE : BK * MN_STRIDE;  // 1280
+constexpr int STAGES = 6;
+constexpr int MIN_CTAS = 2;
+constexpr int OPER_DOUBLES = BM * BK;    // 1024: one operand tile, dense 128-byte rows
 constexpr int STAGE_DOUBLES = 2 * OPER_DOUBLES;
-constexpr int SMEM_BYTES = STAGES * STAGE_DOUBLES * 8;   // 61440 → 3 CTAs per SM
+constexpr int SMEM_BYTES = STAGES * STAGE_DOUBLES * 8;   // 98304 → 2 CTAs per SM
 
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool pred) {
-    unsigned s = static_cast<unsigned>(__cvta_generic_to_shared(smem));
-    int n = pred ? 16 : 0;   // src-size 0 → 16 bytes of zeros
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(n));
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+// TMA bulk copy global → shared, completing `bytes` on the mbarrier (bytes a multiple of 16)
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
 }
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -45,81 +63,44 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                  : "d"(a), "d"(b));
 }
 
-// ---- loader ------------------------------------------------------------------------------------
-// Per-thread copy plan of one operand for the current segment: every stage this thread issues four
-// 16-byte cp.async; everything that does not change from k-tile to k-tile is computed once per segment
-// so the per-stage cost is a pointer bump and four predicated copies.
-struct OpPlan {
-    const char* ptr;      // source of copy j = 0 for the next k-tile (bytes)
-    const char* safe;     // a valid address for predicated-off copies (block origin)
-    long long step_j;     // source distance between copies j and j+1 (bytes)
-    long long step_k;     // source advance per k-tile (bytes)
-    uint32_t dst;         // destination of copy j = 0 inside the operand tile (bytes)
-    uint32_t dst_step;    // destination distance between copies (bytes)
-    int32_t mask;         // bit j: copy j is inside the operand along the M/N direction
-    int32_t krow;         // MN-major: k-row of copy 0 (copy j is krow + 4j); K-major: −64 (never cut by klen)
-};
-
-// Operand tile origin `o0` (row/column offset of the tile in the block), `ext` = block extent in that
-// direction (rows for K-major predication; ld for MN-major), `mn_major` = the tile is stored [k][i].
-__device__ __forceinline__ void make_plan(OpPlan& p, const char* base, int ld, bool mn_major, int o0, int ext,
-                                          int tid) {
-    p.safe = base;
-    if (!mn_major) {
-        const int row = tid / KM_CPR, ch = tid % KM_CPR;   // copies j: rows row + KM_RPP·j, chunk ch
-        p.ptr = base + (int64_t(o0 + row) * ld + ch * 2) * 8;
-        p.step_j = int64_t(KM_RPP) * ld * 8;
-        p.step_k = BK * 8;
-        p.dst = (row * KM_STRIDE + ch * 2) * 8;
-        p.dst_step = KM_RPP * KM_STRIDE * 8;
-        int m = 0;
-#pragma unroll
-        for (int j = 0; j < NCOPY; ++j) m |= ((o0 + row + KM_RPP * j) < ext) << j;
-        p.mask = m;
-        p.krow = -64;
-    } else {
-        const int row = tid >> 5, ch = tid & 31;           // copies j: k-rows row + 4 j, chunk ch
-        p.ptr = base + (int64_t(row) * ld + o0 + ch * 2) * 8;
-        p.step_j = int64_t(4) * ld * 8;
-        p.step_k = int64_t(BK) * ld * 8;
-        p.dst = (row * MN_STRIDE + ch * 2) * 8;
-        p.dst_step = 4 * MN_STRIDE * 8;
-        p.mask = (o0 + ch * 2) < ext ? ((1 << NCOPY) - 1) : 0;
-        p.krow = row;
-    }
-}
-
-// Issue the four copies of one operand for a k-tile with `rem` contraction elements left (≥ 1).
-__device__ __forceinline__ void issue_plan(OpPlan& p, uint32_t smem_operand, int rem) {
-#pragma unroll
-    for (int j = 0; j < NCOPY; ++j) {
-        const bool ok = ((p.mask >> j) & 1) && (p.krow + 4 * j) < rem;
-        const char* src = ok ? p.ptr + j * p.step_j : p.safe;
-        const int n = ok ? 16 : 0;   // src-size 0 → 16 bytes of zeros
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_operand + p.dst + j * p.dst_step),
-                     "l"(src), "r"(n));
-    }
-    p.ptr += p.step_k;
-}
-
 // ---- consumer ----------------------------------------------------------------------------------
+// Shared image of an operand tile (doubles from the operand's origin in the stage):
+//   K-major  (stored [i][k]): element (i, k) at i·16 + (k xor ((i & 3) << 2))        [64 rows × 16]
+//   MN-major (stored [k][i]): element (i, k) at (i >> 4)·256 + k·16 + ((i & 15) xor ((k & 3) << 2))
+//                                                                    [4 panels × 16 k-rows × 16]
+// A lane (g = lane >> 2, t4 = lane & 3) of fragment f reads row i = w·32 + f·8 + g at k = 4·ks + t4:
+//   K-major : k0 + f·128 + ((ks xor (g & 3)) << 2)           with k0 = (w·32 + g)·16 + t4
+//   MN-major: m[f & 1] + (f >> 1)·256 + ks·64                with m[h] = w·512 + t4·16 + ((8h + g) xor (t4 << 2))
+// In both cases the 16 lanes of a half-warp hit 16 distinct 8-byte banks.
+struct FragBase {
+    int k0, m0, m1;
+};
+__device__ __forceinline__ FragBase make_frag_base(int origin, int w, int g, int t4) {
+    FragBase b;
+    b.k0 = origin + (w * 32 + g) * 16 + t4;
+    b.m0 = origin + w * 512 + t4 * 16 + (g ^ (t4 << 2));
+    b.m1 = origin + w * 512 + t4 * 16 + ((8 + g) ^ (t4 << 2));
+    return b;
+}
+template <bool MN>
+__device__ __forceinline__ double frag(const double* __restrict__ st, const FragBase& b, int g3, int f, int ks) {
+    if (MN) return st[((f & 1) ? b.m1 : b.m0) + (f >> 1) * 256 + ks * 64];
+    return st[b.k0 + f * 128 + ((ks ^ g3) << 2)];
+}
+
 // One k-tile (BK = 16, `nks` steps of 4) of a warp tile of FM × FN fragments.  FM, FN and the operand
-// layouts are compile-time: accumulator indices are static, no DMMA carries a guard, and every LDS.64
-// has an immediate offset.  Element (i, k) of A sits at i·20 + k (K-major) or k·68 + i (M-major);
-// the same for B with j.
+// layouts are compile-time: accumulator indices are static and no DMMA carries a guard.
 template <int FM, int FN, bool AM, bool BN_, bool FULLK>
-__device__ __forceinline__ void mma_ktile(const double* __restrict__ pa, const double* __restrict__ pb, int nks,
-                                          double (&acc)[4][4][2]) {
-    constexpr int a_fs = 8 * (AM ? 1 : KM_STRIDE), a_ks4 = 4 * (AM ? MN_STRIDE : 1);
-    constexpr int b_fs = 8 * (BN_ ? 1 : KM_STRIDE), b_ks4 = 4 * (BN_ ? MN_STRIDE : 1);
+__device__ __forceinline__ void mma_ktile(const double* __restrict__ st, const FragBase& fa, const FragBase& fb, int g3,
+                                          int nks, double (&acc)[4][4][2]) {
     if (FULLK) {
 #pragma unroll
         for (int ks = 0; ks < BK / 4; ++ks) {
             double af[FM], bf[FN];
 #pragma unroll
-            for (int f = 0; f < FM; ++f) af[f] = pa[f * a_fs + ks * a_ks4];
+            for (int f = 0; f < FM; ++f) af[f] = frag<AM>(st, fa, g3, f, ks);
 #pragma unroll
-            for (int f = 0; f < FN; ++f) bf[f] = pb[f * b_fs + ks * b_ks4];
+            for (int f = 0; f < FN; ++f) bf[f] = frag<BN_>(st, fb, g3, f, ks);
 #pragma unroll
             for (int i = 0; i < FM; ++i)
 #pragma unroll
@@ -130,70 +111,79 @@ __device__ __forceinline__ void mma_ktile(const double* __restrict__ pa, const d
         for (int ks = 0; ks < nks; ++ks) {
             double af[FM], bf[FN];
 #pragma unroll
-            for (int f = 0; f < FM; ++f) af[f] = pa[f * a_fs];
+            for (int f = 0; f < FM; ++f) af[f] = frag<AM>(st, fa, g3, f, ks);
 #pragma unroll
-            for (int f = 0; f < FN; ++f) bf[f] = pb[f * b_fs];
+            for (int f = 0; f < FN; ++f) bf[f] = frag<BN_>(st, fb, g3, f, ks);
 #pragma unroll
             for (int i = 0; i < FM; ++i)
 #pragma unroll
                 for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
-            pa += a_ks4;
-            pb += b_ks4;
         }
     }
 }
 
 template <int FM, bool AM, bool BN_>
-__device__ __forceinline__ void mma_ktile_n(int nfn, const double* pa, const double* pb, int nks,
-                                            double (&acc)[4][4][2]) {
+__device__ __forceinline__ void mma_ktile_n(int nfn, const double* st, const FragBase& fa, const FragBase& fb, int g3,
+                                            int nks, double (&acc)[4][4][2]) {
     switch (nfn) {
-        case 1: mma_ktile<FM, 1, AM, BN_, false>(pa, pb, nks, acc); break;
-        case 2: mma_ktile<FM, 2, AM, BN_, false>(pa, pb, nks, acc); break;
-        case 3: mma_ktile<FM, 3, AM, BN_, false>(pa, pb, nks, acc); break;
-        default: mma_ktile<FM, 4, AM, BN_, false>(pa, pb, nks, acc); break;
+        case 1: mma_ktile<FM, 1, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
+        case 2: mma_ktile<FM, 2, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
+        case 3: mma_ktile<FM, 3, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
+        default: mma_ktile<FM, 4, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
     }
 }
 
 // All fragment shapes of one operand-layout combination; branches are warp-uniform.
 template <bool AM, bool BN_>
-__device__ __forceinline__ void mma_layout(int nfm, int nfn, int nks, const double* sA, const double* sB, int wm,
-                                           int wn, int g, int t4, double (&acc)[4][4][2]) {
-    const double* pa = sA + (wm * 32 + g) * (AM ? 1 : KM_STRIDE) + t4 * (AM ? MN_STRIDE : 1);
-    const double* pb = sB + (wn * 32 + g) * (BN_ ? 1 : KM_STRIDE) + t4 * (BN_ ? MN_STRIDE : 1);
+__device__ __forceinline__ void mma_layout(int nfm, int nfn, int nks, const double* st, const FragBase& fa,
+                                           const FragBase& fb, int g3, double (&acc)[4][4][2]) {
     if (nfm == 4 && nfn == 4 && nks == BK / 4) {
-        mma_ktile<4, 4, AM, BN_, true>(pa, pb, BK / 4, acc);
+        mma_ktile<4, 4, AM, BN_, true>(st, fa, fb, g3, BK / 4, acc);
     } else {
         switch (nfm) {
-            case 1: mma_ktile_n<1, AM, BN_>(nfn, pa, pb, nks, acc); break;
-            case 2: mma_ktile_n<2, AM, BN_>(nfn, pa, pb, nks, acc); break;
-            case 3: mma_ktile_n<3, AM, BN_>(nfn, pa, pb, nks, acc); break;
-            default: mma_ktile_n<4, AM, BN_>(nfn, pa, pb, nks, acc); break;
+            case 1: mma_ktile_n<1, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+            case 2: mma_ktile_n<2, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+            case 3: mma_ktile_n<3, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+            default: mma_ktile_n<4, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
         }
     }
 }
 
-// Per-stage note left by the loader for the consumers (read after the barrier that publishes the stage).
+// Per-stage note left by the producer for the consumers (published by the stage's full barrier).
 struct StageNote {
     uint32_t flags;   // segment flags (operand majors)
     int32_t nks;      // k-steps of 4 that hold data in this k-tile (1..4)
 };
 
-__global__ void __launch_bounds__(NTHREADS, 3)
+__global__ void __launch_bounds__(NTHREADS, MIN_CTAS)
 heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ segs, Bases bases) {
-    extern __shared__ __align__(16) double smem[];
+    extern __shared__ __align__(128) double smem[];
+    __shared__ __align__(8) unsigned long long bars[2 * STAGES];   // full[0..S), empty[S..2S)
     __shared__ StageNote notes[STAGES];
     const Unit u = units[blockIdx.x];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp >> 1, wn = warp & 1;
-    const int g = lane >> 2, t4 = lane & 3;
-    const uint32_t smem_base = static_cast<uint32_t>(__cvta_generic_to_shared(smem));
+    const int g = lane >> 2, t4 = lane & 3, g3 = g & 3;
+    const uint32_t smem_base = smem_u32(smem), bar0 = smem_u32(bars);
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(bar0 + s * 8, 1);                   // full: the producer's arrive (+ the copies' bytes)
+            mbar_init(bar0 + (STAGES + s) * 8, 4);        // empty: one arrive per warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
 
     // rows / columns of this tile that hold data, in 8-wide fragments, for this warp
     const int rows_t = min(BM, u.mrows - u.i0);
     const int cols_t = min(BN, u.ncols_st - u.j0);
+    const int cols_b = min(BN, u.ncols - u.j0);          // B-operand columns that exist
     const int nfm = max(0, min(4, (rows_t - wm * 32 + 7) >> 3));
-    const int nfn = max(0, min(4, (min(BN, u.ncols - u.j0) - wn * 32 + 7) >> 3));
+    const int nfn = max(0, min(4, (cols_b - wn * 32 + 7) >> 3));
     const bool busy = nfm > 0 && nfn > 0;
+    const FragBase fa = make_frag_base(0, wm, g, t4), fb = make_frag_base(OPER_DOUBLES, wn, g, t4);
 
     double acc[4][4][2];
 #pragma unroll
@@ -201,91 +191,123 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    // loader state: segment cursor, remaining contraction length of the segment, the two copy plans
-    int ld_seg = u.seg_begin, ld_rem = 0;
-    uint32_t ld_flags = 0;
-    OpPlan planA, planB;
+    // ---- producer cursor (kept by every thread, uniform): the segment and k-offset of the next tile ----
+    int p_seg = u.seg_begin, p_k0 = 0;
+    struct {
+        unsigned long long A, B;
+        int a_rp, b_rp, klen;
+        uint32_t flags;
+    } p_sg = {0ull, 0ull, 0, 0, 0, 0u};
     auto open_segment = [&]() {
-        while (ld_seg < u.seg_end) {
-            const Seg sg = segs[ld_seg];
-            if (sg.klen > 0) {
-                ld_rem = sg.klen;
-                ld_flags = sg.flags;
-                const char* A = reinterpret_cast<const char*>(bases.b[(sg.flags >> SEG_A_SEL_SHIFT) & 3u] + sg.A);
-                const char* B = reinterpret_cast<const char*>(bases.b[(sg.flags >> SEG_B_SEL_SHIFT) & 3u] + sg.B);
-                const bool am = (sg.flags & SEG_A_MMAJOR) != 0, bn = (sg.flags & SEG_B_NMAJOR) != 0;
-                make_plan(planA, A, sg.lda, am, u.i0, am ? sg.lda : u.mrows, tid);
-                make_plan(planB, B, sg.ldb, bn, u.j0, bn ? sg.ldb : u.ncols, tid);
+        while (p_seg < u.seg_end) {
+            const int4 lo = __ldg(reinterpret_cast<const int4*>(segs + p_seg));          // A, B
+            const int4 hi = __ldg(reinterpret_cast<const int4*>(segs + p_seg) + 1);      // a_rp, b_rp, klen, flags
+            if (hi.z > 0) {
+                p_sg.A = (unsigned long long)(unsigned)lo.x | ((unsigned long long)(unsigned)lo.y << 32);
+                p_sg.B = (unsigned long long)(unsigned)lo.z | ((unsigned long long)(unsigned)lo.w << 32);
+                p_sg.a_rp = hi.x;
+                p_sg.b_rp = hi.y;
+                p_sg.klen = hi.z;
+                p_sg.flags = uint32_t(hi.w);
+                p_k0 = 0;
                 return;
             }
-            ++ld_seg;
+            ++p_seg;
         }
     };
     open_segment();
     const int total = u.nkt;
-
-    auto load_next = [&](int stage) {
-        const uint32_t sA = smem_base + stage * (STAGE_DOUBLES * 8);
-        issue_plan(planA, sA, ld_rem);
-        issue_plan(planB, sA + OPER_DOUBLES * 8, ld_rem);
-        if (tid == 0) {
-            notes[stage].flags = ld_flags;
-            notes[stage].nks = min(BK / 4, (ld_rem + 3) >> 2);
+    const int rows_a = rows_t;                            // A-operand rows that exist in this tile
+    // Fetch tile `t` (the cursor's tile) into its stage; `wait_parity` < 0: the stage has never been used.
+    auto produce = [&](int t, int stage, int wait_parity) {
+        if (lane == 0 && warp == (t & 3)) {
+            const uint32_t full = bar0 + stage * 8;
+            if (wait_parity >= 0) mbar_wait(bar0 + (STAGES + stage) * 8, uint32_t(wait_parity));
+            const int nk = min(BK, p_sg.klen - p_k0), nk4 = (nk + 3) & ~3;
+            const bool am = (p_sg.flags & SEG_A_MMAJOR) != 0, bn = (p_sg.flags & SEG_B_NMAJOR) != 0;
+            const char* A = reinterpret_cast<const char*>(bases.b[(p_sg.flags >> SEG_A_SEL_SHIFT) & 3u] + p_sg.A);
+            const char* B = reinterpret_cast<const char*>(bases.b[(p_sg.flags >> SEG_B_SEL_SHIFT) & 3u] + p_sg.B);
+            const int npa = (rows_a + 15) >> 4, npb = (cols_b + 15) >> 4;
+            const uint32_t bytes_a = am ? uint32_t(npa * nk4 * 128) : uint32_t(rows_a * 128);
+            const uint32_t bytes_b = bn ? uint32_t(npb * nk4 * 128) : uint32_t(cols_b * 128);
+            notes[stage].flags = p_sg.flags;
+            notes[stage].nks = nk4 >> 2;
+            mbar_expect_tx(full, bytes_a + bytes_b);
+            const uint32_t dA = smem_base + stage * (STAGE_DOUBLES * 8), dB = dA + OPER_DOUBLES * 8;
+            if (!am) {
+                bulk_g2s(dA, A + (int64_t(p_k0 >> 4) * p_sg.a_rp + u.i0) * 128, bytes_a, full);
+            } else {
+                for (int pp = 0; pp < npa; ++pp)
+                    bulk_g2s(dA + pp * 2048, A + (int64_t((u.i0 >> 4) + pp) * p_sg.a_rp + p_k0) * 128, uint32_t(nk4 * 128), full);
+            }
+            if (!bn) {
+                bulk_g2s(dB, B + (int64_t(p_k0 >> 4) * p_sg.b_rp + u.j0) * 128, bytes_b, full);
+            } else {
+                for (int pp = 0; pp < npb; ++pp)
+                    bulk_g2s(dB + pp * 2048, B + (int64_t((u.j0 >> 4) + pp) * p_sg.b_rp + p_k0) * 128, uint32_t(nk4 * 128), full);
+            }
         }
-        ld_rem -= BK;
-        if (ld_rem <= 0) {
-            ++ld_seg;
+        // advance the cursor (all threads)
+        p_k0 += BK;
+        if (p_k0 >= p_sg.klen) {
+            ++p_seg;
             open_segment();
         }
     };
 
-    // prologue: STAGES−1 stages in flight
-#pragma unroll
-    for (int s = 0; s < STAGES - 1; ++s) {
-        if (s < total) load_next(s);
-        cp_async_commit();
-    }
+    // prologue: STAGES−1 tiles in flight
+#pragma unroll 1
+    for (int t = 0; t < STAGES - 1 && t < total; ++t) produce(t, t, -1);
 
-    int stage = 0;
+    int stage = 0, prev_stage = STAGES - 1;
+    uint32_t ph = 0, prev_ph = 0;
+#pragma unroll 1
     for (int it = 0; it < total; ++it) {
-        cp_async_wait<STAGES - 2>();
-        __syncthreads();
-        {
-            int ns = stage + STAGES - 1;
-            if (ns >= STAGES) ns -= STAGES;
-            if (it + STAGES - 1 < total) load_next(ns);
-            cp_async_commit();
-        }
+        // refill: tile it+STAGES−1 goes into the stage tile it−1 used; its consumers must be done
+        const int nt = it + STAGES - 1;
+        if (nt < total) produce(nt, prev_stage, it >= 1 ? int(prev_ph) : -1);
+        __syncwarp();
+        mbar_wait(bar0 + stage * 8, ph);
         if (busy) {
             const StageNote note = notes[stage];
-            const double* sA = smem + stage * STAGE_DOUBLES;
-            const double* sB = sA + OPER_DOUBLES;
+            const double* st = smem + stage * STAGE_DOUBLES;
             switch (note.flags & (SEG_A_MMAJOR | SEG_B_NMAJOR)) {
-                case 0: mma_layout<false, false>(nfm, nfn, note.nks, sA, sB, wm, wn, g, t4, acc); break;
-                case SEG_A_MMAJOR: mma_layout<true, false>(nfm, nfn, note.nks, sA, sB, wm, wn, g, t4, acc); break;
-                case SEG_B_NMAJOR: mma_layout<false, true>(nfm, nfn, note.nks, sA, sB, wm, wn, g, t4, acc); break;
-                default: mma_layout<true, true>(nfm, nfn, note.nks, sA, sB, wm, wn, g, t4, acc); break;
+                case 0: mma_layout<false, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                case SEG_A_MMAJOR: mma_layout<true, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                case SEG_B_NMAJOR: mma_layout<false, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                default: mma_layout<true, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
             }
         }
-        if (++stage == STAGES) stage = 0;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar0 + (STAGES + stage) * 8);
+        prev_stage = stage;
+        prev_ph = ph;
+        if (++stage == STAGES) {
+            stage = 0;
+            ph ^= 1u;
+        }
     }
-    cp_async_wait<0>();
 
     // epilogue: lane holds C[row g][cols 2·t4, 2·t4+1] of each 8×8 fragment
     double* C = reinterpret_cast<double*>(bases.b[(u.mode >> UNIT_C_SEL_SHIFT) & 3u] + u.C);
-    const bool accum = (u.mode & UNIT_ACCUM) != 0;
+    const bool accum = (u.mode & UNIT_ACCUM) != 0, plain = (u.mode & UNIT_C_PLAIN) != 0;
+    // a panel-layout C block also gets its padding rows (up to rows_pad) written with zeros, so that it
+    // can be read MN-major later (padding rows take part in the last k-step of 4)
+    const int rows_st = plain ? rows_t : min(BM, u.c_rp - u.i0);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int r = wm * 32 + i * 8 + g;
-        if (r >= rows_t) continue;
+        if (r >= rows_st) continue;
+        const bool live = r < rows_t;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int c = wn * 32 + j * 8 + 2 * t4;
             if (c >= cols_t) continue;
-            double2* p = reinterpret_cast<double2*>(C + int64_t(r) * u.ldc + c);
+            // (c, c+1) with c even stay adjacent under the 32-byte-group swizzle
+            double2* p = reinterpret_cast<double2*>(plain ? C + r * BN + c : C + panel_off(u.i0 + r, u.j0 + c, u.c_rp));
             double2 v;
-            v.x = (u.j0 + c < u.ncols) ? u.alpha * acc[i][j][0] : 0.0;
-            v.y = (u.j0 + c + 1 < u.ncols) ? u.alpha * acc[i][j][1] : 0.0;
+            v.x = (live && u.j0 + c < u.ncols) ? u.alpha * acc[i][j][0] : 0.0;
+            v.y = (live && u.j0 + c + 1 < u.ncols) ? u.alpha * acc[i][j][1] : 0.0;
             if (accum) {
                 double2 o = *p;
                 v.x += o.x;
@@ -296,32 +318,33 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
     }
 }
 
-// Scalar check kernel over the same work lists: one thread per 4×8 patch, plain FMA loops reading
-// global memory directly.  A debugging aid (dmrgk_heff_opts.kernel = 1), never the product path.
+// Scalar check kernel over the same work lists: one thread per output element, plain FMA loops reading
+// global memory directly through panel_off.  A debugging aid (dmrgk_heff_opts.kernel = 1), never the
+// product path.
 __global__ void __launch_bounds__(NTHREADS)
 heff_gemm_scalar_kernel(const Unit* __restrict__ units, const Seg* __restrict__ segs, Bases bases) {
     const Unit u = units[blockIdx.x];
-    const int rows_t = min(BM, u.mrows - u.i0);
+    const int rows_t = (u.mode & UNIT_C_PLAIN) ? min(BM, u.mrows - u.i0) : min(BM, u.c_rp - u.i0);   // incl. padding rows
     const int cols_t = min(BN, u.ncols_st - u.j0);
     double* C = reinterpret_cast<double*>(bases.b[(u.mode >> UNIT_C_SEL_SHIFT) & 3u] + u.C);
     for (int e = threadIdx.x; e < rows_t * cols_t; e += NTHREADS) {
         const int r = e / cols_t, c = e % cols_t;
         const int i = u.i0 + r, j = u.j0 + c;
         double s = 0.0;
-        if (j < u.ncols) {
+        if (i < u.mrows && j < u.ncols) {
             for (int sidx = u.seg_begin; sidx < u.seg_end; ++sidx) {
                 const Seg sg = segs[sidx];
                 const double* A = reinterpret_cast<const double*>(bases.b[(sg.flags >> SEG_A_SEL_SHIFT) & 3u] + sg.A);
                 const double* B = reinterpret_cast<const double*>(bases.b[(sg.flags >> SEG_B_SEL_SHIFT) & 3u] + sg.B);
                 for (int k = 0; k < sg.klen; ++k) {
-                    double a = (sg.flags & SEG_A_MMAJOR) ? A[int64_t(k) * sg.lda + i] : A[int64_t(i) * sg.lda + k];
-                    double b = (sg.flags & SEG_B_NMAJOR) ? B[int64_t(k) * sg.ldb + j] : B[int64_t(j) * sg.ldb + k];
+                    double a = (sg.flags & SEG_A_MMAJOR) ? A[panel_off(k, i, sg.a_rp)] : A[panel_off(i, k, sg.a_rp)];
+                    double b = (sg.flags & SEG_B_NMAJOR) ? B[panel_off(k, j, sg.b_rp)] : B[panel_off(j, k, sg.b_rp)];
                     s = fma(a, b, s);
                 }
             }
         }
         double v = u.alpha * s;
-        double* p = C + int64_t(r) * u.ldc + c;
+        double* p = (u.mode & UNIT_C_PLAIN) ? C + r * BN + c : C + panel_off(i, j, u.c_rp);
         if (u.mode & UNIT_ACCUM) v += *p;
         *p = v;
     }
@@ -337,7 +360,7 @@ heff_reduce_kernel(const RUnit* __restrict__ runits, Bases bases) {
     const int r = (blockIdx.x % RED_SLABS) * 8 + (threadIdx.x >> 5);
     const int c = (threadIdx.x & 31) * 2;
     if (r >= u.rows || c >= u.cols) return;   // cols is even (multiple of 16 or the tile width 64)
-    double2* p = reinterpret_cast<double2*>(reinterpret_cast<double*>(bases.b[BASE_SIGMA] + u.C) + int64_t(r) * u.ldc + c);
+    double2* p = reinterpret_cast<double2*>(reinterpret_cast<double*>(bases.b[BASE_SIGMA] + u.C) + panel_off(u.i0 + r, u.j0 + c, u.c_rp));
     const double2* P = reinterpret_cast<const double2*>(reinterpret_cast<const double*>(bases.b[BASE_WS] + u.P) + r * BN + c);
     double2 v = *p;
     int s = 0;
@@ -379,8 +402,8 @@ heff_diag_kernel(const DiagBlock* __restrict__ blocks, const DiagTask* __restric
                 const DiagTask tk = tasks[t0 + t];
                 const double* L = reinterpret_cast<const double*>(bases.b[tk.sel & 3u] + tk.L);
                 const double* R = reinterpret_cast<const double*>(bases.b[(tk.sel >> 2) & 3u] + tk.R);
-                sl[t][x] = (i0 + x < b.rows) ? tk.alpha * L[int64_t(i0 + x) * (tk.ldl + 1)] : 0.0;
-                sr[t][x] = (j0 + x < b.cols) ? R[int64_t(j0 + x) * (tk.ldr + 1)] : 0.0;
+                sl[t][x] = (i0 + x < b.rows) ? tk.alpha * L[panel_off(i0 + x, i0 + x, tk.l_rp)] : 0.0;
+                sr[t][x] = (j0 + x < b.cols) ? R[panel_off(j0 + x, j0 + x, tk.r_rp)] : 0.0;
             }
             __syncthreads();
             for (int t = 0; t < nt; ++t) {
@@ -392,7 +415,7 @@ heff_diag_kernel(const DiagBlock* __restrict__ blocks, const DiagTask* __restric
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const int i = i0 + ty + 8 * q, j = j0 + tx;
-            if (i < b.rows && j < b.cols) diag[b.off + int64_t(i) * b.ld + j] += acc[q];
+            if (i < b.rows && j < b.cols) diag[b.off + panel_off(i, j, b.rows_pad)] += acc[q];
         }
     }
 }

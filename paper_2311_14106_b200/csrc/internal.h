@@ -30,20 +30,36 @@ void count_launch(int64_t n = 1);
 static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 static inline bool aligned128(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 127u) == 0; }
 
-constexpr int LD_PAD = 16;  // leading dimensions and block offsets are multiples of 16 doubles (128 B)
+constexpr int LD_PAD = 16;   // column counts are padded to multiples of 16 doubles (one 128-byte panel row)
+constexpr int ROW_PAD = 4;   // row counts are padded to multiples of 4 (one DMMA k-step) with zero rows
+
+// ---- panel layout of a stored block ------------------------------------------------
+// A block (rows × cols) is stored as ceil(cols/16) column PANELS, panel after panel; a panel holds
+// rows_pad = round_up(rows, 4) rows of 16 doubles (128 bytes), so a (≤64 rows × 16 columns) operand tile
+// — and a (≤16 rows × 16 columns) piece of a transposed one — is ONE contiguous chunk that a single
+// cp.async.bulk moves to shared memory.  Inside a row the 32-byte groups are XOR-swizzled with the row
+// index, so that the shared-memory copy (taken verbatim) is read conflict-free by the DMMA fragment
+// loads both K-major and MN-major (heff_kernels.cu).  Padding rows and columns hold exact zeros.
+__host__ __device__ inline int64_t panel_off(int r, int c, int rows_pad) {
+    return (int64_t(c >> 4) * rows_pad + r) * 16 + ((c & 15) ^ ((r & 3) << 2));
+}
+static inline int32_t pad_rows(int32_t rows) { return (rows + ROW_PAD - 1) / ROW_PAD * ROW_PAD; }
 
 // ---- a1: sectors and blocks --------------------------------------------------------------------
 struct Block {
     int32_t r_idx, c_idx;  // sector indices (row, column); for ψ: (a, b)
-    int32_t rows, cols, ld;
+    int32_t rows, cols, ld;   // ld = round_up(cols, 16): the padded column count
+    int32_t rows_pad;         // round_up(rows, 4); the block occupies rows_pad·ld doubles
     int64_t off;           // doubles into the packed arena
     int64_t uoff;          // elements into the unpadded form
+    int64_t size() const { return int64_t(rows_pad) * ld; }
 };
 
 // Block table mirrored on the device for the fill kernel.
 struct DevBlock {
     int64_t off, uoff;
     int32_t rows, cols, ld, square_diag;
+    int32_t rows_pad, pad_;
 };
 
 }  // namespace dmrgk
@@ -114,8 +130,9 @@ struct Bases {
     unsigned long long b[4];
 };
 
-// One GEMM "segment": C_tile += A[i, k]·B[k, j] over k < klen.  A is K-major (A[i·lda + k]) or
-// M-major (A[k·lda + i]); B is K-major (B[j·ldb + k]) or N-major (B[k·ldb + j]).
+// One GEMM "segment": C_tile += A[i, k]·B[k, j] over k < klen.  Operands are whole stored blocks in the
+// panel layout; A is K-major (stored block = [i][k]) or M-major (stored block = [k][i], the transposed
+// use of an operator); B is K-major (stored [j][k]) or N-major (stored [k][j]).
 enum : uint32_t {
     SEG_A_MMAJOR = 1u,
     SEG_B_NMAJOR = 2u,
@@ -124,38 +141,40 @@ enum : uint32_t {
 };
 struct Seg {
     unsigned long long A, B;   // byte address / byte offset of the operand BLOCK origin
-    int32_t lda, ldb;
+    int32_t a_rp, b_rp;        // rows_pad of the stored A / B block (panel stride = rows_pad·128 bytes)
     int32_t klen;
     uint32_t flags;
 };  // 32 B
 
 // One CTA work unit: a (≤64 × ≤64) tile of C summed over segments [seg_begin, seg_end).
-enum : uint32_t { UNIT_ACCUM = 1u, UNIT_C_SEL_SHIFT = 4 };
+// C is a block in the panel layout (origin + rows_pad) or, with UNIT_C_PLAIN, a private row-major
+// 64×64 tile (split-k partial in the workspace).
+enum : uint32_t { UNIT_ACCUM = 1u, UNIT_C_PLAIN = 2u, UNIT_C_SEL_SHIFT = 4 };
 struct Unit {
-    unsigned long long C;   // byte address / offset of the tile origin
+    unsigned long long C;   // byte address / offset of the C block origin (or of the plain tile)
     double alpha;
-    int32_t ldc;
-    int32_t i0, j0;     // tile origin inside the operand blocks
+    int32_t c_rp;       // rows_pad of the C block
+    int32_t i0, j0;     // tile origin inside the operand blocks and inside the C block
     int32_t mrows;      // block rows (A-operand row extent)
     int32_t ncols;      // block cols (B-operand column extent)
     int32_t ncols_st;   // columns to store (padded ld of the C block); columns ≥ ncols get zeros
     int32_t seg_begin, seg_end;
-    uint32_t mode;      // UNIT_ACCUM | selector << UNIT_C_SEL_SHIFT
+    uint32_t mode;      // UNIT_ACCUM | UNIT_C_PLAIN | selector << UNIT_C_SEL_SHIFT
     int32_t nkt;        // Σ over the unit's segments of ceil(klen/TILE_K)
 };  // 56 B
 
-// Fixed-order reduction of split-k partial tiles into σ: C[r, c] += Σ_s P[s][r·64 + c].
+// Fixed-order reduction of split-k partial tiles into σ: σ_block[i0 + r, j0 + c] += Σ_s P[s][r·64 + c].
 struct RUnit {
-    unsigned long long C;   // byte offset into σ of the tile origin
+    unsigned long long C;   // byte offset into σ of the BLOCK origin
     unsigned long long P;   // byte offset into the workspace of the first partial tile (64×64 each)
-    int32_t ldc, rows, cols, n_split;
-};  // 32 B
+    int32_t c_rp, i0, j0, rows, cols, n_split;
+};  // 40 B
 
 // diag(H_eff) work: ψ block `DiagBlock` sums alpha·L[i,i]·R[j,j] over tasks [t_begin, t_end).
 struct DiagTask {
-    unsigned long long L, R;   // block origins; the diagonal is walked with stride ld+1
+    unsigned long long L, R;   // block origins (panel layout)
     double alpha;
-    int32_t ldl, ldr;
+    int32_t l_rp, r_rp;        // rows_pad of the L / R block
     uint32_t sel;              // selector of L in bits 0-1, of R in bits 2-3
     int32_t pad_;
 };
@@ -163,7 +182,7 @@ struct DiagBlock {
     int64_t off;               // doubles into the ψ-layout arena
     int32_t rows, cols, ld;
     int32_t t_begin, t_end;
-    int32_t pad_;
+    int32_t rows_pad;
 };
 
 constexpr int TILE_M = 64, TILE_N = 64;

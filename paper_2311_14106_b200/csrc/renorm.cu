@@ -85,7 +85,7 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
         for (int64_t i = 0; i < n_ops; ++i)
             for (const Block& ob : in[i]->blocks) {
                 const int pc = phi->by_enl[ob.c_idx], pr = phi->by_enl[ob.r_idx];
-                if (pc >= 0 && pr >= 0) total += int64_t(ob.rows) * phi->blocks[pc].ld * 8;
+                if (pc >= 0 && pr >= 0) total += int64_t(ob.rows_pad) * phi->blocks[pc].ld * 8;
             }
         o.t_chunk_bytes = std::min<int64_t>(int64_t(4) << 30, std::max<int64_t>(int64_t(256) << 20, total / 16));
     }
@@ -112,7 +112,7 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
                     return fail(DMRGK_ESHAPE, "renorm_create: out[%lld] has no block for kept sectors (%d, %d)", (long long)i1, br.c_idx, bc.c_idx);
                 }
                 mine.push_back({&ob, &bc, &br, in[i1]->dev, out[i1]->dev, &out[i1]->blocks[oi]});
-                tb += int64_t(ob.rows) * bc.ld * 8;
+                tb += int64_t(ob.rows_pad) * bc.ld * 8;
             }
             if (!tasks.empty() && t_bytes + tb > o.t_chunk_bytes) break;
             tasks.insert(tasks.end(), mine.begin(), mine.end());
@@ -137,9 +137,9 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
             Seg s1;
             memset(&s1, 0, sizeof(s1));
             s1.A = (unsigned long long)(uintptr_t)(t.in + t.ob->off);
-            s1.lda = t.ob->ld;
+            s1.a_rp = t.ob->rows_pad;
             s1.B = (unsigned long long)(uintptr_t)(phi->dev + t.pc->off);
-            s1.ldb = t.pc->ld;
+            s1.b_rp = t.pc->rows_pad;
             s1.klen = e_c;
             s1.flags = SEG_B_NMAJOR | (BASE_ABS << SEG_A_SEL_SHIFT) | (BASE_ABS << SEG_B_SEL_SHIFT);
             const int32_t si1 = int32_t(segs.size());
@@ -149,9 +149,9 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
                 for (int c0 = 0; c0 < ldt; c0 += TILE_N) {
                     Unit u;
                     memset(&u, 0, sizeof(u));
-                    u.C = (unsigned long long)(t_off + (int64_t(r0) * ldt + c0) * 8);
+                    u.C = (unsigned long long)t_off;            // block origin of T (e_r × n_c, panel layout)
                     u.alpha = 1.0;
-                    u.ldc = ldt;
+                    u.c_rp = pad_rows(e_r);
                     u.i0 = r0;
                     u.j0 = c0;
                     u.mrows = e_r;
@@ -167,9 +167,9 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
             Seg s2;
             memset(&s2, 0, sizeof(s2));
             s2.A = (unsigned long long)(uintptr_t)(phi->dev + t.pr->off);
-            s2.lda = t.pr->ld;
+            s2.a_rp = t.pr->rows_pad;
             s2.B = (unsigned long long)t_off;
-            s2.ldb = ldt;
+            s2.b_rp = pad_rows(e_r);
             s2.klen = e_r;
             s2.flags = SEG_A_MMAJOR | SEG_B_NMAJOR | (BASE_ABS << SEG_A_SEL_SHIFT) | (BASE_WS << SEG_B_SEL_SHIFT);
             const int32_t si2 = int32_t(segs.size());
@@ -180,9 +180,9 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
                 for (int c0 = 0; c0 < ldo; c0 += TILE_N) {
                     Unit u;
                     memset(&u, 0, sizeof(u));
-                    u.C = (unsigned long long)(uintptr_t)(t.out + t.outb->off + int64_t(r0) * ldo + c0);
+                    u.C = (unsigned long long)(uintptr_t)(t.out + t.outb->off);     // block origin
                     u.alpha = 1.0;
-                    u.ldc = ldo;
+                    u.c_rp = t.outb->rows_pad;
                     u.i0 = r0;
                     u.j0 = c0;
                     u.mrows = n_r;
@@ -194,7 +194,7 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
                     u.nkt = int32_t(nkt2);
                     p2.push_back({tile_cost(std::min(TILE_M, n_r - r0), std::min(TILE_N, ldo - c0), nkt2), u});
                 }
-            t_off += int64_t(e_r) * ldt * 8;
+            t_off += int64_t(pad_rows(e_r)) * ldt * 8;
         }
         auto by_cost = [](const CU& a, const CU& b) { return a.cost > b.cost; };
         std::stable_sort(p1.begin(), p1.end(), by_cost);

@@ -33,6 +33,8 @@ static int32_t upload_table(const std::vector<Block>& blocks, DevBlock** out) {
         t[i].rows = blocks[i].rows;
         t[i].cols = blocks[i].cols;
         t[i].ld = blocks[i].ld;
+        t[i].rows_pad = blocks[i].rows_pad;
+        t[i].pad_ = 0;
         t[i].square_diag = (blocks[i].r_idx == blocks[i].c_idx && blocks[i].rows == blocks[i].cols);
     }
     DMRGK_CUDA(cudaMalloc(out, t.size() * sizeof(DevBlock)));
@@ -44,8 +46,8 @@ static void pack_blocks(const std::vector<Block>& blocks, int64_t n_padded, cons
     memset(p, 0, size_t(n_padded) * sizeof(double));
     for (const Block& b : blocks)
         for (int r = 0; r < b.rows; ++r)
-            memcpy(p + b.off + int64_t(r) * b.ld, u + b.uoff + int64_t(r) * b.cols,
-                   size_t(b.cols) * sizeof(double));
+            for (int c = 0; c < b.cols; ++c)
+                p[b.off + panel_off(r, c, b.rows_pad)] = u[b.uoff + int64_t(r) * b.cols + c];
 }
 
 }  // namespace dmrgk
@@ -161,9 +163,10 @@ int32_t dmrgk_layout_create(dmrgk_ctx* ctx, const dmrgk_space* A, const dmrgk_sp
         k.rows = A->dim[a];
         k.cols = B->dim[b];
         k.ld = int32_t(round_up(k.cols, LD_PAD));
+        k.rows_pad = pad_rows(k.rows);
         k.off = off;
         k.uoff = uoff;
-        off += int64_t(k.rows) * k.ld;
+        off += k.size();
         uoff += int64_t(k.rows) * k.cols;
         l->by_a[a] = int32_t(l->blocks.size());
         l->blocks.push_back(k);
@@ -222,8 +225,8 @@ int32_t dmrgk_layout_unpack(const dmrgk_layout* l, const double* p, double* u) {
     if (!l || (l->n_padded && (!u || !p))) return fail(DMRGK_EINVAL, "layout_unpack: NULL argument");
     for (const Block& b : l->blocks)
         for (int r = 0; r < b.rows; ++r)
-            memcpy(u + b.uoff + int64_t(r) * b.cols, p + b.off + int64_t(r) * b.ld,
-                   size_t(b.cols) * sizeof(double));
+            for (int c = 0; c < b.cols; ++c)
+                u[b.uoff + int64_t(r) * b.cols + c] = p[b.off + panel_off(r, c, b.rows_pad)];
     return DMRGK_OK;
 }
 
@@ -252,9 +255,10 @@ int32_t dmrgk_op_create(dmrgk_ctx* ctx, const dmrgk_space* space, const int32_t*
         k.rows = space->dim[r];
         k.cols = space->dim[c];
         k.ld = int32_t(round_up(k.cols, LD_PAD));
+        k.rows_pad = pad_rows(k.rows);
         k.off = off;
         k.uoff = uoff;
-        off += int64_t(k.rows) * k.ld;
+        off += k.size();
         uoff += int64_t(k.rows) * k.cols;
         op->by_col[c] = op->by_row[r] = int32_t(op->blocks.size());
         op->blocks.push_back(k);
@@ -294,6 +298,38 @@ int32_t dmrgk_op_blocks(const dmrgk_op* op, int32_t* row_idx, int32_t* col_idx, 
 int32_t dmrgk_op_pack(const dmrgk_op* op, const double* u, double* p) {
     if (!op || (op->n_padded && (!u || !p))) return fail(DMRGK_EINVAL, "op_pack: NULL argument");
     pack_blocks(op->blocks, op->n_padded, u, p);
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_op_unpack(const dmrgk_op* op, const double* p, double* u) {
+    if (!op || (op->n_padded && (!u || !p))) return fail(DMRGK_EINVAL, "op_unpack: NULL argument");
+    for (const Block& b : op->blocks)
+        for (int r = 0; r < b.rows; ++r)
+            for (int c = 0; c < b.cols; ++c)
+                u[b.uoff + int64_t(r) * b.cols + c] = p[b.off + panel_off(r, c, b.rows_pad)];
+    return DMRGK_OK;
+}
+
+int64_t dmrgk_block_size(int32_t rows, int32_t cols) {
+    if (rows < 0 || cols < 0) return 0;
+    return int64_t(pad_rows(rows)) * round_up(cols, LD_PAD);
+}
+
+int32_t dmrgk_block_unpack(int32_t rows, int32_t cols, const double* packed_host, double* dense_host) {
+    if (rows < 0 || cols < 0 || ((rows && cols) && (!packed_host || !dense_host)))
+        return fail(DMRGK_EINVAL, "block_unpack: bad argument");
+    const int rp = pad_rows(rows);
+    for (int r = 0; r < rows; ++r)
+        for (int c = 0; c < cols; ++c) dense_host[int64_t(r) * cols + c] = packed_host[panel_off(r, c, rp)];
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_block_padding_is_zero(int32_t rows, int32_t cols, const double* packed_host) {
+    if (rows < 0 || cols < 0 || ((rows && cols) && !packed_host)) return fail(DMRGK_EINVAL, "block_padding_is_zero: bad argument");
+    const int rp = pad_rows(rows), ld = int(round_up(cols, LD_PAD));
+    for (int r = 0; r < rp; ++r)
+        for (int c = 0; c < ld; ++c)
+            if ((r >= rows || c >= cols) && packed_host[panel_off(r, c, rp)] != 0.0) return 1;
     return DMRGK_OK;
 }
 
@@ -353,9 +389,10 @@ int32_t dmrgk_iso_create(dmrgk_ctx* ctx, const dmrgk_space* enlarged, const dmrg
         b.rows = enlarged->dim[e];
         b.cols = kept->dim[k];
         b.ld = int32_t(round_up(b.cols, LD_PAD));
+        b.rows_pad = pad_rows(b.rows);
         b.off = off;
         b.uoff = uoff;
-        off += int64_t(b.rows) * b.ld;
+        off += b.size();
         uoff += int64_t(b.rows) * b.cols;
         p->by_enl[e] = int32_t(p->blocks.size());
         p->blocks.push_back(b);

@@ -145,8 +145,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     bool need_ident = false;
     for (int64_t k = 0; k < K; ++k) need_ident |= (flags[k] & (DMRGK_IDENT_L | DMRGK_IDENT_R)) != 0;
     if (need_ident) {
-        std::vector<double> id(size_t(ident_ld) * ident_ld, 0.0);
-        for (int i = 0; i < ident_ld; ++i) id[size_t(i) * ident_ld + i] = 1.0;
+        std::vector<double> id(size_t(ident_ld) * ident_ld, 0.0);      // panel layout, rows_pad = ident_ld
+        for (int i = 0; i < ident_ld; ++i) id[size_t(panel_off(i, i, ident_ld))] = 1.0;
         cudaError_t e = cudaMalloc(&h->ident_dev, id.size() * 8);
         if (e == cudaSuccess) e = cudaMemcpy(h->ident_dev, id.data(), id.size() * 8, cudaMemcpyHostToDevice);
         if (e != cudaSuccess) return bail(fail(DMRGK_ECUDA, "heff_create: identity block: %s", cudaGetErrorString(e)));
@@ -181,7 +181,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 ao = a;
                 t.mo = t.m;
                 t.s1.A = (unsigned long long)(uintptr_t)h->ident_dev;
-                t.s1.lda = ident_ld;
+                t.s1.a_rp = ident_ld;
                 t.s1.flags = BASE_ABS << SEG_A_SEL_SHIFT;
             } else {
                 const int bi = (f & DMRGK_TRANS_L) ? L[k]->by_row[a] : L[k]->by_col[a];
@@ -189,7 +189,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 const Block& lb = L[k]->blocks[bi];
                 ao = (f & DMRGK_TRANS_L) ? lb.c_idx : lb.r_idx;
                 t.mo = (f & DMRGK_TRANS_L) ? lb.cols : lb.rows;
-                t.s1.lda = lb.ld;
+                t.s1.a_rp = lb.rows_pad;
                 t.s1.flags = (f & DMRGK_TRANS_L) ? SEG_A_MMAJOR : 0u;
                 if (L[k]->dev) {
                     t.s1.A = (unsigned long long)(uintptr_t)(L[k]->dev + lb.off);
@@ -203,7 +203,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 bo = b;
                 t.no = t.n;
                 t.s2.B = (unsigned long long)(uintptr_t)h->ident_dev;
-                t.s2.ldb = ident_ld;
+                t.s2.b_rp = ident_ld;
                 t.s2.flags = BASE_ABS << SEG_B_SEL_SHIFT;
             } else {
                 const int bi = (f & DMRGK_TRANS_R) ? R[k]->by_row[b] : R[k]->by_col[b];
@@ -211,7 +211,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 const Block& rb = R[k]->blocks[bi];
                 bo = (f & DMRGK_TRANS_R) ? rb.c_idx : rb.r_idx;
                 t.no = (f & DMRGK_TRANS_R) ? rb.cols : rb.rows;
-                t.s2.ldb = rb.ld;
+                t.s2.b_rp = rb.rows_pad;
                 t.s2.flags = (f & DMRGK_TRANS_R) ? SEG_B_NMAJOR : 0u;
                 if (R[k]->dev) {
                     t.s2.B = (unsigned long long)(uintptr_t)(R[k]->dev + rb.off);
@@ -229,13 +229,13 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             t.diag = (ob == ib);
             // phase-1 B operand = ψ block (N-major), phase-2 A operand = T (K-major, set per chunk)
             t.s1.B = (unsigned long long)(pb[ib].off * 8);
-            t.s1.ldb = pb[ib].ld;
+            t.s1.b_rp = pb[ib].rows_pad;
             t.s1.klen = t.m;
             t.s1.flags |= SEG_B_NMAJOR | (BASE_PSI << SEG_B_SEL_SHIFT);
-            t.s2.lda = pb[ib].ld;
+            t.s2.a_rp = pad_rows(t.mo);                     // T_t is a block (m′ × n) in the panel layout
             t.s2.klen = t.n;
             t.s2.flags |= BASE_WS << SEG_A_SEL_SHIFT;
-            tb += int64_t(t.mo) * pb[ib].ld * 8;
+            tb += int64_t(pad_rows(t.mo)) * pb[ib].ld * 8;
             mine.push_back(t);
         }
         return tb;
@@ -314,7 +314,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             int64_t off = 0;
             for (size_t i = 0; i < tasks.size(); ++i) {
                 t_off[i] = off;
-                off += int64_t(tasks[i].mo) * pb[tasks[i].ib].ld * 8;
+                off += int64_t(pad_rows(tasks[i].mo)) * pb[tasks[i].ib].ld * 8;
             }
             struct U1 {
                 int64_t cost;
@@ -331,9 +331,9 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                     for (int j0 = 0; j0 < ldt; j0 += TILE_N) {
                         Unit u;
                         memset(&u, 0, sizeof(u));
-                        u.C = (unsigned long long)(t_off[i] + (int64_t(i0) * ldt + j0) * 8);
+                        u.C = (unsigned long long)t_off[i];      // block origin of T_t
                         u.alpha = t.alpha;
-                        u.ldc = ldt;
+                        u.c_rp = pad_rows(t.mo);
                         u.i0 = i0;
                         u.j0 = j0;
                         u.mrows = t.mo;
@@ -400,10 +400,10 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                         u.mrows = B.rows;
                         u.ncols = B.cols;
                         u.ncols_st = B.ld;
-                        const unsigned long long c_sigma = (unsigned long long)((B.off + int64_t(i0) * B.ld + j0) * 8);
+                        const unsigned long long c_sigma = (unsigned long long)(B.off * 8);     // block origin in σ
+                        u.c_rp = B.rows_pad;
                         if (n_split == 1) {
                             u.C = c_sigma;
-                            u.ldc = B.ld;
                             u.seg_begin = seg0;
                             u.seg_end = seg0 + ns;
                             u.mode = UNIT_ACCUM | (BASE_SIGMA << UNIT_C_SEL_SHIFT);
@@ -413,7 +413,9 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                             RUnit r;
                             r.C = c_sigma;
                             r.P = (unsigned long long)(partial_tiles * TILE_M * TILE_N * 8);   // rebased below
-                            r.ldc = B.ld;
+                            r.c_rp = B.rows_pad;
+                            r.i0 = i0;
+                            r.j0 = j0;
                             r.rows = rt;
                             r.cols = ct;
                             int made = 0, sb = 0;
@@ -425,10 +427,9 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                                 if (s == n_split - 1) se = ns;
                                 if (se == sb) continue;
                                 u.C = (unsigned long long)((partial_tiles + made) * TILE_M * TILE_N * 8);
-                                u.ldc = TILE_N;
                                 u.seg_begin = seg0 + sb;
                                 u.seg_end = seg0 + se;
-                                u.mode = BASE_WS << UNIT_C_SEL_SHIFT;
+                                u.mode = UNIT_C_PLAIN | (BASE_WS << UNIT_C_SEL_SHIFT);
                                 u.nkt = int32_t(prefix[se] - prefix[sb]);
                                 tmp.push_back({cost_of(rt, ct, u.nkt), u});
                                 ++made;
@@ -461,6 +462,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 d.rows = pb[b].rows;
                 d.cols = pb[b].cols;
                 d.ld = pb[b].ld;
+                d.rows_pad = pb[b].rows_pad;
                 d.t_begin = int32_t(dtasks.size());
                 for (int i : by_b[b]) {
                     const Task& t = tasks[i];
@@ -469,13 +471,12 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                     dt.L = t.s1.A;
                     dt.R = t.s2.B;
                     dt.alpha = t.alpha;
-                    dt.ldl = t.s1.lda;
-                    dt.ldr = t.s2.ldb;
+                    dt.l_rp = t.s1.a_rp;
+                    dt.r_rp = t.s2.b_rp;
                     dt.sel = ((t.s1.flags >> SEG_A_SEL_SHIFT) & 3u) | (((t.s2.flags >> SEG_B_SEL_SHIFT) & 3u) << 2);
                     dtasks.push_back(dt);
                 }
                 d.t_end = int32_t(dtasks.size());
-                d.pad_ = 0;
                 dblocks.push_back(d);
             }
             ch.d_blocks = int64_t(dblocks.size()) - ch.d_block0;
@@ -510,7 +511,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
         for (int64_t i = c.p2_unit0; i < c.p2_unit0 + c.p2_units; ++i) {
             units[i].seg_begin += int32_t(c.p2_seg0);
             units[i].seg_end += int32_t(c.p2_seg0);
-            if (!(units[i].mode & UNIT_ACCUM)) units[i].C += part_base;
+            if (units[i].mode & UNIT_C_PLAIN) units[i].C += part_base;
         }
         for (int64_t i = c.r_unit0; i < c.r_unit0 + c.r_units; ++i) runits[i].P += part_base;
         for (int64_t s = c.p1_seg0; s < c.p1_seg0 + c.p1_segs; ++s)

@@ -61,6 +61,10 @@ SIGNATURES = {
     "dmrgk_op_query": (_i32, [_p, _pi64, _pi64, _pi64]),
     "dmrgk_op_blocks": (_i32, [_p, _p, _p, _p, _p, _p, _p]),
     "dmrgk_op_pack": (_i32, [_p, _p, _p]),
+    "dmrgk_op_unpack": (_i32, [_p, _p, _p]),
+    "dmrgk_block_size": (_i64, [_i32, _i32]),
+    "dmrgk_block_unpack": (_i32, [_i32, _i32, _p, _p]),
+    "dmrgk_block_padding_is_zero": (_i32, [_i32, _i32, _p]),
     "dmrgk_op_bind_device": (_i32, [_p, _p]),
     "dmrgk_op_bind_pinned": (_i32, [_p, _p]),
     "dmrgk_heff_create": (_i32, [_p, _p, _i64, _p, _p, _p, _p, _p, _pp]),
@@ -297,6 +301,29 @@ class Op(_Blocked):
         if getattr(self, "h", None):
             self.lib.dmrgk_op_destroy(self.h)
             self.h = None
+
+
+def block_size(rows, cols):
+    """Doubles a rows×cols block occupies in the panel layout."""
+    return load().dmrgk_block_size(int(rows), int(cols))
+
+
+def block_unpack(packed, rows, cols):
+    """Dense rows×cols array of ONE block from its packed (panel-layout) doubles."""
+    p = np.ascontiguousarray(packed, dtype=np.float64)
+    assert p.size >= block_size(rows, cols)
+    out = np.zeros((int(rows), int(cols)), np.float64)
+    check(load().dmrgk_block_unpack(int(rows), int(cols), p.ctypes.data, out.ctypes.data))
+    return out
+
+
+def block_padding_is_zero(packed, rows, cols):
+    p = np.ascontiguousarray(packed, dtype=np.float64)
+    assert p.size >= block_size(rows, cols)
+    st = load().dmrgk_block_padding_is_zero(int(rows), int(cols), p.ctypes.data)
+    if st < 0:
+        check(st)
+    return st == 0
 
 
 class Iso(_Blocked):

@@ -112,8 +112,8 @@ class DeviceProblem:
         host = src.cpu().numpy()
         out = {}
         for b in range(len(r)):
-            blk = host[off[b]:off[b] + int(rows[b]) * int(ld[b])].reshape(int(rows[b]), int(ld[b]))
-            out[(int(r[b]), int(c[b]))] = blk[:, :cols[b]].copy()
+            n = dmrgk.block_size(rows[b], cols[b])
+            out[(int(r[b]), int(c[b]))] = dmrgk.block_unpack(host[off[b]:off[b] + n], rows[b], cols[b])
         return out
 
     # ---- H_eff ----------------------------------------------------------------------------------
@@ -266,7 +266,7 @@ class RenormProblem:
         host = self.out_views[j].cpu().numpy()
         out, pad_ok = {}, True
         for b in range(len(r)):
-            blk = host[off[b]:off[b] + int(rows[b]) * int(ld[b])].reshape(int(rows[b]), int(ld[b]))
-            out[(int(r[b]), int(c[b]))] = blk[:, :cols[b]].copy()
-            pad_ok = pad_ok and not np.any(blk[:, cols[b]:] != 0.0)
+            blk = host[off[b]:off[b] + dmrgk.block_size(rows[b], cols[b])]
+            out[(int(r[b]), int(c[b]))] = dmrgk.block_unpack(blk, rows[b], cols[b])
+            pad_ok = pad_ok and dmrgk.block_padding_is_zero(blk, rows[b], cols[b])
         return out, pad_ok

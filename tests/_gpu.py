@@ -23,11 +23,12 @@ def rel_max(got, ref):
 
 def padding_is_zero(dp, vec):
     """Every padding column of the packed arena must hold exact zeros."""
+    from paper_2311_14106_b200 import dmrgk
     r, c, rows, cols, ld, off = dp.table
     host = vec[:dp.layout.n_padded].cpu().numpy()
     for b in range(len(r)):
-        blk = host[off[b]:off[b] + int(rows[b]) * int(ld[b])].reshape(int(rows[b]), int(ld[b]))
-        if np.any(blk[:, cols[b]:] != 0.0):
+        blk = host[off[b]:off[b] + dmrgk.block_size(rows[b], cols[b])]
+        if not dmrgk.block_padding_is_zero(blk, rows[b], cols[b]):
             return False
     return True
 
@@ -131,9 +132,11 @@ class DeviceInputs:
         return (key[0] if trans else key[1]), key
 
     def block(self, i, key):
+        from paper_2311_14106_b200 import dmrgk
         rows, cols, ld, off = self.table(i)[key]
         src = self.dp.op_views[i] if i in self.dp.op_views else self.dp.pinned_views[i]
-        blk = src[off:off + rows * ld].view(rows, ld)[:, :cols].cpu().numpy().copy()
+        packed = src[off:off + dmrgk.block_size(rows, cols)].cpu().numpy()
+        blk = dmrgk.block_unpack(packed, rows, cols)       # index translation only (panel layout → dense)
         self.n_read += blk.size
         return blk
 

@@ -33,6 +33,7 @@ def _check_ops(wl, rp, sectors_new, phi, which):
 
 @pytest.mark.parametrize("kernel", [0, 1])
 def test_small_all_operators(kernel):
+    from paper_2311_14106_b200 import dmrgk
     wl = wlmod.lattice_workload("spinless", 5, 24, seed=3)
     dp, rp, sectors_new, table = _device(wl, 11, kernel=kernel)
     phi = wlmod.fill_phi_host(wl, table)
@@ -40,8 +41,9 @@ def test_small_all_operators(kernel):
     r, c, rows, cols, ld, off = rp.phi.blocks()
     host = rp.phi_arena.cpu().numpy()
     for b in range(len(r)):
-        blk = host[off[b]:off[b] + int(rows[b]) * int(ld[b])].reshape(int(rows[b]), int(ld[b]))[:, :cols[b]]
-        assert np.array_equal(blk, phi[(int(r[b]), int(c[b]))])
+        packed = host[off[b]:off[b] + dmrgk.block_size(rows[b], cols[b])]
+        assert np.array_equal(dmrgk.block_unpack(packed, rows[b], cols[b]), phi[(int(r[b]), int(c[b]))])
+        assert dmrgk.block_padding_is_zero(packed, rows[b], cols[b])
     rp.apply()
     torch.cuda.synchronize()
     _check_ops(wl, rp, sectors_new, phi, range(len(rp.idx)))
