@@ -321,7 +321,10 @@ def run_ours(args):
     if args.shard == "k" and world > 1:
         return run_sharded(args, wl, rank, world, local)
     staged = wlmod.config5_staged_ops(wl) if args.config == "5" else []
-    dp = problem.from_workload(wl, device=local, pinned=staged, **({"ring_bytes": 6 << 30} if staged else {}))
+    opts = {"ring_bytes": 6 << 30} if staged else {}
+    if args.kernel:
+        opts["kernel"] = args.kernel
+    dp = problem.from_workload(wl, device=local, pinned=staged, **opts)
     torch.cuda.synchronize()
     h = dp.heff
     n = dp.layout.n_padded
@@ -404,7 +407,7 @@ def run_ours(args):
                    "setup_s": {"tables": round(su["structures"] + su["tasklist"], 3), "tables_what": "sector/block tables + "
                                "task-list build and upload (the paper's 'Tables', PAPER.md:142)", "seeded_fill": round(su["fill"], 3),
                                "seeded_fill_what": "harness fill of the operator arena (stands in for operators a sweep already holds)"},
-                   "chunks": h.n_chunks, "source_hash": dmrgk.source_hash(),
+                   "chunks": h.n_chunks, "source_hash": dmrgk.source_hash(), "kernel_variant": args.kernel,
                    "staged_ops": len(staged), "staged_bytes_per_apply": int(sum(dp.ops[i].n_padded for i in staged) * 8)},
         "davidson_step_ms": ms_step, "theta_last": r["theta"], "resnorm_last": r["rho"],
         "apply_burst": {"ms": burst_ms, "tflops": h.flops_alg / burst_ms / 1e9, "what": "best of 10 single applies, each timed alone"},
@@ -647,6 +650,9 @@ def main():
     ap.add_argument("--config", default="4", choices=["2", "3", "3b", "4", "5", "5r"])
     ap.add_argument("--m-max", dest="m_max", type=int, default=16)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--kernel", type=int, default=0, choices=[0, 2, 3, 4],
+                    help="GEMM kernel variant (dmrgk_heff_opts.kernel): 0 = product path; 2, 3, 4 = other (stages, CTAs/SM) "
+                         "instantiations kept for measurement")
     ap.add_argument("--no-extras", dest="no_extras", action="store_true",
                     help="skip the extra rows (renormalisation, configs 3 and 2) of the default config-4 line")
     ap.add_argument("--shard", default="none", choices=["none", "k"],

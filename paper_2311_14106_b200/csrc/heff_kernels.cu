@@ -22,11 +22,9 @@ namespace dmrgk {
 
 constexpr int BM = TILE_M, BN = TILE_N, BK = TILE_K;
 constexpr int NTHREADS = 128;           // 4 warps as 2×2, each a 32×32 warp tile = 4×4 DMMA frags
-constexpr int STAGES = 6;
-constexpr int MIN_CTAS = 2;
 constexpr int OPER_DOUBLES = BM * BK;    // 1024: one operand tile, dense 128-byte rows
-constexpr int STAGE_DOUBLES = 2 * OPER_DOUBLES;
-constexpr int SMEM_BYTES = STAGES * STAGE_DOUBLES * 8;   // 98304 → 2 CTAs per SM
+constexpr int STAGE_DOUBLES = 2 * OPER_DOUBLES;          // 16 KB per stage
+constexpr int smem_bytes(int stages) { return stages * STAGE_DOUBLES * 8; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -155,6 +153,7 @@ struct StageNote {
     int32_t nks;      // k-steps of 4 that hold data in this k-tile (1..4)
 };
 
+template <int STAGES, int MIN_CTAS>
 __global__ void __launch_bounds__(NTHREADS, MIN_CTAS)
 heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ segs, Bases bases) {
     extern __shared__ __align__(128) double smem[];
@@ -192,30 +191,33 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     // ---- producer cursor (kept by every thread, uniform): the segment and k-offset of the next tile ----
+    // The descriptor of the FOLLOWING segment is loaded while the current one is being consumed, so a
+    // segment switch costs no memory latency (the host never emits a segment with klen = 0).
     int p_seg = u.seg_begin, p_k0 = 0;
     struct {
         unsigned long long A, B;
         int a_rp, b_rp, klen;
         uint32_t flags;
     } p_sg = {0ull, 0ull, 0, 0, 0, 0u};
-    auto open_segment = [&]() {
-        while (p_seg < u.seg_end) {
-            const int4 lo = __ldg(reinterpret_cast<const int4*>(segs + p_seg));          // A, B
-            const int4 hi = __ldg(reinterpret_cast<const int4*>(segs + p_seg) + 1);      // a_rp, b_rp, klen, flags
-            if (hi.z > 0) {
-                p_sg.A = (unsigned long long)(unsigned)lo.x | ((unsigned long long)(unsigned)lo.y << 32);
-                p_sg.B = (unsigned long long)(unsigned)lo.z | ((unsigned long long)(unsigned)lo.w << 32);
-                p_sg.a_rp = hi.x;
-                p_sg.b_rp = hi.y;
-                p_sg.klen = hi.z;
-                p_sg.flags = uint32_t(hi.w);
-                p_k0 = 0;
-                return;
-            }
-            ++p_seg;
+    int4 n_lo = make_int4(0, 0, 0, 0), n_hi = make_int4(0, 0, 0, 0);
+    auto prefetch_segment = [&](int idx) {
+        if (idx < u.seg_end) {
+            n_lo = __ldg(reinterpret_cast<const int4*>(segs + idx));          // A, B
+            n_hi = __ldg(reinterpret_cast<const int4*>(segs + idx) + 1);      // a_rp, b_rp, klen, flags
         }
     };
-    open_segment();
+    auto adopt_segment = [&]() {
+        p_sg.A = (unsigned long long)(unsigned)n_lo.x | ((unsigned long long)(unsigned)n_lo.y << 32);
+        p_sg.B = (unsigned long long)(unsigned)n_lo.z | ((unsigned long long)(unsigned)n_lo.w << 32);
+        p_sg.a_rp = n_hi.x;
+        p_sg.b_rp = n_hi.y;
+        p_sg.klen = n_hi.z;
+        p_sg.flags = uint32_t(n_hi.w);
+        p_k0 = 0;
+    };
+    prefetch_segment(p_seg);
+    adopt_segment();
+    prefetch_segment(p_seg + 1);
     const int total = u.nkt;
     const int rows_a = rows_t;                            // A-operand rows that exist in this tile
     // Fetch tile `t` (the cursor's tile) into its stage; `wait_parity` < 0: the stage has never been used.
@@ -251,7 +253,8 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
         p_k0 += BK;
         if (p_k0 >= p_sg.klen) {
             ++p_seg;
-            open_segment();
+            adopt_segment();
+            prefetch_segment(p_seg + 1);
         }
     };
 
@@ -420,8 +423,31 @@ heff_diag_kernel(const DiagBlock* __restrict__ blocks, const DiagTask* __restric
     }
 }
 
+static int g_gemm_ctas_per_sm = 0;
+int gemm_ctas_per_sm() { return g_gemm_ctas_per_sm; }
+
+// Kernel variants (dmrgk_heff_opts.kernel): 0 = product path; 1 = scalar check kernel; 2, 3, 4 = other
+// (stages, CTAs per SM) instantiations of the same DMMA kernel, kept for measurement (profiles/).
+template <int STAGES, int MIN_CTAS>
+static int32_t setup_variant(int* resident) {
+    auto* fn = heff_gemm_dmma_kernel<STAGES, MIN_CTAS>;
+    DMRGK_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes(STAGES)));
+    // the L1/shared split must leave room for MIN_CTAS CTAs: ask for the largest shared-memory carve-out
+    // and verify the residency instead of trusting the driver's heuristic
+    DMRGK_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    int n = 0;
+    DMRGK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, NTHREADS, smem_bytes(STAGES)));
+    if (resident) *resident = n;
+    if (n < MIN_CTAS)
+        return fail(DMRGK_ECUDA, "gemm kernel <%d stages, %d CTAs>: only %d CTA(s) per SM resident", STAGES, MIN_CTAS, n);
+    return DMRGK_OK;
+}
+
 int32_t gemm_kernel_setup() {
-    DMRGK_CUDA(cudaFuncSetAttribute(heff_gemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    DMRGK_TRY((setup_variant<3, 4>(&g_gemm_ctas_per_sm)));
+    DMRGK_TRY((setup_variant<4, 3>(nullptr)));
+    DMRGK_TRY((setup_variant<4, 2>(nullptr)));
+    DMRGK_TRY((setup_variant<6, 2>(nullptr)));
     return DMRGK_OK;
 }
 
@@ -429,10 +455,14 @@ int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev
                           const Bases& bases, cudaStream_t st) {
     if (n_units <= 0) return DMRGK_OK;
     if (n_units > 0x7fffffffLL) return fail(DMRGK_EINVAL, "too many work units in one launch: %lld", (long long)n_units);
-    if (kernel == 1)
-        heff_gemm_scalar_kernel<<<unsigned(n_units), NTHREADS, 0, st>>>(units_dev, segs_dev, bases);
-    else
-        heff_gemm_dmma_kernel<<<unsigned(n_units), NTHREADS, SMEM_BYTES, st>>>(units_dev, segs_dev, bases);
+    const unsigned grid = unsigned(n_units);
+    switch (kernel) {
+        case 1: heff_gemm_scalar_kernel<<<grid, NTHREADS, 0, st>>>(units_dev, segs_dev, bases); break;
+        case 2: heff_gemm_dmma_kernel<4, 3><<<grid, NTHREADS, smem_bytes(4), st>>>(units_dev, segs_dev, bases); break;
+        case 3: heff_gemm_dmma_kernel<4, 2><<<grid, NTHREADS, smem_bytes(4), st>>>(units_dev, segs_dev, bases); break;
+        case 4: heff_gemm_dmma_kernel<6, 2><<<grid, NTHREADS, smem_bytes(6), st>>>(units_dev, segs_dev, bases); break;
+        default: heff_gemm_dmma_kernel<3, 4><<<grid, NTHREADS, smem_bytes(3), st>>>(units_dev, segs_dev, bases); break;
+    }
     count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;

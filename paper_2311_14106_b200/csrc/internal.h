@@ -195,6 +195,7 @@ int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cu
 int32_t launch_diag(const DiagBlock* blocks_dev, const DiagTask* tasks_dev, int64_t n_blocks,
                     double* diag, const Bases& bases, cudaStream_t st);
 int32_t gemm_kernel_setup();   // opt-in shared memory attribute, once
+int gemm_ctas_per_sm();        // resident CTAs per SM of the GEMM kernel, as reported by the occupancy API
 
 // chunk = contiguous range of operator pairs processed together
 struct StageCopy {
