@@ -17,6 +17,7 @@
 // the warps (tile t is fetched by lane 0 of warp t mod 4).  2 CTAs per SM: with the warps decoupled
 // by mbarriers the DMMA pipe runs fastest at two resident warps per scheduler (profiles/r2_tma_summary.md).
 #include "internal.h"
+#include <algorithm>
 
 namespace dmrgk {
 
@@ -321,6 +322,216 @@ heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ se
     }
 }
 
+
+// ---- persistent, warp-specialised form (the product path) ------------------------------------------
+// grid = CTAS_PER_SM · n_SM CTAs of 5 warps.  Warp 4 is the PRODUCER: it claims work units from a
+// device-side queue (atomicAdd on a per-launch counter; units are sorted longest first, so this is LPT
+// list scheduling), publishes each unit's descriptor in a small shared-memory ring and streams the
+// operand tiles of unit after unit through the stage ring with cp.async.bulk — it never waits for a
+// unit to finish, so the pipeline does not drain between units and the unit-descriptor, segment-
+// descriptor and first-tile latencies that a one-unit-per-CTA launch pays at every CTA start are
+// hidden.  Warps 0-3 are CONSUMERS: wait full → LDS.64 + DMMA → arrive empty; at a unit's end each
+// warp stores its own fragment rows and moves on (no CTA-wide barrier anywhere after the prologue).
+// The stop signal is a descriptor with nkt = 0 published through the same ring on a data-less tile.
+constexpr int P_NTHREADS = 160;
+
+template <int STAGES, int MIN_CTAS>
+__global__ void __launch_bounds__(P_NTHREADS, MIN_CTAS)
+heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __restrict__ segs, int n_units,
+                                 int* __restrict__ queue_head, Bases bases) {
+    constexpr int RING = STAGES + 1;       // a unit has ≥ 1 tile, the producer runs ≤ STAGES tiles ahead
+    extern __shared__ __align__(128) double smem[];
+    __shared__ __align__(8) unsigned long long bars[2 * STAGES];   // full[0..S), empty[S..2S)
+    __shared__ StageNote notes[STAGES];
+    __shared__ __align__(16) Unit ring[RING];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t smem_base = smem_u32(smem), bar0 = smem_u32(bars);
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(bar0 + s * 8, 1);                   // full: the producer's arrive (+ the copies' bytes)
+            mbar_init(bar0 + (STAGES + s) * 8, 4);        // empty: one arrive per consumer warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == 4) {
+        // ================================ PRODUCER ================================
+        auto claim = [&]() -> int {
+            int v = 0;
+            if (lane == 0) v = atomicAdd(queue_head, 1);
+            return __shfl_sync(0xffffffffu, v, 0);
+        };
+        auto load_unit = [&](int idx, int4 (&w)[4]) {
+            if (idx < n_units) {
+                const int4* p = reinterpret_cast<const int4*>(units + idx);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) w[q] = __ldg(p + q);
+            }
+        };
+        // two claims ahead: cur is being produced, nxt's descriptor is in flight, nx2's index is in flight
+        int cur = claim(), nxt = claim(), nx2 = claim();
+        int4 uw[4], nw[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) uw[q] = nw[q] = make_int4(0, 0, 0, 0);
+        load_unit(cur, uw);
+        load_unit(nxt, nw);
+        int T = 0, stage = 0, ring_pos = 0;
+        uint32_t eph = 1;                                 // parity to wait for on empty[stage]: (T/S − 1) & 1
+        auto advance_stage = [&]() {
+            ++T;
+            if (++stage == STAGES) {
+                stage = 0;
+                eph ^= 1u;
+            }
+        };
+        int4 s_lo = make_int4(0, 0, 0, 0), s_hi = make_int4(0, 0, 0, 0);
+        while (cur < n_units) {
+            // fields of the unit (Unit layout: C, alpha | c_rp, i0, j0, mrows | ncols, ncols_st, seg_begin, seg_end | mode, nkt, -, -)
+            const int i0 = uw[1].y, j0 = uw[1].z, mrows = uw[1].w, ncols = uw[2].x;
+            const int seg_begin = uw[2].z, seg_end = uw[2].w;
+            const int rows_a = min(BM, mrows - i0), cols_b = min(BN, ncols - j0);
+            const int npa = (rows_a + 15) >> 4, npb = (cols_b + 15) >> 4;
+            bool first = true;
+            s_lo = __ldg(reinterpret_cast<const int4*>(segs + seg_begin));
+            s_hi = __ldg(reinterpret_cast<const int4*>(segs + seg_begin) + 1);
+            for (int sg = seg_begin; sg < seg_end; ++sg) {
+                const unsigned long long sA = (unsigned long long)(unsigned)s_lo.x | ((unsigned long long)(unsigned)s_lo.y << 32);
+                const unsigned long long sB = (unsigned long long)(unsigned)s_lo.z | ((unsigned long long)(unsigned)s_lo.w << 32);
+                const int a_rp = s_hi.x, b_rp = s_hi.y, klen = s_hi.z;
+                const uint32_t flags = uint32_t(s_hi.w);
+                if (sg + 1 < seg_end) {                   // the next descriptor travels while this segment streams
+                    s_lo = __ldg(reinterpret_cast<const int4*>(segs + sg + 1));
+                    s_hi = __ldg(reinterpret_cast<const int4*>(segs + sg + 1) + 1);
+                }
+                const bool am = (flags & SEG_A_MMAJOR) != 0, bn = (flags & SEG_B_NMAJOR) != 0;
+                const char* A = reinterpret_cast<const char*>(bases.b[(flags >> SEG_A_SEL_SHIFT) & 3u] + sA);
+                const char* B = reinterpret_cast<const char*>(bases.b[(flags >> SEG_B_SEL_SHIFT) & 3u] + sB);
+                const int na = am ? npa : 1, nb = bn ? npb : 1;      // copies of this segment's tiles
+                for (int k0 = 0; k0 < klen; k0 += BK) {
+                    if (T >= STAGES) mbar_wait(bar0 + (STAGES + stage) * 8, eph);
+                    const int nk4 = (min(BK, klen - k0) + 3) & ~3;
+                    const uint32_t bytes_a = am ? uint32_t(npa * nk4 * 128) : uint32_t(rows_a * 128);
+                    const uint32_t bytes_b = bn ? uint32_t(npb * nk4 * 128) : uint32_t(cols_b * 128);
+                    const uint32_t full = bar0 + stage * 8;
+                    if (lane == 0) {
+                        if (first) {
+                            int4* slot = reinterpret_cast<int4*>(&ring[ring_pos]);
+#pragma unroll
+                            for (int q = 0; q < 4; ++q) slot[q] = uw[q];
+                        }
+                        notes[stage].flags = flags;
+                        notes[stage].nks = nk4 >> 2;
+                        mbar_expect_tx(full, bytes_a + bytes_b);
+                    }
+                    __syncwarp();
+                    // lane l issues copy l: A copies first, then B copies (≤ 8 in all)
+                    const uint32_t dA = smem_base + stage * (STAGE_DOUBLES * 8), dB = dA + OPER_DOUBLES * 8;
+                    if (lane < na) {
+                        if (!am) bulk_g2s(dA, A + (int64_t(k0 >> 4) * a_rp + i0) * 128, bytes_a, full);
+                        else bulk_g2s(dA + lane * 2048, A + (int64_t((i0 >> 4) + lane) * a_rp + k0) * 128, uint32_t(nk4 * 128), full);
+                    } else if (lane < na + nb) {
+                        const int pp = lane - na;
+                        if (!bn) bulk_g2s(dB, B + (int64_t(k0 >> 4) * b_rp + j0) * 128, bytes_b, full);
+                        else bulk_g2s(dB + pp * 2048, B + (int64_t((j0 >> 4) + pp) * b_rp + k0) * 128, uint32_t(nk4 * 128), full);
+                    }
+                    if (first) {
+                        first = false;
+                        if (++ring_pos == RING) ring_pos = 0;
+                    }
+                    advance_stage();
+                }
+            }
+            // next unit: its descriptor was requested one unit ago, its successor's index two units ago
+            cur = nxt;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) uw[q] = nw[q];
+            nxt = nx2;
+            load_unit(nxt, nw);
+            nx2 = claim();
+        }
+        // stop sentinel on a data-less tile
+        if (T >= STAGES) mbar_wait(bar0 + (STAGES + stage) * 8, eph);
+        if (lane == 0) {
+            int4* slot = reinterpret_cast<int4*>(&ring[ring_pos]);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) slot[q] = make_int4(0, 0, 0, 0);      // nkt = 0
+            mbar_arrive(bar0 + stage * 8);
+        }
+        return;
+    }
+
+    // ================================ CONSUMERS ================================
+    const int wm = warp >> 1, wn = warp & 1;
+    const int g = lane >> 2, t4 = lane & 3, g3 = g & 3;
+    const FragBase fa = make_frag_base(0, wm, g, t4), fb = make_frag_base(OPER_DOUBLES, wn, g, t4);
+    int stage = 0, ring_pos = 0;
+    uint32_t ph = 0;
+    while (true) {
+        mbar_wait(bar0 + stage * 8, ph);                  // first tile of the next unit (or the stop tile)
+        const Unit u = ring[ring_pos];
+        if (++ring_pos == RING) ring_pos = 0;
+        if (u.nkt == 0) break;
+        const int rows_t = min(BM, u.mrows - u.i0);
+        const int cols_t = min(BN, u.ncols_st - u.j0);
+        const int cols_b = min(BN, u.ncols - u.j0);
+        const int nfm = max(0, min(4, (rows_t - wm * 32 + 7) >> 3));
+        const int nfn = max(0, min(4, (cols_b - wn * 32 + 7) >> 3));
+        const bool busy = nfm > 0 && nfn > 0;
+        double acc[4][4][2];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+#pragma unroll 1
+        for (int it = 0; it < u.nkt; ++it) {
+            if (it > 0) mbar_wait(bar0 + stage * 8, ph);
+            if (busy) {
+                const StageNote note = notes[stage];
+                const double* st = smem + stage * STAGE_DOUBLES;
+                switch (note.flags & (SEG_A_MMAJOR | SEG_B_NMAJOR)) {
+                    case 0: mma_layout<false, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                    case SEG_A_MMAJOR: mma_layout<true, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                    case SEG_B_NMAJOR: mma_layout<false, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                    default: mma_layout<true, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar0 + (STAGES + stage) * 8);
+            if (++stage == STAGES) {
+                stage = 0;
+                ph ^= 1u;
+            }
+        }
+        // epilogue: lane holds C[row g][cols 2·t4, 2·t4+1] of each 8×8 fragment
+        double* C = reinterpret_cast<double*>(bases.b[(u.mode >> UNIT_C_SEL_SHIFT) & 3u] + u.C);
+        const bool accum = (u.mode & UNIT_ACCUM) != 0, plain = (u.mode & UNIT_C_PLAIN) != 0;
+        const int rows_st = plain ? rows_t : min(BM, u.c_rp - u.i0);      // padding rows get zeros
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int r = wm * 32 + i * 8 + g;
+            if (r >= rows_st) continue;
+            const bool live = r < rows_t;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int c = wn * 32 + j * 8 + 2 * t4;
+                if (c >= cols_t) continue;
+                double2* p = reinterpret_cast<double2*>(plain ? C + r * BN + c : C + panel_off(u.i0 + r, u.j0 + c, u.c_rp));
+                double2 v;
+                v.x = (live && u.j0 + c < u.ncols) ? u.alpha * acc[i][j][0] : 0.0;
+                v.y = (live && u.j0 + c + 1 < u.ncols) ? u.alpha * acc[i][j][1] : 0.0;
+                if (accum) {
+                    double2 o = *p;
+                    v.x += o.x;
+                    v.y += o.y;
+                }
+                *p = v;
+            }
+        }
+    }
+}
+
 // Scalar check kernel over the same work lists: one thread per output element, plain FMA loops reading
 // global memory directly through panel_off.  A debugging aid (dmrgk_heff_opts.kernel = 1), never the
 // product path.
@@ -426,42 +637,45 @@ heff_diag_kernel(const DiagBlock* __restrict__ blocks, const DiagTask* __restric
 static int g_gemm_ctas_per_sm = 0;
 int gemm_ctas_per_sm() { return g_gemm_ctas_per_sm; }
 
-// Kernel variants (dmrgk_heff_opts.kernel): 0 = product path; 1 = scalar check kernel; 2, 3, 4 = other
-// (stages, CTAs per SM) instantiations of the same DMMA kernel, kept for measurement (profiles/).
-template <int STAGES, int MIN_CTAS>
-static int32_t setup_variant(int* resident) {
-    auto* fn = heff_gemm_dmma_kernel<STAGES, MIN_CTAS>;
-    DMRGK_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes(STAGES)));
-    // the L1/shared split must leave room for MIN_CTAS CTAs: ask for the largest shared-memory carve-out
+// Kernel variants (dmrgk_heff_opts.kernel): 0 = product path (persistent, warp-specialised); 1 = scalar
+// check kernel; 2, 3 = other (stages, CTAs per SM) instantiations of the persistent kernel; 4 = the
+// one-unit-per-CTA kernel it replaced — all kept for measurement (profiles/).
+template <class K>
+static int32_t setup_kernel(K* fn, int threads, int stages, int min_ctas, int* resident) {
+    DMRGK_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes(stages)));
+    // the L1/shared split must leave room for min_ctas CTAs: ask for the largest shared-memory carve-out
     // and verify the residency instead of trusting the driver's heuristic
     DMRGK_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     int n = 0;
-    DMRGK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, NTHREADS, smem_bytes(STAGES)));
+    DMRGK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, threads, smem_bytes(stages)));
     if (resident) *resident = n;
-    if (n < MIN_CTAS)
-        return fail(DMRGK_ECUDA, "gemm kernel <%d stages, %d CTAs>: only %d CTA(s) per SM resident", STAGES, MIN_CTAS, n);
+    if (n < min_ctas)
+        return fail(DMRGK_ECUDA, "gemm kernel <%d stages, %d CTAs>: only %d CTA(s) per SM resident", stages, min_ctas, n);
     return DMRGK_OK;
 }
 
 int32_t gemm_kernel_setup() {
-    DMRGK_TRY((setup_variant<3, 4>(&g_gemm_ctas_per_sm)));
-    DMRGK_TRY((setup_variant<4, 3>(nullptr)));
-    DMRGK_TRY((setup_variant<4, 2>(nullptr)));
-    DMRGK_TRY((setup_variant<6, 2>(nullptr)));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<6, 2>, P_NTHREADS, 6, 2, &g_gemm_ctas_per_sm));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, 3>, P_NTHREADS, 4, 3, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, 2>, P_NTHREADS, 4, 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_kernel<3, 4>, NTHREADS, 3, 4, nullptr));
     return DMRGK_OK;
 }
 
 int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
-                          const Bases& bases, cudaStream_t st) {
+                          const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm) {
     if (n_units <= 0) return DMRGK_OK;
     if (n_units > 0x7fffffffLL) return fail(DMRGK_EINVAL, "too many work units in one launch: %lld", (long long)n_units);
     const unsigned grid = unsigned(n_units);
+    const int nu = int(n_units);
+    auto pgrid = [&](int ctas) { return unsigned(std::min<int64_t>(n_units, int64_t(n_sm) * ctas)); };
+    if (kernel != 1 && kernel != 4 && !counter_dev) return fail(DMRGK_EINVAL, "launch_gemm_units: the persistent kernel needs a queue counter");
     switch (kernel) {
         case 1: heff_gemm_scalar_kernel<<<grid, NTHREADS, 0, st>>>(units_dev, segs_dev, bases); break;
-        case 2: heff_gemm_dmma_kernel<4, 3><<<grid, NTHREADS, smem_bytes(4), st>>>(units_dev, segs_dev, bases); break;
-        case 3: heff_gemm_dmma_kernel<4, 2><<<grid, NTHREADS, smem_bytes(4), st>>>(units_dev, segs_dev, bases); break;
-        case 4: heff_gemm_dmma_kernel<6, 2><<<grid, NTHREADS, smem_bytes(6), st>>>(units_dev, segs_dev, bases); break;
-        default: heff_gemm_dmma_kernel<3, 4><<<grid, NTHREADS, smem_bytes(3), st>>>(units_dev, segs_dev, bases); break;
+        case 2: heff_gemm_dmma_persistent_kernel<4, 3><<<pgrid(3), P_NTHREADS, smem_bytes(4), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 3: heff_gemm_dmma_persistent_kernel<4, 2><<<pgrid(2), P_NTHREADS, smem_bytes(4), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 4: heff_gemm_dmma_kernel<3, 4><<<grid, NTHREADS, smem_bytes(3), st>>>(units_dev, segs_dev, bases); break;
+        default: heff_gemm_dmma_persistent_kernel<6, 2><<<pgrid(2), P_NTHREADS, smem_bytes(6), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
     }
     count_launch();
     DMRGK_CUDA(cudaGetLastError());

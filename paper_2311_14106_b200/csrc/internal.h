@@ -160,8 +160,10 @@ struct Unit {
     int32_t ncols_st;   // columns to store (padded ld of the C block); columns ≥ ncols get zeros
     int32_t seg_begin, seg_end;
     uint32_t mode;      // UNIT_ACCUM | UNIT_C_PLAIN | selector << UNIT_C_SEL_SHIFT
-    int32_t nkt;        // Σ over the unit's segments of ceil(klen/TILE_K)
-};  // 56 B
+    int32_t nkt;        // Σ over the unit's segments of ceil(klen/TILE_K); ≥ 1 (0 marks the stop sentinel)
+    int32_t pad_[2];
+};  // 64 B: four 16-byte words (the persistent kernel passes descriptors through shared memory)
+static_assert(sizeof(Unit) == 64, "Unit must be 64 bytes");
 
 // Fixed-order reduction of split-k partial tiles into σ: σ_block[i0 + r, j0 + c] += Σ_s P[s][r·64 + c].
 struct RUnit {
@@ -189,8 +191,9 @@ constexpr int TILE_M = 64, TILE_N = 64;
 constexpr int TILE_K = 16;   // contraction depth of one pipeline stage (k-tile); Unit::nkt counts these
 
 // kernel launchers (heff_kernels.cu)
+// `counter_dev`: a zeroed int the persistent kernel uses as its unit queue head (one per launch in flight)
 int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
-                          const Bases& bases, cudaStream_t st);
+                          const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm);
 int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cudaStream_t st);
 int32_t launch_diag(const DiagBlock* blocks_dev, const DiagTask* tasks_dev, int64_t n_blocks,
                     double* diag, const Bases& bases, cudaStream_t st);
@@ -226,6 +229,7 @@ struct dmrgk_renorm {
     std::vector<RChunk> chunks;
     dmrgk::Unit* units_dev = nullptr;
     dmrgk::Seg* segs_dev = nullptr;
+    int* counters_dev = nullptr;          // unit-queue heads of the persistent kernel, two per chunk
     // same choreography as dmrgk_heff_apply: phase 1 of chunk c+1 (lowest-priority stream) overlaps
     // phase 2 of chunk c (greatest-priority stream); T is double-buffered
     cudaStream_t s1 = nullptr, s2 = nullptr;
@@ -250,6 +254,7 @@ struct dmrgk_heff {
     dmrgk::DiagTask* dtasks_dev = nullptr;
     int64_t n_dblocks = 0;
     double* ident_dev = nullptr;       // identity block for IDENT_L / IDENT_R factors
+    int* counters_dev = nullptr;       // unit-queue heads of the persistent kernel, two per chunk (zeroed per apply)
     cudaEvent_t ev_copy[3] = {nullptr, nullptr, nullptr}, ev_done[3] = {nullptr, nullptr, nullptr};
     // phase 1 of chunk c+1 runs on a library-owned side stream concurrently with phase 2 of chunk c
     // (T is double-buffered), so the tail of one launch is filled by the CTAs of the other

@@ -41,6 +41,7 @@ void dmrgk_renorm_destroy(dmrgk_renorm* r) {
     if (!r) return;
     cudaFree(r->units_dev);
     cudaFree(r->segs_dev);
+    cudaFree(r->counters_dev);
     for (int i = 0; i < 2; ++i) {
         if (r->ev_p1[i]) cudaEventDestroy(r->ev_p1[i]);
         if (r->ev_p2[i]) cudaEventDestroy(r->ev_p2[i]);
@@ -241,6 +242,8 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
     for (const auto& c : r->chunks) r->n_launches += (c.p1_units > 0) + (c.p2_units > 0);
     int32_t s = upload(units, &r->units_dev);
     if (s == DMRGK_OK) s = upload(segs, &r->segs_dev);
+    if (s == DMRGK_OK && cudaMalloc(&r->counters_dev, (2 * r->chunks.size() + 2) * sizeof(int)) != cudaSuccess)
+        s = fail(DMRGK_ECUDA, "renorm_create: queue counters");
     if (s != DMRGK_OK) {
         dmrgk_renorm_destroy(r);
         return s;
@@ -271,6 +274,7 @@ int32_t dmrgk_renorm_apply(dmrgk_renorm* r, void* workspace_dev, void* stream) {
     bases.b[BASE_WS] = (unsigned long long)(uintptr_t)workspace_dev;
     bases.b[BASE_PSI] = 0;
     bases.b[BASE_SIGMA] = 0;
+    DMRGK_CUDA(cudaMemsetAsync(r->counters_dev, 0, (2 * r->chunks.size() + 2) * sizeof(int), st));
     DMRGK_CUDA(cudaEventRecord(r->ev_fork, st));
     DMRGK_CUDA(cudaStreamWaitEvent(r->s1, r->ev_fork, 0));
     DMRGK_CUDA(cudaStreamWaitEvent(r->s2, r->ev_fork, 0));
@@ -279,10 +283,10 @@ int32_t dmrgk_renorm_apply(dmrgk_renorm* r, void* workspace_dev, void* stream) {
         for (size_t c = 0; c < r->chunks.size(); ++c) {
             const auto& ch = r->chunks[c];
             if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(r->s1, r->ev_p2[c & 1], 0));     // T buffer re-use
-            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p1_unit0, r->segs_dev, ch.p1_units, bases, r->s1));
+            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p1_unit0, r->segs_dev, ch.p1_units, bases, r->s1, r->counters_dev + 2 * c, r->ctx->n_sm));
             DMRGK_CUDA(cudaEventRecord(r->ev_p1[c & 1], r->s1));
             DMRGK_CUDA(cudaStreamWaitEvent(r->s2, r->ev_p1[c & 1], 0));
-            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p2_unit0, r->segs_dev, ch.p2_units, bases, r->s2));
+            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p2_unit0, r->segs_dev, ch.p2_units, bases, r->s2, r->counters_dev + 2 * c + 1, r->ctx->n_sm));
             DMRGK_CUDA(cudaEventRecord(r->ev_p2[c & 1], r->s2));
         }
         return DMRGK_OK;

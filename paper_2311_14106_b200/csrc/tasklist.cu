@@ -59,6 +59,7 @@ void dmrgk_heff_destroy(dmrgk_heff* h) {
     cudaFree(h->dblocks_dev);
     cudaFree(h->dtasks_dev);
     cudaFree(h->ident_dev);
+    cudaFree(h->counters_dev);
     for (int i = 0; i < 3; ++i) {
         if (h->ev_copy[i]) cudaEventDestroy(h->ev_copy[i]);
         if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
@@ -535,6 +536,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     if (s == DMRGK_OK) s = upload(dblocks, &h->dblocks_dev);
     if (s == DMRGK_OK) s = upload(dtasks, &h->dtasks_dev);
     if (s != DMRGK_OK) return bail(s);
+    if (cudaMalloc(&h->counters_dev, (2 * h->chunks.size() + 2) * sizeof(int)) != cudaSuccess)
+        return bail(fail(DMRGK_ECUDA, "heff_create: queue counters"));
     {
         int prio_lo = 0, prio_hi = 0;
         cudaError_t e = cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
@@ -656,6 +659,7 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
     bases.b[BASE_PSI] = (unsigned long long)(uintptr_t)psi_dev;
     bases.b[BASE_SIGMA] = (unsigned long long)(uintptr_t)sigma_dev;
     DMRGK_CUDA(cudaMemsetAsync(sigma_dev, 0, size_t(n) * 8, main));
+    DMRGK_CUDA(cudaMemsetAsync(h->counters_dev, 0, (2 * h->chunks.size() + 2) * sizeof(int), main));
     // Stream choreography (all ordering by events; s1 and s2 are library-owned, non-blocking):
     //   s1 (lowest priority)  : p1(0)            p1(1)              p1(2) …   phase 1 of chunk c → T buffer c mod 2
     //   s2 (greatest priority):        p2(0) r(0)       p2(1) r(1) …          phase 2 + reduce of chunk c
@@ -685,13 +689,13 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
         if (ch.p1_units) {
             if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(s1, h->ev_p2[c & 1], 0));
             if (serial) DMRGK_TRY(prof_begin(h, 0, s1, &slot));
-            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, s1));
+            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, s1, h->counters_dev + 2 * c, h->ctx->n_sm));
             if (serial) DMRGK_TRY(prof_end(h, slot, s1));
             DMRGK_CUDA(cudaEventRecord(h->ev_p1[c & 1], s1));
             DMRGK_CUDA(cudaStreamWaitEvent(s2, h->ev_p1[c & 1], 0));
         }
         if (serial && ch.p2_units) DMRGK_TRY(prof_begin(h, 1, s2, &slot));
-        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, s2));
+        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, s2, h->counters_dev + 2 * c + 1, h->ctx->n_sm));
         if (serial && ch.p2_units) DMRGK_TRY(prof_end(h, slot, s2));
         if (serial && ch.r_units) DMRGK_TRY(prof_begin(h, 2, s2, &slot));
         DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, s2));
