@@ -142,8 +142,9 @@ typedef struct dmrgk_heff_opts {
     int64_t ring_bytes;     /* staging ring for pinned operators, split in three parts
                                (0 = no ring: binding a pinned operator is then an error)     */
     int32_t kernel;         /* 0 = DMMA tensor-core kernel (product path),
-                               1 = scalar check kernel (same task lists; debugging aid)     */
-    int32_t split_waves;    /* phase-2 split-k target: units per CTA slot (0 = default 8)   */
+                               1 = scalar check kernel (same task lists; debugging aid),
+                               2, 3 = the DMMA kernel at other residencies (measurement aid)  */
+    int32_t split_waves;    /* phase-2 split-k target: units per CTA slot (0 = default 32)  */
     int32_t reserved[4];
 } dmrgk_heff_opts;
 

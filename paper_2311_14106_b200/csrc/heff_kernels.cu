@@ -23,8 +23,10 @@ namespace dmrgk {
 
 constexpr int BM = TILE_M, BN = TILE_N, BK = TILE_K;
 constexpr int NTHREADS = 128;           // 4 warps as 2×2, each a 32×32 warp tile = 4×4 DMMA frags
-constexpr int OPER_DOUBLES = BM * BK;    // 1024: one operand tile, dense 128-byte rows
-constexpr int STAGE_DOUBLES = 2 * OPER_DOUBLES;          // 16 KB per stage
+constexpr int KP = BK / 16;              // 16-column k-panels per k-tile
+constexpr int OPER_DOUBLES = BM * BK;    // one operand tile, dense 128-byte rows
+constexpr int STAGE_DOUBLES = 2 * OPER_DOUBLES;
+constexpr int MN_PANEL = BK * 16;        // doubles of one 16-column panel of an MN-major tile (BK k-rows)
 constexpr int smem_bytes(int stages) { return stages * STAGE_DOUBLES * 8; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
@@ -64,12 +66,13 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 
 // ---- consumer ----------------------------------------------------------------------------------
 // Shared image of an operand tile (doubles from the operand's origin in the stage):
-//   K-major  (stored [i][k]): element (i, k) at i·16 + (k xor ((i & 3) << 2))        [64 rows × 16]
-//   MN-major (stored [k][i]): element (i, k) at (i >> 4)·256 + k·16 + ((i & 15) xor ((k & 3) << 2))
-//                                                                    [4 panels × 16 k-rows × 16]
+//   K-major  (stored [i][k]): element (i, k) at (k >> 4)·1024 + i·16 + ((k & 15) xor ((i & 3) << 2))
+//                                                                    [BK/16 k-panels × 64 rows × 16]
+//   MN-major (stored [k][i]): element (i, k) at (i >> 4)·16·BK + k·16 + ((i & 15) xor ((k & 3) << 2))
+//                                                                    [4 panels × BK k-rows × 16]
 // A lane (g = lane >> 2, t4 = lane & 3) of fragment f reads row i = w·32 + f·8 + g at k = 4·ks + t4:
-//   K-major : k0 + f·128 + ((ks xor (g & 3)) << 2)           with k0 = (w·32 + g)·16 + t4
-//   MN-major: m[f & 1] + (f >> 1)·256 + ks·64                with m[h] = w·512 + t4·16 + ((8h + g) xor (t4 << 2))
+//   K-major : k0 + f·128 + (ks >> 2)·1024 + (((ks & 3) xor (g & 3)) << 2)    with k0 = (w·32 + g)·16 + t4
+//   MN-major: m[f & 1] + (f >> 1)·16·BK + ks·64     with m[h] = w·32·BK + t4·16 + ((8h + g) xor (t4 << 2))
 // In both cases the 16 lanes of a half-warp hit 16 distinct 8-byte banks.
 struct FragBase {
     int k0, m0, m1;
@@ -77,14 +80,14 @@ struct FragBase {
 __device__ __forceinline__ FragBase make_frag_base(int origin, int w, int g, int t4) {
     FragBase b;
     b.k0 = origin + (w * 32 + g) * 16 + t4;
-    b.m0 = origin + w * 512 + t4 * 16 + (g ^ (t4 << 2));
-    b.m1 = origin + w * 512 + t4 * 16 + ((8 + g) ^ (t4 << 2));
+    b.m0 = origin + w * 2 * MN_PANEL + t4 * 16 + (g ^ (t4 << 2));
+    b.m1 = origin + w * 2 * MN_PANEL + t4 * 16 + ((8 + g) ^ (t4 << 2));
     return b;
 }
 template <bool MN>
 __device__ __forceinline__ double frag(const double* __restrict__ st, const FragBase& b, int g3, int f, int ks) {
-    if (MN) return st[((f & 1) ? b.m1 : b.m0) + (f >> 1) * 256 + ks * 64];
-    return st[b.k0 + f * 128 + ((ks ^ g3) << 2)];
+    if (MN) return st[((f & 1) ? b.m1 : b.m0) + (f >> 1) * MN_PANEL + ks * 64];
+    return st[b.k0 + f * 128 + (ks >> 2) * 1024 + (((ks & 3) ^ g3) << 2)];
 }
 
 // One k-tile (BK = 16, `nks` steps of 4) of a warp tile of FM × FN fragments.  FM, FN and the operand
@@ -151,177 +154,8 @@ __device__ __forceinline__ void mma_layout(int nfm, int nfn, int nks, const doub
 // Per-stage note left by the producer for the consumers (published by the stage's full barrier).
 struct StageNote {
     uint32_t flags;   // segment flags (operand majors)
-    int32_t nks;      // k-steps of 4 that hold data in this k-tile (1..4)
+    int32_t nks;      // k-steps of 4 that hold data in this k-tile (1..BK/4)
 };
-
-template <int STAGES, int MIN_CTAS>
-__global__ void __launch_bounds__(NTHREADS, MIN_CTAS)
-heff_gemm_dmma_kernel(const Unit* __restrict__ units, const Seg* __restrict__ segs, Bases bases) {
-    extern __shared__ __align__(128) double smem[];
-    __shared__ __align__(8) unsigned long long bars[2 * STAGES];   // full[0..S), empty[S..2S)
-    __shared__ StageNote notes[STAGES];
-    const Unit u = units[blockIdx.x];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm = warp >> 1, wn = warp & 1;
-    const int g = lane >> 2, t4 = lane & 3, g3 = g & 3;
-    const uint32_t smem_base = smem_u32(smem), bar0 = smem_u32(bars);
-
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(bar0 + s * 8, 1);                   // full: the producer's arrive (+ the copies' bytes)
-            mbar_init(bar0 + (STAGES + s) * 8, 4);        // empty: one arrive per warp
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
-    }
-    __syncthreads();
-
-    // rows / columns of this tile that hold data, in 8-wide fragments, for this warp
-    const int rows_t = min(BM, u.mrows - u.i0);
-    const int cols_t = min(BN, u.ncols_st - u.j0);
-    const int cols_b = min(BN, u.ncols - u.j0);          // B-operand columns that exist
-    const int nfm = max(0, min(4, (rows_t - wm * 32 + 7) >> 3));
-    const int nfn = max(0, min(4, (cols_b - wn * 32 + 7) >> 3));
-    const bool busy = nfm > 0 && nfn > 0;
-    const FragBase fa = make_frag_base(0, wm, g, t4), fb = make_frag_base(OPER_DOUBLES, wn, g, t4);
-
-    double acc[4][4][2];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-    // ---- producer cursor (kept by every thread, uniform): the segment and k-offset of the next tile ----
-    // The descriptor of the FOLLOWING segment is loaded while the current one is being consumed, so a
-    // segment switch costs no memory latency (the host never emits a segment with klen = 0).
-    int p_seg = u.seg_begin, p_k0 = 0;
-    struct {
-        unsigned long long A, B;
-        int a_rp, b_rp, klen;
-        uint32_t flags;
-    } p_sg = {0ull, 0ull, 0, 0, 0, 0u};
-    int4 n_lo = make_int4(0, 0, 0, 0), n_hi = make_int4(0, 0, 0, 0);
-    auto prefetch_segment = [&](int idx) {
-        if (idx < u.seg_end) {
-            n_lo = __ldg(reinterpret_cast<const int4*>(segs + idx));          // A, B
-            n_hi = __ldg(reinterpret_cast<const int4*>(segs + idx) + 1);      // a_rp, b_rp, klen, flags
-        }
-    };
-    auto adopt_segment = [&]() {
-        p_sg.A = (unsigned long long)(unsigned)n_lo.x | ((unsigned long long)(unsigned)n_lo.y << 32);
-        p_sg.B = (unsigned long long)(unsigned)n_lo.z | ((unsigned long long)(unsigned)n_lo.w << 32);
-        p_sg.a_rp = n_hi.x;
-        p_sg.b_rp = n_hi.y;
-        p_sg.klen = n_hi.z;
-        p_sg.flags = uint32_t(n_hi.w);
-        p_k0 = 0;
-    };
-    prefetch_segment(p_seg);
-    adopt_segment();
-    prefetch_segment(p_seg + 1);
-    const int total = u.nkt;
-    const int rows_a = rows_t;                            // A-operand rows that exist in this tile
-    // Fetch tile `t` (the cursor's tile) into its stage; `wait_parity` < 0: the stage has never been used.
-    auto produce = [&](int t, int stage, int wait_parity) {
-        if (lane == 0 && warp == (t & 3)) {
-            const uint32_t full = bar0 + stage * 8;
-            if (wait_parity >= 0) mbar_wait(bar0 + (STAGES + stage) * 8, uint32_t(wait_parity));
-            const int nk = min(BK, p_sg.klen - p_k0), nk4 = (nk + 3) & ~3;
-            const bool am = (p_sg.flags & SEG_A_MMAJOR) != 0, bn = (p_sg.flags & SEG_B_NMAJOR) != 0;
-            const char* A = reinterpret_cast<const char*>(bases.b[(p_sg.flags >> SEG_A_SEL_SHIFT) & 3u] + p_sg.A);
-            const char* B = reinterpret_cast<const char*>(bases.b[(p_sg.flags >> SEG_B_SEL_SHIFT) & 3u] + p_sg.B);
-            const int npa = (rows_a + 15) >> 4, npb = (cols_b + 15) >> 4;
-            const uint32_t bytes_a = am ? uint32_t(npa * nk4 * 128) : uint32_t(rows_a * 128);
-            const uint32_t bytes_b = bn ? uint32_t(npb * nk4 * 128) : uint32_t(cols_b * 128);
-            notes[stage].flags = p_sg.flags;
-            notes[stage].nks = nk4 >> 2;
-            mbar_expect_tx(full, bytes_a + bytes_b);
-            const uint32_t dA = smem_base + stage * (STAGE_DOUBLES * 8), dB = dA + OPER_DOUBLES * 8;
-            if (!am) {
-                bulk_g2s(dA, A + (int64_t(p_k0 >> 4) * p_sg.a_rp + u.i0) * 128, bytes_a, full);
-            } else {
-                for (int pp = 0; pp < npa; ++pp)
-                    bulk_g2s(dA + pp * 2048, A + (int64_t((u.i0 >> 4) + pp) * p_sg.a_rp + p_k0) * 128, uint32_t(nk4 * 128), full);
-            }
-            if (!bn) {
-                bulk_g2s(dB, B + (int64_t(p_k0 >> 4) * p_sg.b_rp + u.j0) * 128, bytes_b, full);
-            } else {
-                for (int pp = 0; pp < npb; ++pp)
-                    bulk_g2s(dB + pp * 2048, B + (int64_t((u.j0 >> 4) + pp) * p_sg.b_rp + p_k0) * 128, uint32_t(nk4 * 128), full);
-            }
-        }
-        // advance the cursor (all threads)
-        p_k0 += BK;
-        if (p_k0 >= p_sg.klen) {
-            ++p_seg;
-            adopt_segment();
-            prefetch_segment(p_seg + 1);
-        }
-    };
-
-    // prologue: STAGES−1 tiles in flight
-#pragma unroll 1
-    for (int t = 0; t < STAGES - 1 && t < total; ++t) produce(t, t, -1);
-
-    int stage = 0, prev_stage = STAGES - 1;
-    uint32_t ph = 0, prev_ph = 0;
-#pragma unroll 1
-    for (int it = 0; it < total; ++it) {
-        // refill: tile it+STAGES−1 goes into the stage tile it−1 used; its consumers must be done
-        const int nt = it + STAGES - 1;
-        if (nt < total) produce(nt, prev_stage, it >= 1 ? int(prev_ph) : -1);
-        __syncwarp();
-        mbar_wait(bar0 + stage * 8, ph);
-        if (busy) {
-            const StageNote note = notes[stage];
-            const double* st = smem + stage * STAGE_DOUBLES;
-            switch (note.flags & (SEG_A_MMAJOR | SEG_B_NMAJOR)) {
-                case 0: mma_layout<false, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
-                case SEG_A_MMAJOR: mma_layout<true, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
-                case SEG_B_NMAJOR: mma_layout<false, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
-                default: mma_layout<true, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
-            }
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar0 + (STAGES + stage) * 8);
-        prev_stage = stage;
-        prev_ph = ph;
-        if (++stage == STAGES) {
-            stage = 0;
-            ph ^= 1u;
-        }
-    }
-
-    // epilogue: lane holds C[row g][cols 2·t4, 2·t4+1] of each 8×8 fragment
-    double* C = reinterpret_cast<double*>(bases.b[(u.mode >> UNIT_C_SEL_SHIFT) & 3u] + u.C);
-    const bool accum = (u.mode & UNIT_ACCUM) != 0, plain = (u.mode & UNIT_C_PLAIN) != 0;
-    // a panel-layout C block also gets its padding rows (up to rows_pad) written with zeros, so that it
-    // can be read MN-major later (padding rows take part in the last k-step of 4)
-    const int rows_st = plain ? rows_t : min(BM, u.c_rp - u.i0);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int r = wm * 32 + i * 8 + g;
-        if (r >= rows_st) continue;
-        const bool live = r < rows_t;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int c = wn * 32 + j * 8 + 2 * t4;
-            if (c >= cols_t) continue;
-            // (c, c+1) with c even stay adjacent under the 32-byte-group swizzle
-            double2* p = reinterpret_cast<double2*>(plain ? C + r * BN + c : C + panel_off(u.i0 + r, u.j0 + c, u.c_rp));
-            double2 v;
-            v.x = (live && u.j0 + c < u.ncols) ? u.alpha * acc[i][j][0] : 0.0;
-            v.y = (live && u.j0 + c + 1 < u.ncols) ? u.alpha * acc[i][j][1] : 0.0;
-            if (accum) {
-                double2 o = *p;
-                v.x += o.x;
-                v.y += o.y;
-            }
-            *p = v;
-        }
-    }
-}
-
 
 // ---- persistent, warp-specialised form (the product path) ------------------------------------------
 // grid = CTAS_PER_SM · n_SM CTAs of 5 warps.  Warp 4 is the PRODUCER: it claims work units from a
@@ -408,12 +242,11 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                 const bool am = (flags & SEG_A_MMAJOR) != 0, bn = (flags & SEG_B_NMAJOR) != 0;
                 const char* A = reinterpret_cast<const char*>(bases.b[(flags >> SEG_A_SEL_SHIFT) & 3u] + sA);
                 const char* B = reinterpret_cast<const char*>(bases.b[(flags >> SEG_B_SEL_SHIFT) & 3u] + sB);
-                const int na = am ? npa : 1, nb = bn ? npb : 1;      // copies of this segment's tiles
                 for (int k0 = 0; k0 < klen; k0 += BK) {
                     if (T >= STAGES) mbar_wait(bar0 + (STAGES + stage) * 8, eph);
-                    const int nk4 = (min(BK, klen - k0) + 3) & ~3;
-                    const uint32_t bytes_a = am ? uint32_t(npa * nk4 * 128) : uint32_t(rows_a * 128);
-                    const uint32_t bytes_b = bn ? uint32_t(npb * nk4 * 128) : uint32_t(cols_b * 128);
+                    const int nk = min(BK, klen - k0), nk4 = (nk + 3) & ~3, nkp = (nk + 15) >> 4;
+                    const uint32_t bytes_a = am ? uint32_t(npa * nk4 * 128) : uint32_t(nkp * rows_a * 128);
+                    const uint32_t bytes_b = bn ? uint32_t(npb * nk4 * 128) : uint32_t(nkp * cols_b * 128);
                     const uint32_t full = bar0 + stage * 8;
                     if (lane == 0) {
                         if (first) {
@@ -425,16 +258,25 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                         notes[stage].nks = nk4 >> 2;
                         mbar_expect_tx(full, bytes_a + bytes_b);
                     }
-                    __syncwarp();
-                    // lane l issues copy l: A copies first, then B copies (≤ 8 in all)
-                    const uint32_t dA = smem_base + stage * (STAGE_DOUBLES * 8), dB = dA + OPER_DOUBLES * 8;
-                    if (lane < na) {
-                        if (!am) bulk_g2s(dA, A + (int64_t(k0 >> 4) * a_rp + i0) * 128, bytes_a, full);
-                        else bulk_g2s(dA + lane * 2048, A + (int64_t((i0 >> 4) + lane) * a_rp + k0) * 128, uint32_t(nk4 * 128), full);
-                    } else if (lane < na + nb) {
-                        const int pp = lane - na;
-                        if (!bn) bulk_g2s(dB, B + (int64_t(k0 >> 4) * b_rp + j0) * 128, bytes_b, full);
-                        else bulk_g2s(dB + pp * 2048, B + (int64_t((j0 >> 4) + pp) * b_rp + k0) * 128, uint32_t(nk4 * 128), full);
+                    // copies of this tile: a K-major operand is BK/16 k-panels of (rows × 128 B), an MN-major
+                    // one is ceil(extent/16) panels of (nk4 × 128 B); the elected lane issues them one by one
+                    // (UBLKCP takes uniform operands, so spreading them over lanes would be serialised anyway)
+                    if (lane == 0) {
+                        const uint32_t dA = smem_base + stage * (STAGE_DOUBLES * 8), dB = dA + OPER_DOUBLES * 8;
+                        if (!am) {
+                            for (int kp = 0; kp < nkp; ++kp)
+                                bulk_g2s(dA + kp * 8192, A + (int64_t((k0 >> 4) + kp) * a_rp + i0) * 128, uint32_t(rows_a * 128), full);
+                        } else {
+                            for (int pp = 0; pp < npa; ++pp)
+                                bulk_g2s(dA + pp * (MN_PANEL * 8), A + (int64_t((i0 >> 4) + pp) * a_rp + k0) * 128, uint32_t(nk4 * 128), full);
+                        }
+                        if (!bn) {
+                            for (int kp = 0; kp < nkp; ++kp)
+                                bulk_g2s(dB + kp * 8192, B + (int64_t((k0 >> 4) + kp) * b_rp + j0) * 128, uint32_t(cols_b * 128), full);
+                        } else {
+                            for (int pp = 0; pp < npb; ++pp)
+                                bulk_g2s(dB + pp * (MN_PANEL * 8), B + (int64_t((j0 >> 4) + pp) * b_rp + k0) * 128, uint32_t(nk4 * 128), full);
+                        }
                     }
                     if (first) {
                         first = false;
@@ -637,9 +479,10 @@ heff_diag_kernel(const DiagBlock* __restrict__ blocks, const DiagTask* __restric
 static int g_gemm_ctas_per_sm = 0;
 int gemm_ctas_per_sm() { return g_gemm_ctas_per_sm; }
 
-// Kernel variants (dmrgk_heff_opts.kernel): 0 = product path (persistent, warp-specialised); 1 = scalar
-// check kernel; 2, 3 = other (stages, CTAs per SM) instantiations of the persistent kernel; 4 = the
-// one-unit-per-CTA kernel it replaced — all kept for measurement (profiles/).
+// Kernel variants (dmrgk_heff_opts.kernel): 0 = product path, 3 CTAs per SM with 64 KB of stages each;
+// 1 = scalar check kernel; 2 = 2 CTAs per SM with 96 KB of stages; 3 = 2 CTAs per SM with 64 KB — other
+// residencies of the same persistent kernel, kept for measurement (profiles/r2_tma_summary.md).
+constexpr int ST64 = 65536 / (STAGE_DOUBLES * 8), ST96 = 98304 / (STAGE_DOUBLES * 8);
 template <class K>
 static int32_t setup_kernel(K* fn, int threads, int stages, int min_ctas, int* resident) {
     DMRGK_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes(stages)));
@@ -655,10 +498,9 @@ static int32_t setup_kernel(K* fn, int threads, int stages, int min_ctas, int* r
 }
 
 int32_t gemm_kernel_setup() {
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<6, 2>, P_NTHREADS, 6, 2, &g_gemm_ctas_per_sm));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, 3>, P_NTHREADS, 4, 3, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, 2>, P_NTHREADS, 4, 2, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_kernel<3, 4>, NTHREADS, 3, 4, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<ST64, 3>, P_NTHREADS, ST64, 3, &g_gemm_ctas_per_sm));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<ST96, 2>, P_NTHREADS, ST96, 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<ST64, 2>, P_NTHREADS, ST64, 2, nullptr));
     return DMRGK_OK;
 }
 
@@ -666,16 +508,14 @@ int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev
                           const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm) {
     if (n_units <= 0) return DMRGK_OK;
     if (n_units > 0x7fffffffLL) return fail(DMRGK_EINVAL, "too many work units in one launch: %lld", (long long)n_units);
-    const unsigned grid = unsigned(n_units);
     const int nu = int(n_units);
     auto pgrid = [&](int ctas) { return unsigned(std::min<int64_t>(n_units, int64_t(n_sm) * ctas)); };
-    if (kernel != 1 && kernel != 4 && !counter_dev) return fail(DMRGK_EINVAL, "launch_gemm_units: the persistent kernel needs a queue counter");
+    if (kernel != 1 && !counter_dev) return fail(DMRGK_EINVAL, "launch_gemm_units: the persistent kernel needs a queue counter");
     switch (kernel) {
-        case 1: heff_gemm_scalar_kernel<<<grid, NTHREADS, 0, st>>>(units_dev, segs_dev, bases); break;
-        case 2: heff_gemm_dmma_persistent_kernel<4, 3><<<pgrid(3), P_NTHREADS, smem_bytes(4), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        case 3: heff_gemm_dmma_persistent_kernel<4, 2><<<pgrid(2), P_NTHREADS, smem_bytes(4), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        case 4: heff_gemm_dmma_kernel<3, 4><<<grid, NTHREADS, smem_bytes(3), st>>>(units_dev, segs_dev, bases); break;
-        default: heff_gemm_dmma_persistent_kernel<6, 2><<<pgrid(2), P_NTHREADS, smem_bytes(6), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 1: heff_gemm_scalar_kernel<<<unsigned(n_units), NTHREADS, 0, st>>>(units_dev, segs_dev, bases); break;
+        case 2: heff_gemm_dmma_persistent_kernel<ST96, 2><<<pgrid(2), P_NTHREADS, smem_bytes(ST96), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 3: heff_gemm_dmma_persistent_kernel<ST64, 2><<<pgrid(2), P_NTHREADS, smem_bytes(ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        default: heff_gemm_dmma_persistent_kernel<ST64, 3><<<pgrid(3), P_NTHREADS, smem_bytes(ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
     }
     count_launch();
     DMRGK_CUDA(cudaGetLastError());

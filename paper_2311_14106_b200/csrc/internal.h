@@ -188,7 +188,7 @@ struct DiagBlock {
 };
 
 constexpr int TILE_M = 64, TILE_N = 64;
-constexpr int TILE_K = 16;   // contraction depth of one pipeline stage (k-tile); Unit::nkt counts these
+constexpr int TILE_K = 32;   // contraction depth of one pipeline stage (k-tile); Unit::nkt counts these
 
 // kernel launchers (heff_kernels.cu)
 // `counter_dev`: a zeroed int the persistent kernel uses as its unit queue head (one per launch in flight)

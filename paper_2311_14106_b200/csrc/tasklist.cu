@@ -89,8 +89,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     dmrgk_heff_opts o;
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
-    if (o.split_waves <= 0) o.split_waves = 8;
-    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 4))
+    if (o.split_waves <= 0) o.split_waves = 32;   // units per CTA slot: the queue's tail is ≈ one unit long
+    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 3))
         return fail(DMRGK_EINVAL, "heff_create: bad options");
     const int64_t ring_part = (o.ring_bytes / 3) / 128 * 128;   // three parts: see dmrgk_heff_apply
 
