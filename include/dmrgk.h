@@ -296,6 +296,33 @@ int32_t dmrgk_renorm_query(const dmrgk_renorm* plan, int64_t* n_tasks, double* f
  * the call and joined back into `stream` (two library-owned streams overlap the two phases). */
 int32_t dmrgk_renorm_apply(dmrgk_renorm* plan, void* workspace_dev, void* stream);
 
+/* ---- block enlargement (second half; "Ren_l") -------------
+ * The next bond's enlarged block is A′ = (kept block) ⊗ (site).  Every operator on A′ is a sum of products
+ *        O_{A′} = Σ_j coef_j · (X_j · P^{π_j}) ⊗ y_j ,
+ * X_j a stored operator on the KEPT space (its transpose when flag bit 0 is set; the identity when
+ * t_x[j] is NULL), y_j a d×d site operator (row-major, t_y[j·d·d …]), P = (−1)^N on the kept column index,
+ * π_j = flag bit 1 (set when the site factor is fermionic: the site's Jordan–Wigner string runs over the
+ * block).  Which products make up which operator — the complementary-operator sums over t and V — is
+ * host bookkeeping (paper_2311_14106_b200/blockops.py: "complementary operators built on the host").
+ *
+ * `enlarged` must be the sector-major product space: sector q′ holds, in the order of the kept space's
+ * sectors, every kept sector k for which q′ − q_k is the charge of a site state; site_charges is
+ * [d][n_charges], all distinct.  out[i] live on `enlarged` and are bound to DEVICE arenas, which
+ * dmrgk_enlarge_apply overwrites completely (zero fill, then every sub-block once — contributions are
+ * grouped by destination, no atomics).  Errors: DMRGK_ESHAPE (spaces / sector dimensions inconsistent),
+ * DMRGK_ECHARGE (shift or parity of a product does not match its target), DMRGK_ESTATE (unbound), DMRGK_EINVAL. */
+typedef struct dmrgk_enlarge dmrgk_enlarge;
+int32_t dmrgk_enlarge_create(dmrgk_ctx* ctx, const dmrgk_space* kept, const dmrgk_space* enlarged, int32_t d,
+                             const int32_t* site_charges, int64_t n_out, dmrgk_op* const* out,
+                             int64_t n_terms, const int32_t* t_out, dmrgk_op* const* t_x,
+                             const uint32_t* t_flags, const double* t_coef, const double* t_y,
+                             dmrgk_enlarge** plan);
+void dmrgk_enlarge_destroy(dmrgk_enlarge* plan);
+/* n_tiles: 32×32 destination tiles; n_sources: (sub-block, source) pairs; bytes = 8·elements moved. */
+int32_t dmrgk_enlarge_query(const dmrgk_enlarge* plan, int64_t* n_tiles, int64_t* n_sources,
+                            int64_t* bytes_read, int64_t* bytes_written);
+int32_t dmrgk_enlarge_apply(dmrgk_enlarge* plan, void* stream);
+
 /* ---- harness kernels (outside the hot path): seeded inputs and FP64 pipe probes ----------- */
 /* Counter-based values, bit-identical to workloads/rng.py normal12(seed, stream, index): fills the
  * packed arena of an operator / a ψ layout from the UNPADDED element index of each entry, times

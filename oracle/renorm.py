@@ -63,3 +63,54 @@ def flops(op, phi):
             n_r, n_c = by_enl[ri][1], by_enl[ci][1]
             total += 2 * e_r * e_c * n_c + 2 * n_r * e_r * n_c
     return total
+
+
+# ----------------------------------------------------------------------------
+# Enlarging a block by a site (the other half of the renormalisation step)
+# ----------------------------------------------------------------------------
+# After the kept basis Φ has been applied, the next bond's enlarged block is A′ = (kept block) ⊗ (site).
+# With the block's modes preceding the site's in the Jordan–Wigner string, a block operator x acts as
+# x̃ ⊗ 1 and a site operator y as P^{π(y)} ⊗ ỹ, P = (−1)^{N_block}, so a product "block operator left of
+# site operator" is (x̃ · P^π) ⊗ ỹ — the rule of SURVEY.md §8.0 with the site in the role of B.  Every
+# operator the next bond needs on A′ is a sum of such products,
+#
+#       O_enl = Σ_j coef_j · (X_j · P^{π_j}) ⊗ y_j ,
+#
+# and by definition it equals Φ_{A′}† O Φ_{A′} with Φ_{A′} = Φ_kept ⊗ 1_site ("renormalized
+# block operators"; PAPER.md:142 Ren_l / Ren_r).  `enlarge_dense` is the sum written out with explicit
+# Kronecker products in the sector-major basis of A′; tests/test_oracle_enlarge.py pins it (and the
+# product lists of the library's host builder) against the definition built from Fock-space matrices.
+def enlarged_order(sectors_K, site_charges):
+    """Sector-major ordering of the product basis |l⟩⊗|σ⟩ (l major): returns (perm, sectors_E) with
+    perm[new index] = l·d + σ, charges ascending lexicographically, stable inside a sector — the
+    ordering oracle.dmrg.sector_major gives kron_basis(left, site)."""
+    qs = []
+    for q, dim in sectors_K:
+        qs += [tuple(q)] * dim
+    d = len(site_charges)
+    keys = [tuple(a + b for a, b in zip(ql, tuple(site_charges[s]))) for ql in qs for s in range(d)]
+    perm = sorted(range(len(keys)), key=lambda i: (keys[i], i))
+    sectors = []
+    for i in perm:
+        if sectors and sectors[-1][0] == keys[i]:
+            sectors[-1][1] += 1
+        else:
+            sectors.append([keys[i], 1])
+    return np.array(perm), [(k, n) for k, n in sectors]
+
+
+def enlarge_dense(terms, sectors_K, site_charges):
+    """Σ_j coef_j · kron(X_j P^{π_j}, y_j), rows and columns in the sector-major order of A′.
+
+    terms: [(X dense M_K×M_K or None for the identity, y dense d×d, coef, π)], π = 1 if y is odd."""
+    M = sum(dim for _, dim in sectors_K)
+    d = len(site_charges)
+    par = np.concatenate([np.full(dim, 1.0 - 2.0 * (int(sum(q)) % 2)) for q, dim in sectors_K]) if M else np.zeros(0)
+    O = np.zeros((M * d, M * d))
+    for X, y, coef, pi in terms:
+        Xd = np.eye(M) if X is None else np.asarray(X, dtype=np.float64)
+        if pi:
+            Xd = Xd * par[None, :]
+        O += coef * np.kron(Xd, np.asarray(y, dtype=np.float64))
+    perm, _ = enlarged_order(sectors_K, site_charges)
+    return O[np.ix_(perm, perm)]

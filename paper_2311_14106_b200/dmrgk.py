@@ -86,6 +86,10 @@ SIGNATURES = {
     "dmrgk_renorm_destroy": (None, [_p]),
     "dmrgk_renorm_query": (_i32, [_p, _pi64, _pf64, _pi64, _pi64]),
     "dmrgk_renorm_apply": (_i32, [_p, _p, _p]),
+    "dmrgk_enlarge_create": (_i32, [_p, _p, _p, _i32, _p, _i64, _p, _i64, _p, _p, _p, _p, _p, _pp]),
+    "dmrgk_enlarge_destroy": (None, [_p]),
+    "dmrgk_enlarge_query": (_i32, [_p, _pi64, _pi64, _pi64, _pi64]),
+    "dmrgk_enlarge_apply": (_i32, [_p, _p]),
     "dmrgk_vec_scratch_bytes": (_i64, [_i32]),
     "dmrgk_vec_multi_dot": (_i32, [_p, _i64, _i32, _p, _i64, _p, _p, _p, _p]),
     "dmrgk_vec_multi_axpy": (_i32, [_p, _i64, _i32, _p, _i64, _p, _f64, _f64, _p, _p]),
@@ -300,6 +304,45 @@ class Op(_Blocked):
     def __del__(self):
         if getattr(self, "h", None):
             self.lib.dmrgk_op_destroy(self.h)
+            self.h = None
+
+
+class Enlarge:
+    """dmrgk_enlarge: out[i] = Σ_j coef_j (X_j P^π_j) ⊗ y_j.
+    terms = [(index into out_ops, X Op or None, transposed, site_odd, coef, y (d×d array))]."""
+
+    def __init__(self, ctx, kept, enlarged, site_charges, out_ops, terms):
+        self.lib, self.ctx = ctx.lib, ctx
+        sc = np.ascontiguousarray(site_charges, dtype=np.int32).reshape(len(site_charges), -1)
+        d = sc.shape[0]
+        n_out, n_terms = len(out_ops), len(terms)
+        oarr = (C.c_void_p * max(n_out, 1))(*[o.h for o in out_ops])
+        xarr = (C.c_void_p * max(n_terms, 1))()
+        t_out = np.zeros(max(n_terms, 1), np.int32)
+        t_flags = np.zeros(max(n_terms, 1), np.uint32)
+        t_coef = np.zeros(max(n_terms, 1), np.float64)
+        t_y = np.zeros((max(n_terms, 1), d, d), np.float64)
+        for j, (o, X, trans, odd, coef, y) in enumerate(terms):
+            t_out[j], t_coef[j] = o, coef
+            xarr[j] = X.h if X is not None else None
+            t_flags[j] = (1 if trans else 0) | (2 if odd else 0)
+            t_y[j] = np.asarray(y, dtype=np.float64)
+        self._keep = (out_ops, [t[1] for t in terms], kept, enlarged)
+        h = C.c_void_p()
+        check(self.lib.dmrgk_enlarge_create(ctx.h, kept.h, enlarged.h, d, sc.ctypes.data, n_out, oarr, n_terms,
+                                            t_out.ctypes.data, xarr, t_flags.ctypes.data, t_coef.ctypes.data,
+                                            t_y.ctypes.data, C.byref(h)))
+        self.h = h
+        a, b, c_, d_ = (C.c_int64() for _ in range(4))
+        check(self.lib.dmrgk_enlarge_query(self.h, C.byref(a), C.byref(b), C.byref(c_), C.byref(d_)))
+        self.n_tiles, self.n_sources, self.bytes_read, self.bytes_written = a.value, b.value, c_.value, d_.value
+
+    def apply(self, stream=None):
+        check(self.lib.dmrgk_enlarge_apply(self.h, _stream(stream)))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.dmrgk_enlarge_destroy(self.h)
             self.h = None
 
 
