@@ -605,6 +605,98 @@ def run_renorm(args):
     print(json.dumps(out), flush=True)
 
 
+def run_enlarge(args):
+    """--op enlarge: one step = forming every operator of the next enlarged left block,
+    O_A' = sum_j coef_j (X_j P^pi) (x) y_j (second half), from kept operators with the
+    sector structure of config 4 at D = 4096 kept states and a Hubbard site; 4 block sites (8 modes) + 1 site
+    + 13 sites to the right, synthetic symmetric t, V (seeded).  HBM-bound: its own metric (GB/s)."""
+    import numpy as np
+    import torch
+    import workloads as wlmod
+    from workloads.rng import normal12
+    from paper_2311_14106_b200 import dmrgk, blockops
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    wl = make_workload("4")
+    sectors_K, _ = wlmod.renorm_basis(wl)
+    n_modes, nA = 36, 8
+    mc = np.array([(1, 0), (0, 1)] * (n_modes // 2), dtype=np.int64)
+    A, S, right = list(range(nA)), [nA, nA + 1], list(range(nA + 2, n_modes))
+    g = normal12(11, 1, np.arange(n_modes * n_modes)).reshape(n_modes, n_modes)
+    T = 0.5 * (g + g.T)
+    G = normal12(11, 2, np.arange(n_modes ** 4)).reshape((n_modes,) * 4) * 0.1
+    V = G + G.transpose(3, 2, 1, 0)
+    # keep only charge-conserving coefficients (n_up, n_down are conserved by Eq. (1) of the Hubbard-type models)
+    up = mc[:, 0]
+    T = T * (up[:, None] == up[None, :])
+    V = V * ((up[:, None, None, None] + up[None, :, None, None]) == (up[None, None, :, None] + up[None, None, None, :]))
+    t0 = time.perf_counter()
+    site, lists = blockops.enlarge_left_lists(T, V, mc, A, S, right)
+    t_lists = time.perf_counter() - t0
+    ctx = dmrgk.Ctx(0)
+    st = torch.cuda.current_stream()
+    sp_K = dmrgk.Space(ctx, 2, sectors_K)
+    sectors_E = blockops.enlarged_sectors(sectors_K, site.charges.tolist())
+    sp_E = dmrgk.Space(ctx, 2, sectors_E)
+    keys_A, keys_Ap = blockops.left_block_keys(A, S + right), blockops.left_block_keys(A + S, right)
+
+    def alloc(space, keys):
+        ops = [dmrgk.Op(ctx, space, *blockops.operator_spec(k, mc)) for k in keys]
+        arena = torch.zeros(max(sum(o.n_padded for o in ops), 16), dtype=torch.float64, device=dev)
+        o = 0
+        for op in ops:
+            op.bind_device(arena[o:o + op.n_padded] if op.n_padded else arena[0:16])
+            o += op.n_padded
+        return ops, arena
+
+    ops_K, arena_K = alloc(sp_K, keys_A)
+    o = 0
+    for i, op in enumerate(ops_K):
+        if op.n_padded:
+            op.fill_normal(arena_K[o:o + op.n_padded], 11, 100 + i, 1, 0, st)
+        o += op.n_padded
+    ops_E, arena_E = alloc(sp_E, keys_Ap)
+    index_K = {k: i for i, k in enumerate(keys_A)}
+    terms = [(oi, None if k is None else ops_K[index_K[k]], tr, bool(pi), 1.0, y)
+             for oi, key in enumerate(keys_Ap) for (k, tr, y, pi) in lists[key]]
+    t0 = time.perf_counter()
+    enl = dmrgk.Enlarge(ctx, sp_K, sp_E, site.charges, ops_E, terms)
+    t_plan = time.perf_counter() - t0
+    for _ in range(args.warmup):
+        enl.apply(st)
+    clocks = ClockSampler(0)
+    clocks.start()
+    dmrgk.launch_count(reset=True)
+    ms = timed(st, lambda: enl.apply(st), reps=args.steps) / args.steps
+    launches = dmrgk.launch_count()
+    clk = clocks.stop()
+    zero_bytes = int(arena_E.numel() * 8)
+    # algorithmic HBM bytes: every kept operator read once, every formed operator written once (its zero
+    # blocks included).  The gather reads each kept block once PER PRODUCT (enl.bytes_read, served by L2:
+    # the kept set is small), so that figure is reported as L2-level traffic, not as HBM work.
+    kept_bytes = int(arena_K.numel() * 8)
+    moved = kept_bytes + zero_bytes
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        src = "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        hbm_peak, src = 6650.0, "fallback (B200_PROFILING.md)"
+    gbs = moved / ms / 1e6
+    print(json.dumps({
+        "metric": "enlarge_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "enlarge_left_block_config4_sectors_D4096_hubbard_site", "kept_states": sum(d for _, d in sectors_K),
+                   "enlarged_states": sum(d for _, d in sectors_E), "kept_operators": len(ops_K), "formed_operators": len(ops_E),
+                   "products": len(terms), "tiles": enl.n_tiles, "sources": enl.n_sources, "kept_bytes": kept_bytes,
+                   "formed_bytes": zero_bytes, "gather_reads_l2_bytes": enl.bytes_read, "gather_writes_bytes": enl.bytes_written,
+                   "l2_read_gbs": enl.bytes_read / ms / 1e6, "host_lists_s": round(t_lists, 3),
+                   "host_plan_s": round(t_plan, 3), "l2": "formed operators (>> 126 MB L2) are written once per step"},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "kernel": "enlarge_gather_kernel (+ zero fill)", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
+                     "frac": gbs / hbm_peak, "peak_source": src, "traffic": None},
+        "clocks": clk}), flush=True)
+
+
 def run_loop_probe(args):
     """--op loop_probe: the k-tile-loop skeletons of csrc/probe_gemm.cu (harness, not the product path)
     and the register-only pipe probes in all shapes — the ceilings design decisions are judged against."""
@@ -658,13 +750,15 @@ def main():
     ap.add_argument("--shard", default="none", choices=["none", "k"],
                     help="N > 1 only: 'none' = independent replicas (the scope of BASELINE.json), 'k' = split the operator-pair "
                          "list over the ranks and all-reduce sigma (SURVEY §8(f) NEXT-2)")
-    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "loop_probe"],
+    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "enlarge", "loop_probe"],
                     help="davidson (default, the headline hot path) or renorm (NEXT-1 row, its own metric)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
     elif args.op == "renorm":
         run_renorm(args)
+    elif args.op == "enlarge":
+        run_enlarge(args)
     elif args.op == "loop_probe":
         run_loop_probe(args)
     else:

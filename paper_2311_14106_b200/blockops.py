@@ -128,6 +128,19 @@ class _Accumulator:
         return [(key, trans, y, pi) for (key, trans, pi), y in self.groups.items() if np.any(y)]
 
 
+def enlarged_sectors(sectors_K, site_charges):
+    """Sector list [(charge, dim)] of kept ⊗ site, charges ascending; dim = Σ over the kept sectors k with
+    q′ − q_k a site charge (the sector-major product space dmrgk_enlarge expects)."""
+    dims = {}
+    for q, dim in sectors_K:
+        if dim <= 0:
+            continue
+        for sq in site_charges:
+            key = tuple(int(a) + int(b) for a, b in zip(q, sq))
+            dims[key] = dims.get(key, 0) + dim
+    return [(k, dims[k]) for k in sorted(dims)]
+
+
 def left_block_keys(A, right):
     """Keys of the operator set the left block A carries when the modes `right` lie to its right."""
     A = list(A)
