@@ -131,7 +131,11 @@ enum {
     DMRGK_TRANS_L = 1u, /* apply the transpose of the stored L operator (h.c. partner)  */
     DMRGK_TRANS_R = 2u, /* apply the transpose of the stored R operator                 */
     DMRGK_IDENT_L = 4u, /* L is the identity on A (L[k] must be NULL)                   */
-    DMRGK_IDENT_R = 8u  /* R is the identity on B (R[k] must be NULL)                   */
+    DMRGK_IDENT_R = 8u, /* R is the identity on B (R[k] must be NULL)                   */
+    DMRGK_HC_OF_PREV = 16u /* pair k is the Hermitian conjugate of pair k−1: L[k], R[k] are ignored (may
+                           be NULL) and the stored operators of pair k−1 are applied transposed
+                           (its TRANS flags toggled, its IDENT flags kept); coef[k] is the caller's —
+                           −coef[k−1] for a fermionic (odd) pair, +coef[k−1] for an even one */
 };
 
 typedef struct dmrgk_heff_opts {
@@ -145,7 +149,10 @@ typedef struct dmrgk_heff_opts {
                                1 = scalar check kernel (same task lists; debugging aid),
                                2, 3 = the DMMA kernel at other residencies (measurement aid)  */
     int32_t split_waves;    /* phase-2 split-k target: units per CTA slot (0 = default 32)  */
-    int32_t reserved[4];
+    int32_t order_policy;   /* GEMM order per task: 0 = the cheaper of (Lψ)Rᵀ and
+                               L(ψRᵀ) by flop count, 1 = always (Lψ)Rᵀ, 2 = always L(ψRᵀ); tasks
+                               with an identity factor are a single product either way            */
+    int32_t reserved[3];
 } dmrgk_heff_opts;
 
 /* Builds the task list of σ = Σ_k coef[k] (L[k] ⊗ R[k]) ψ for the given layout: enumerates
@@ -160,7 +167,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                           const uint32_t* flags, const dmrgk_heff_opts* opts, dmrgk_heff** out);
 void dmrgk_heff_destroy(dmrgk_heff* h);
 /* flops_alg = Σ_tasks min(2m′n(m+n′), 2mn′(n+m′)) (identity factor → one product),
- * flops_exec = flops the kernels actually issue for useful elements (L-first order),
+ * flops_exec = flops of the products the kernels execute in the chosen GEMM order (= flops_alg with
+ * order_policy 0),
  * op_bytes = 8·Σ_tasks (m′m + n′n), workspace_bytes = what heff_apply needs (128-B aligned). */
 int32_t dmrgk_heff_query(const dmrgk_heff* h, int64_t* n_tasks, double* flops_alg,
                          double* flops_exec, int64_t* op_bytes, int64_t* workspace_bytes,
@@ -193,7 +201,12 @@ int32_t dmrgk_heff_diag(dmrgk_heff* h, double* diag_dev, void* workspace_dev, vo
 int32_t dmrgk_heff_profile(dmrgk_heff* h, int32_t enable);
 int32_t dmrgk_heff_profile_read(dmrgk_heff* h, double* ms, int64_t* launches);
 
-/* ---- a8: vector kernels over the flat padded arena (n doubles) ---------------------------- */
+/* ---- a8: vector kernels over the flat padded arena (n doubles) ----------------------------
+ * The iterative diagonalisation of H_eff ("Lánczos or Davidson", §II.A, thresholds
+ * ε_Davidson of PAPER.md:114, 118) needs, besides σ = H_eff ψ, only BLAS-1 work on ψ-sized vectors: the
+ * Rayleigh-matrix dots, the Ritz vector and residual, the diagonal preconditioner and the
+ * Gram–Schmidt passes (SURVEY §8(a) a8, §8(c) "Davidson, step by step").  Fused multi-vector forms
+ * first (what the driver uses), the plain BLAS-1 names of SURVEY §8(b) after them. */
 /* Reductions are two-stage and fixed-order (bit-reproducible); scratch_dev needs
  * dmrgk_vec_scratch_bytes(nv) bytes; results land in out_dev[nv] (device) — asynchronous. */
 int64_t dmrgk_vec_scratch_bytes(int32_t nv);
@@ -213,6 +226,15 @@ int32_t dmrgk_vec_axpby(dmrgk_ctx* ctx, int64_t n, double alpha, const double* x
  * 3: f = 1/sqrt(a)  (normalisation by a squared norm without a host round trip).  y may alias x. */
 int32_t dmrgk_vec_scal_dev(dmrgk_ctx* ctx, int64_t n, const double* alpha_dev, int32_t mode,
                            const double* x_dev, double* y_dev, void* stream);
+/* out[0] = x·y ;  out[0] = ‖x‖₂ ;  y += alpha·x ;  x *= alpha  (host scalars; dot / nrm2 results land in
+ * device memory like multi_dot's, scratch as for nv = 1). */
+int32_t dmrgk_vec_dot(dmrgk_ctx* ctx, int64_t n, const double* x_dev, const double* y_dev,
+                      double* out_dev, void* scratch_dev, void* stream);
+int32_t dmrgk_vec_nrm2(dmrgk_ctx* ctx, int64_t n, const double* x_dev, double* out_dev,
+                       void* scratch_dev, void* stream);
+int32_t dmrgk_vec_axpy(dmrgk_ctx* ctx, int64_t n, double alpha, const double* x_dev, double* y_dev,
+                       void* stream);
+int32_t dmrgk_vec_scal(dmrgk_ctx* ctx, int64_t n, double alpha, double* x_dev, void* stream);
 /* Davidson residual and correction (SURVEY §8(c) "Davidson, step by step"):
  *   r = Σ_j y[j]·(W_j − θ V_j);  out[0] = ‖r‖²  (y, θ from device: coef_dev[0..m) = y, coef_dev[m] = θ) */
 int32_t dmrgk_vec_residual(dmrgk_ctx* ctx, int64_t n, int32_t m, const double* V_dev,

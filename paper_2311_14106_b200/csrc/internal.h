@@ -136,6 +136,8 @@ struct Bases {
 enum : uint32_t {
     SEG_A_MMAJOR = 1u,
     SEG_B_NMAJOR = 2u,
+    SEG_A_TBUF = 4u,       // host only: A is the phase-1 intermediate (offset into the T buffer of its chunk)
+    SEG_B_TBUF = 8u,       // host only: B is the phase-1 intermediate
     SEG_A_SEL_SHIFT = 4,   // bits 4-5: base selector of A
     SEG_B_SEL_SHIFT = 6    // bits 6-7: base selector of B
 };
@@ -240,7 +242,7 @@ struct dmrgk_heff {
     dmrgk_ctx* ctx;
     const dmrgk_layout* layout;
     dmrgk_heff_opts opts;
-    int64_t n_tasks = 0;
+    int64_t n_tasks = 0, n_rfirst = 0;
     double flops_alg = 0, flops_exec = 0;
     int64_t op_bytes = 0;
     int64_t t_bytes = 0, partial_bytes = 0, ring_bytes = 0, ring_part_bytes = 0, workspace_bytes = 0;

@@ -23,9 +23,18 @@ struct Task {
     int32_t k;
     int32_t ib, ob;          // input / output ψ block
     int32_t mo, m, n, no;    // m′, m, n, n′
-    Seg s1, s2;              // phase-1 / phase-2 segment templates (A of s2 filled per chunk)
+    Seg s1, s2;              // phase-1 / phase-2 segment templates (the intermediate's offset is set per chunk)
     double alpha;
     bool diag;
+    bool rfirst;             // GEMM order: false (L ψ) Rᵀ, true L (ψ Rᵀ)
+    int32_t t_rows, t_cols, t_ld;   // shape of the phase-1 intermediate (m′ × n, or m × n′ when rfirst)
+    // where the L / R operand of the pair sits in the two segments
+    unsigned long long& Laddr() { return rfirst ? s2.A : s1.A; }
+    unsigned long long& Raddr() { return rfirst ? s1.B : s2.B; }
+    int32_t Lrp() const { return rfirst ? s2.a_rp : s1.a_rp; }
+    int32_t Rrp() const { return rfirst ? s1.b_rp : s2.b_rp; }
+    uint32_t Lsel() const { return ((rfirst ? s2.flags : s1.flags) >> SEG_A_SEL_SHIFT) & 3u; }
+    uint32_t Rsel() const { return ((rfirst ? s1.flags : s2.flags) >> SEG_B_SEL_SHIFT) & 3u; }
 };
 
 struct OpRef {               // where an operator block lives
@@ -78,19 +87,42 @@ void dmrgk_heff_destroy(dmrgk_heff* h) {
 }
 
 int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
-                          dmrgk_op* const* L, dmrgk_op* const* R, const double* coef,
-                          const uint32_t* flags, const dmrgk_heff_opts* opts, dmrgk_heff** out) {
+                          dmrgk_op* const* L_in, dmrgk_op* const* R_in, const double* coef,
+                          const uint32_t* flags_in, const dmrgk_heff_opts* opts, dmrgk_heff** out) {
     if (!out) return fail(DMRGK_EINVAL, "heff_create: out is NULL");
     *out = nullptr;
     if (!ctx || !layout) return fail(DMRGK_EINVAL, "heff_create: NULL ctx or layout");
-    if (K < 0 || (K > 0 && (!L || !R || !coef || !flags)))
+    if (K < 0 || (K > 0 && (!L_in || !R_in || !coef || !flags_in)))
         return fail(DMRGK_EINVAL, "heff_create: bad pair arrays (K = %lld)", (long long)K);
+    // DMRGK_HC_OF_PREV: pair k re-uses the stored operators of pair k−1, applied transposed
+    std::vector<dmrgk_op*> Lv(static_cast<size_t>(K)), Rv(static_cast<size_t>(K));
+    std::vector<uint32_t> fv(static_cast<size_t>(K));
+    for (int64_t k = 0; k < K; ++k) {
+        if (flags_in[k] & DMRGK_HC_OF_PREV) {
+            if (k == 0) return fail(DMRGK_EINVAL, "heff_create: pair 0 cannot be the h.c. of a previous pair");
+            if (flags_in[k] & ~uint32_t(DMRGK_HC_OF_PREV))
+                return fail(DMRGK_EINVAL, "heff_create: pair %lld: HC_OF_PREV excludes the other flags", (long long)k);
+            Lv[k] = Lv[k - 1];
+            Rv[k] = Rv[k - 1];
+            uint32_t f = fv[k - 1];
+            if (Lv[k]) f ^= DMRGK_TRANS_L;
+            if (Rv[k]) f ^= DMRGK_TRANS_R;
+            fv[k] = f;
+        } else {
+            Lv[k] = L_in[k];
+            Rv[k] = R_in[k];
+            fv[k] = flags_in[k];
+        }
+    }
+    dmrgk_op* const* L = Lv.data();
+    dmrgk_op* const* R = Rv.data();
+    const uint32_t* flags = fv.data();
     DMRGK_CUDA(cudaSetDevice(ctx->device));
     dmrgk_heff_opts o;
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
     if (o.split_waves <= 0) o.split_waves = 32;   // units per CTA slot: the queue's tail is ≈ one unit long
-    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 3))
+    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 3) || o.order_policy < 0 || o.order_policy > 2)
         return fail(DMRGK_EINVAL, "heff_create: bad options");
     const int64_t ring_part = (o.ring_bytes / 3) / 128 * 128;   // three parts: see dmrgk_heff_apply
 
@@ -235,8 +267,39 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             t.s1.flags |= SEG_B_NMAJOR | (BASE_PSI << SEG_B_SEL_SHIFT);
             t.s2.a_rp = pad_rows(t.mo);                     // T_t is a block (m′ × n) in the panel layout
             t.s2.klen = t.n;
-            t.s2.flags |= BASE_WS << SEG_A_SEL_SHIFT;
-            tb += int64_t(pad_rows(t.mo)) * pb[ib].ld * 8;
+            t.s2.flags |= SEG_A_TBUF | (BASE_WS << SEG_A_SEL_SHIFT);
+            t.t_rows = t.mo;
+            t.t_cols = t.n;
+            t.t_ld = pb[ib].ld;
+            // GEMM order: (L ψ) Rᵀ costs 2m′n(m + n′), L (ψ Rᵀ) costs 2mn′(n + m′)
+            if (L[k] && R[k]) {
+                const double cl = 2.0 * t.mo * t.n * (double(t.m) + t.no), cr = 2.0 * t.m * t.no * (double(t.n) + t.mo);
+                t.rfirst = o.order_policy == 2 || (o.order_policy == 0 && cr < cl);
+            }
+            if (t.rfirst) {
+                // phase 1: U = c·s · ψ[a,b] Rapp[b′,b]ᵀ (m × n′);  phase 2: σ[a′,b′] += Lapp[a′,a] U[a,b′]
+                Seg p1, p2;
+                memset(&p1, 0, sizeof(p1));
+                memset(&p2, 0, sizeof(p2));
+                p1.A = (unsigned long long)(pb[ib].off * 8);            // ψ block, K-major (stored [a][b])
+                p1.a_rp = pb[ib].rows_pad;
+                p1.B = t.s2.B;                                          // R: K-major stored [b′][b], N-major if transposed
+                p1.b_rp = t.s2.b_rp;
+                p1.klen = t.n;
+                p1.flags = (BASE_PSI << SEG_A_SEL_SHIFT) | (t.s2.flags & (SEG_B_NMAJOR | (3u << SEG_B_SEL_SHIFT)));
+                p2.A = t.s1.A;                                          // L: K-major stored [a′][a], M-major if transposed
+                p2.a_rp = t.s1.a_rp;
+                p2.B = 0;                                               // U_t (stored [a][b′] = N-major), offset set per chunk
+                p2.b_rp = pad_rows(t.m);
+                p2.klen = t.m;
+                p2.flags = (t.s1.flags & (SEG_A_MMAJOR | (3u << SEG_A_SEL_SHIFT))) | SEG_B_NMAJOR | SEG_B_TBUF | (BASE_WS << SEG_B_SEL_SHIFT);
+                t.s1 = p1;
+                t.s2 = p2;
+                t.t_rows = t.m;
+                t.t_cols = t.no;
+                t.t_ld = pb[ob].ld;
+            }
+            tb += int64_t(pad_rows(t.t_rows)) * t.t_ld * 8;
             mine.push_back(t);
         }
         return tb;
@@ -280,8 +343,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                     ring_used += round_up(op->n_padded * 8, 128);
                 }
             for (Task& t : mine) {
-                if (L[k] && !L[k]->dev) t.s1.A += (unsigned long long)staged[L[k]];
-                if (R[k] && !R[k]->dev) t.s2.B += (unsigned long long)staged[R[k]];
+                if (L[k] && !L[k]->dev) t.Laddr() += (unsigned long long)staged[L[k]];
+                if (R[k] && !R[k]->dev) t.Raddr() += (unsigned long long)staged[R[k]];
                 tasks.push_back(t);
             }
             t_bytes += tb;
@@ -301,7 +364,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             } else {
                 h->flops_alg += std::min(2 * mo * n * (m + no), 2 * m * no * (n + mo));
             }
-            h->flops_exec += 2 * mo * m * n + 2 * mo * n * no;
+            h->flops_exec += t.rfirst ? 2 * m * n * no + 2 * mo * m * no : 2 * mo * m * n + 2 * mo * n * no;
+            h->n_rfirst += t.rfirst;
             if (!il) h->op_bytes += int64_t(8) * t.mo * t.m;
             if (!ir) h->op_bytes += int64_t(8) * t.no * t.n;
         }
@@ -315,7 +379,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             int64_t off = 0;
             for (size_t i = 0; i < tasks.size(); ++i) {
                 t_off[i] = off;
-                off += int64_t(pad_rows(tasks[i].mo)) * pb[tasks[i].ib].ld * 8;
+                off += int64_t(pad_rows(tasks[i].t_rows)) * tasks[i].t_ld * 8;
             }
             struct U1 {
                 int64_t cost;
@@ -325,26 +389,26 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             for (size_t i = 0; i < tasks.size(); ++i) {
                 Task& t = tasks[i];
                 segs.push_back(t.s1);   // a staged A still lacks the ring base (added below)
-                t.s2.A = (unsigned long long)t_off[i];
-                const int ldt = pb[t.ib].ld;
-                const int64_t nkt = (t.m + TILE_K - 1) / TILE_K;
-                for (int i0 = 0; i0 < t.mo; i0 += TILE_M)
+                (t.rfirst ? t.s2.B : t.s2.A) = (unsigned long long)t_off[i];
+                const int ldt = t.t_ld;
+                const int64_t nkt = (t.s1.klen + TILE_K - 1) / TILE_K;
+                for (int i0 = 0; i0 < t.t_rows; i0 += TILE_M)
                     for (int j0 = 0; j0 < ldt; j0 += TILE_N) {
                         Unit u;
                         memset(&u, 0, sizeof(u));
                         u.C = (unsigned long long)t_off[i];      // block origin of T_t
                         u.alpha = t.alpha;
-                        u.c_rp = pad_rows(t.mo);
+                        u.c_rp = pad_rows(t.t_rows);
                         u.i0 = i0;
                         u.j0 = j0;
-                        u.mrows = t.mo;
-                        u.ncols = t.n;
+                        u.mrows = t.t_rows;
+                        u.ncols = t.t_cols;
                         u.ncols_st = ldt;
                         u.seg_begin = int32_t(i);   // chunk-local, rebased below
                         u.seg_end = int32_t(i) + 1;
                         u.mode = BASE_WS << UNIT_C_SEL_SHIFT;
                         u.nkt = int32_t(nkt);
-                        tmp.push_back({cost_of(std::min(TILE_M, t.mo - i0), std::min(TILE_N, ldt - j0), nkt), u});
+                        tmp.push_back({cost_of(std::min(TILE_M, t.t_rows - i0), std::min(TILE_N, ldt - j0), nkt), u});
                     }
             }
             std::stable_sort(tmp.begin(), tmp.end(), [](const U1& a, const U1& b) { return a.cost > b.cost; });
@@ -364,7 +428,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             int64_t total_cost = 0;
             for (size_t ob = 0; ob < pb.size(); ++ob) {
                 int64_t nkt = 0;
-                for (int i : by_ob[ob]) nkt += (tasks[i].n + TILE_K - 1) / TILE_K;
+                for (int i : by_ob[ob]) nkt += (tasks[i].s2.klen + TILE_K - 1) / TILE_K;
                 for (int i0 = 0; i0 < pb[ob].rows; i0 += TILE_M)
                     for (int j0 = 0; j0 < pb[ob].ld; j0 += TILE_N)
                         total_cost += cost_of(std::min(TILE_M, pb[ob].rows - i0), std::min(TILE_N, pb[ob].ld - j0), nkt);
@@ -382,7 +446,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 std::vector<int64_t> prefix(1, 0);
                 for (int i : by_ob[ob]) {
                     segs.push_back(tasks[i].s2);
-                    prefix.push_back(prefix.back() + (tasks[i].n + TILE_K - 1) / TILE_K);
+                    prefix.push_back(prefix.back() + (tasks[i].s2.klen + TILE_K - 1) / TILE_K);
                 }
                 const int ns = int(by_ob[ob].size());
                 const int64_t nkt = prefix.back();
@@ -466,15 +530,15 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                 d.rows_pad = pb[b].rows_pad;
                 d.t_begin = int32_t(dtasks.size());
                 for (int i : by_b[b]) {
-                    const Task& t = tasks[i];
+                    Task& t = tasks[i];
                     DiagTask dt;
                     memset(&dt, 0, sizeof(dt));
-                    dt.L = t.s1.A;
-                    dt.R = t.s2.B;
+                    dt.L = t.Laddr();
+                    dt.R = t.Raddr();
                     dt.alpha = t.alpha;
-                    dt.l_rp = t.s1.a_rp;
-                    dt.r_rp = t.s2.b_rp;
-                    dt.sel = ((t.s1.flags >> SEG_A_SEL_SHIFT) & 3u) | (((t.s2.flags >> SEG_B_SEL_SHIFT) & 3u) << 2);
+                    dt.l_rp = t.Lrp();
+                    dt.r_rp = t.Rrp();
+                    dt.sel = t.Lsel() | (t.Rsel() << 2);
                     dtasks.push_back(dt);
                 }
                 d.t_end = int32_t(dtasks.size());
@@ -508,17 +572,20 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             units[i].seg_end += int32_t(c.p1_seg0);
             units[i].C += tbuf;                                   // phase 1 writes T buffer ci mod 2
         }
-        for (int64_t sgi = c.p2_seg0; sgi < c.p2_seg0 + c.p2_segs; ++sgi) segs[sgi].A += tbuf;   // phase 2 reads it
+        for (int64_t sgi = c.p2_seg0; sgi < c.p2_seg0 + c.p2_segs; ++sgi) {                      // phase 2 reads it
+            if (segs[sgi].flags & SEG_A_TBUF) segs[sgi].A += tbuf;
+            if (segs[sgi].flags & SEG_B_TBUF) segs[sgi].B += tbuf;
+        }
         for (int64_t i = c.p2_unit0; i < c.p2_unit0 + c.p2_units; ++i) {
             units[i].seg_begin += int32_t(c.p2_seg0);
             units[i].seg_end += int32_t(c.p2_seg0);
             if (units[i].mode & UNIT_C_PLAIN) units[i].C += part_base;
         }
         for (int64_t i = c.r_unit0; i < c.r_unit0 + c.r_units; ++i) runits[i].P += part_base;
-        for (int64_t s = c.p1_seg0; s < c.p1_seg0 + c.p1_segs; ++s)
-            if (((segs[s].flags >> SEG_A_SEL_SHIFT) & 3u) == BASE_WS) segs[s].A += ring;   // staged L block
-        for (int64_t s = c.p2_seg0; s < c.p2_seg0 + c.p2_segs; ++s)
-            if (((segs[s].flags >> SEG_B_SEL_SHIFT) & 3u) == BASE_WS) segs[s].B += ring;   // staged R block
+        for (int64_t s = c.p1_seg0; s < c.p2_seg0 + c.p2_segs; ++s) {      // staged operator blocks (the two phases' segments are contiguous)
+            if (((segs[s].flags >> SEG_A_SEL_SHIFT) & 3u) == BASE_WS && !(segs[s].flags & SEG_A_TBUF)) segs[s].A += ring;
+            if (((segs[s].flags >> SEG_B_SEL_SHIFT) & 3u) == BASE_WS && !(segs[s].flags & SEG_B_TBUF)) segs[s].B += ring;
+        }
         for (int64_t b = c.d_block0; b < c.d_block0 + c.d_blocks; ++b)
             for (int t = dblocks[b].t_begin; t < dblocks[b].t_end; ++t) {
                 if ((dtasks[t].sel & 3u) == BASE_WS) dtasks[t].L += ring;

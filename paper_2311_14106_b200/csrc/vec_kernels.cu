@@ -328,4 +328,30 @@ int32_t dmrgk_vec_precond(dmrgk_ctx* ctx, int64_t n, const double* r_dev, const 
     return DMRGK_OK;
 }
 
+// ---- the BLAS-1 names of SURVEY §8(b) (dot, nrm2, axpy, scal), thin forms of the kernels above ----
+__global__ void sqrt_inplace_kernel(double* x) { x[0] = sqrt(x[0]); }
+
+int32_t dmrgk_vec_dot(dmrgk_ctx* ctx, int64_t n, const double* x_dev, const double* y_dev, double* out_dev,
+                      void* scratch_dev, void* stream) {
+    return dmrgk_vec_multi_dot(ctx, n, 1, x_dev, n, y_dev, out_dev, scratch_dev, stream);
+}
+
+int32_t dmrgk_vec_nrm2(dmrgk_ctx* ctx, int64_t n, const double* x_dev, double* out_dev, void* scratch_dev,
+                       void* stream) {
+    DMRGK_TRY(dmrgk_vec_multi_dot(ctx, n, 1, x_dev, n, x_dev, out_dev, scratch_dev, stream));
+    if (n == 0) return DMRGK_OK;
+    sqrt_inplace_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(out_dev);
+    count_launch();
+    DMRGK_CUDA(cudaGetLastError());
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_vec_axpy(dmrgk_ctx* ctx, int64_t n, double alpha, const double* x_dev, double* y_dev, void* stream) {
+    return dmrgk_vec_axpby(ctx, n, alpha, x_dev, 1.0, y_dev, stream);
+}
+
+int32_t dmrgk_vec_scal(dmrgk_ctx* ctx, int64_t n, double alpha, double* x_dev, void* stream) {
+    return dmrgk_vec_axpby(ctx, n, alpha, x_dev, 0.0, x_dev, stream);   // x = alpha·x + 0·x, element by element
+}
+
 }  // extern "C"

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "_build", "libdmrgk.so")
 
 OK, EINVAL, ESHAPE, ECHARGE, EALIGN, ENOMEM, ECUDA, ENOTCONV, ESTATE = 0, -1, -2, -3, -4, -5, -6, -7, -8
-TRANS_L, TRANS_R, IDENT_L, IDENT_R = 1, 2, 4, 8
+TRANS_L, TRANS_R, IDENT_L, IDENT_R, HC_OF_PREV = 1, 2, 4, 8, 16
 
 _STATUS_NAMES = {0: "OK", -1: "EINVAL", -2: "ESHAPE", -3: "ECHARGE", -4: "EALIGN", -5: "ENOMEM",
                  -6: "ECUDA", -7: "ENOTCONV", -8: "ESTATE"}
@@ -33,7 +33,7 @@ class RenormOpts(C.Structure):
 
 class HeffOpts(C.Structure):
     _fields_ = [("t_chunk_bytes", C.c_int64), ("ring_bytes", C.c_int64), ("kernel", C.c_int32),
-                ("split_waves", C.c_int32), ("reserved", C.c_int32 * 4)]
+                ("split_waves", C.c_int32), ("order_policy", C.c_int32), ("reserved", C.c_int32 * 3)]
 
 
 _p, _i32, _i64, _u64, _f64 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_double
@@ -94,6 +94,10 @@ SIGNATURES = {
     "dmrgk_vec_multi_dot": (_i32, [_p, _i64, _i32, _p, _i64, _p, _p, _p, _p]),
     "dmrgk_vec_multi_axpy": (_i32, [_p, _i64, _i32, _p, _i64, _p, _f64, _f64, _p, _p]),
     "dmrgk_vec_axpby": (_i32, [_p, _i64, _f64, _p, _f64, _p, _p]),
+    "dmrgk_vec_dot": (_i32, [_p, _i64, _p, _p, _p, _p, _p]),
+    "dmrgk_vec_nrm2": (_i32, [_p, _i64, _p, _p, _p, _p]),
+    "dmrgk_vec_axpy": (_i32, [_p, _i64, _f64, _p, _p, _p]),
+    "dmrgk_vec_scal": (_i32, [_p, _i64, _f64, _p, _p]),
     "dmrgk_vec_scal_dev": (_i32, [_p, _i64, _p, _i32, _p, _p, _p]),
     "dmrgk_vec_residual": (_i32, [_p, _i64, _i32, _p, _p, _i64, _p, _p, _p, _p, _p]),
     "dmrgk_vec_precond": (_i32, [_p, _i64, _p, _p, _p, _p, _p]),
@@ -433,7 +437,7 @@ class Renorm:
 class Heff:
     """dmrgk_heff: terms = [(L Op or None, R Op or None, coef, trans_L, trans_R)]."""
 
-    def __init__(self, ctx, layout, terms, t_chunk_bytes=0, ring_bytes=0, kernel=0, split_waves=0):
+    def __init__(self, ctx, layout, terms, t_chunk_bytes=0, ring_bytes=0, kernel=0, split_waves=0, order_policy=0):
         self.ctx, self.lib, self.layout = ctx, ctx.lib, layout
         K = len(terms)
         Larr = (C.c_void_p * max(K, 1))()
@@ -442,13 +446,17 @@ class Heff:
         flags = np.zeros(max(K, 1), np.uint32)
         self._ops = []
         for k, (L, R, c, tL, tR) in enumerate(terms):
+            coef[k] = c
+            if tL == "hc":                    # (None, None, coef, "hc", "hc"): the h.c. of the previous pair
+                Larr[k] = Rarr[k] = None
+                flags[k] = HC_OF_PREV
+                continue
             Larr[k] = L.h if L is not None else None
             Rarr[k] = R.h if R is not None else None
-            coef[k] = c
             flags[k] = ((TRANS_L if tL else 0) | (TRANS_R if tR else 0) |
                         (IDENT_L if L is None else 0) | (IDENT_R if R is None else 0))
             self._ops += [L, R]
-        opts = HeffOpts(int(t_chunk_bytes), int(ring_bytes), int(kernel), int(split_waves))
+        opts = HeffOpts(int(t_chunk_bytes), int(ring_bytes), int(kernel), int(split_waves), int(order_policy))
         h = C.c_void_p()
         check(self.lib.dmrgk_heff_create(ctx.h, layout.h, K, Larr, Rarr, coef.ctypes.data, flags.ctypes.data,
                                          C.byref(opts), C.byref(h)))
@@ -560,6 +568,22 @@ def vec_multi_dot(ctx, n, nv, X, stride, y, out, scratch, stream=None):
 
 def vec_multi_axpy(ctx, n, nv, X, stride, coef, alpha, beta, y, stream=None):
     check(ctx.lib.dmrgk_vec_multi_axpy(ctx.h, n, nv, _dev(X), stride, _dev(coef), alpha, beta, _dev(y), _stream(stream)))
+
+
+def vec_dot(ctx, n, x, y, out, scratch, stream=None):
+    check(ctx.lib.dmrgk_vec_dot(ctx.h, n, _dev(x), _dev(y), _dev(out), _dev(scratch), _stream(stream)))
+
+
+def vec_nrm2(ctx, n, x, out, scratch, stream=None):
+    check(ctx.lib.dmrgk_vec_nrm2(ctx.h, n, _dev(x), _dev(out), _dev(scratch), _stream(stream)))
+
+
+def vec_axpy(ctx, n, alpha, x, y, stream=None):
+    check(ctx.lib.dmrgk_vec_axpy(ctx.h, n, alpha, _dev(x), _dev(y), _stream(stream)))
+
+
+def vec_scal(ctx, n, alpha, x, stream=None):
+    check(ctx.lib.dmrgk_vec_scal(ctx.h, n, alpha, _dev(x), _stream(stream)))
 
 
 def vec_axpby(ctx, n, alpha, x, beta, y, stream=None):

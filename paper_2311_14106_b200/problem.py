@@ -119,7 +119,8 @@ class DeviceProblem:
     # ---- H_eff ----------------------------------------------------------------------------------
     def build(self, terms, **opts):
         """terms: [(L index or None, R index or None, coef, trans_L, trans_R)]."""
-        t = [(None if L is None else self.ops[L], None if R is None else self.ops[R], c, tL, tR)
+        t = [(None, None, c, "hc", "hc") if tL == "hc" else
+             (None if L is None else self.ops[L], None if R is None else self.ops[R], c, tL, tR)
              for (L, R, c, tL, tR) in terms]
         self.heff = dmrgk.Heff(self.ctx, self.layout, t, **opts)
         self.workspace = torch.empty(max(self.heff.workspace_bytes, 128), dtype=torch.uint8, device=self.device)

@@ -55,7 +55,7 @@ def test_sigma_vs_dense_kronecker(make, kernel):
 
 
 @pytest.mark.parametrize("make", [medium_config2, medium_spinless, medium_hubbard])
-@pytest.mark.parametrize("opts", [{}, {"split_waves": 64}, {"t_chunk_bytes": 1 << 20}])
+@pytest.mark.parametrize("opts", [{}, {"split_waves": 4}, {"t_chunk_bytes": 1 << 20}, {"order_policy": 1}, {"order_policy": 2}])
 def test_sigma_vs_blockwise_medium(make, opts):
     """T3 at sizes spanning several tiles and ragged tails; split-k and chunking variants."""
     pb = heff.problem_from_workload(make())
@@ -66,6 +66,44 @@ def test_sigma_vs_blockwise_medium(make, opts):
     assert padding_is_zero(dp, sigma)
     if "t_chunk_bytes" in opts:
         assert dp.heff.n_chunks > 1
+    if opts.get("order_policy", 0) == 0:
+        assert dp.heff.flops_exec == dp.heff.flops_alg == heff.flops_alg(pb)      # every task in its cheaper order
+    else:
+        assert dp.heff.flops_exec >= dp.heff.flops_alg
+
+
+def test_gemm_order_is_chosen_per_task_on_skewed_shapes():
+    """Sectors of very different sizes on the two halves: (Lψ)Rᵀ is cheaper for some tasks, L(ψRᵀ) for
+    others.  All three policies give the oracle's σ; only the automatic one executes the
+    algorithmic flop count; a staged (pinned) run goes through the same code with both orders present."""
+    from paper_2311_14106_b200 import problem
+    secA = [((q,), d) for q, d in enumerate([3, 70, 5, 130, 9, 2])]
+    secB = [((q,), d) for q, d in enumerate([90, 4, 150, 6, 40, 11])]
+    wl = wlmod.Workload("skewed", 21, 1, secA, secB, (5,))
+    shifts = [1, -1, 2, 0, -2, 1, -1, 0]
+    for k, dlt in enumerate(shifts):
+        wl.ops.append(wlmod.OpSpec("A", (dlt,), dlt & 1, False, "one", f"L{k}"))
+        wl.ops.append(wlmod.OpSpec("B", (-dlt,), dlt & 1, False, "one", f"R{k}"))
+        wl.terms.append(wlmod.TermSpec(2 * k, 2 * k + 1, 0.3 + 0.1 * k, False, False, "syn"))
+        wl.terms.append(wlmod.TermSpec(2 * k, 2 * k + 1, -0.2 + 0.05 * k, True, True, "syn^T"))
+    pb = heff.problem_from_workload(wl)
+    ref = heff.sigma_blockwise(pb)
+    execd = {}
+    for policy in (0, 1, 2):
+        dp = device_problem(pb, order_policy=policy)
+        sigma = dp.apply(dp.psi_from_host(pb.psi))
+        assert rel_max(dp.to_blocks(sigma), ref) <= TOL_SIGMA, policy
+        assert padding_is_zero(dp, sigma)
+        assert rel_max(dp.to_blocks(dp.diag()), heff.diagonal_blockwise(pb)) <= 1e-13
+        execd[policy] = dp.heff.flops_exec
+        assert dp.heff.flops_alg == heff.flops_alg(pb)
+    assert execd[0] == heff.flops_alg(pb) and execd[1] > execd[0] and execd[2] > execd[0]     # both orders are in use
+    stg = problem.from_workload(wl, pinned=[1, 2, 6, 9], ring_bytes=64 << 20)
+    got = stg.apply(stg.psi_fill(wl.seed, wlmod.PSI_STREAM))
+    res = problem.from_workload(wl)
+    want = res.apply(res.psi_fill(wl.seed, wlmod.PSI_STREAM))
+    torch.cuda.synchronize()
+    assert torch.equal(got, want)
 
 
 def test_device_fill_matches_host_generator():
@@ -219,6 +257,27 @@ def test_staging_ring_too_small_for_a_pair_is_refused():
     got = ok.apply(psi)
     torch.cuda.synchronize()
     assert float((got - ref).abs().max() / ref.abs().max()) <= 1e-13
+
+
+def test_hc_of_prev_flag_equals_explicit_transposes():
+    """DMRGK_HC_OF_PREV: 'pair k is the h.c. of pair k−1' gives the same bits as naming the same stored
+    operators with both transpose flags (SURVEY §8(b) flag list)."""
+    pb = heff.problem_from_workload(medium_spinless())
+    explicit = device_problem(pb)
+    terms = []
+    for k, (L, R, c, tL, tR) in enumerate(pb.terms):
+        prev = pb.terms[k - 1] if k else None
+        if prev is not None and tL and tR and (L, R) == (prev[0], prev[1]) and not prev[3] and not prev[4]:
+            terms.append((None, None, c, "hc", "hc"))
+        else:
+            terms.append((L, R, c, tL, tR))
+    assert any(t[3] == "hc" for t in terms)
+    from paper_2311_14106_b200 import problem
+    dp = problem.from_host(pb.n_charges, pb.sectors_A, pb.sectors_B, pb.target, pb.ops, terms)
+    a = explicit.apply(explicit.psi_from_host(pb.psi))
+    b = dp.apply(dp.psi_from_host(pb.psi))
+    torch.cuda.synchronize()
+    assert torch.equal(a, b) and dp.heff.n_tasks == explicit.heff.n_tasks
 
 
 def test_apply_host_end_to_end():

@@ -87,3 +87,24 @@ def test_residual_and_precond(ctx):
     den = np.where(np.abs(den) < 1e-10, np.where(den < 0, -1e-10, 1e-10), den)
     rr = r.cpu().numpy()
     assert np.abs(t.cpu().numpy() - rr / den).max() <= 1e-15 * np.abs(rr / den).max() * 4
+
+
+def test_blas1_names():
+    """dmrgk_vec_dot / nrm2 / axpy / scal against NumPy."""
+    from paper_2311_14106_b200 import dmrgk
+    ctx = dmrgk.Ctx(0)
+    n = 100_016
+    rng = np.random.default_rng(3)
+    xh, yh = rng.normal(size=n), rng.normal(size=n)
+    x, y = torch.from_numpy(xh).cuda(), torch.from_numpy(yh).cuda()
+    out = torch.zeros(8, dtype=torch.float64, device="cuda")
+    scratch = torch.empty(dmrgk.vec_scratch_bytes(1), dtype=torch.uint8, device="cuda")
+    dmrgk.vec_dot(ctx, n, x, y, out, scratch)
+    assert abs(float(out[0]) - float(xh @ yh)) <= 1e-12 * np.linalg.norm(xh) * np.linalg.norm(yh)
+    dmrgk.vec_nrm2(ctx, n, x, out, scratch)
+    assert abs(float(out[0]) - np.linalg.norm(xh)) <= 1e-12 * np.linalg.norm(xh)
+    dmrgk.vec_axpy(ctx, n, -0.75, x, y)
+    assert np.array_equal(y.cpu().numpy(), np.asarray([-0.75 * a + b for a, b in zip(xh, yh)])) or \
+        np.abs(y.cpu().numpy() - (-0.75 * xh + yh)).max() <= 1e-15 * np.abs(yh).max()
+    dmrgk.vec_scal(ctx, n, 3.0, x)
+    assert np.array_equal(x.cpu().numpy(), 3.0 * xh)
