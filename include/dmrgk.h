@@ -152,7 +152,9 @@ typedef struct dmrgk_heff_opts {
     int32_t order_policy;   /* GEMM order per task: 0 = the cheaper of (Lψ)Rᵀ and
                                L(ψRᵀ) by flop count, 1 = always (Lψ)Rᵀ, 2 = always L(ψRᵀ); tasks
                                with an identity factor are a single product either way            */
-    int32_t reserved[3];
+    int32_t per_pair_output;/* 1: plan for dmrgk_heff_expect — every pair writes its own σ_k = c_k (L_k ⊗ R_k) ψ
+                               (not summed); dmrgk_heff_apply / _diag / Davidson refuse such a plan  */
+    int32_t reserved[2];
 } dmrgk_heff_opts;
 
 /* Builds the task list of σ = Σ_k coef[k] (L[k] ⊗ R[k]) ψ for the given layout: enumerates
@@ -188,6 +190,15 @@ int32_t dmrgk_heff_apply_host(dmrgk_heff* h, const double* psi_host, double* sig
  * coef·sign·L[i,i]·R[j,j].  Pinned operators are read through the ring like in apply. */
 int32_t dmrgk_heff_diag(dmrgk_heff* h, double* diag_dev, void* workspace_dev, void* stream_main,
                         void* stream_copy);
+
+/* Expectation values of the operator pairs ("one- and two-particle reduced
+ * density matrices … computed" on the same kernels): out_dev[k] = ⟨ψ, c_k (L_k ⊗ R_k) ψ⟩ for every pair k of a
+ * plan created with per_pair_output = 1, e.g. γ_ij = ⟨c†_i c_j⟩ with the pair list {c†_i c_j as L ⊗ R}.
+ * Phase 1 as in apply; phase 2 writes σ_k of each pair of a chunk into its own buffer in the workspace;
+ * a fused multi-dot against ψ (fixed-order, bit-reproducible) gives the K numbers.  out_dev: K doubles in
+ * device memory; asynchronous. */
+int32_t dmrgk_heff_expect(dmrgk_heff* h, const double* psi_dev, double* out_dev, void* workspace_dev,
+                          void* stream_main, void* stream_copy);
 
 /* Measurement aid.  enable = 1: every later heff_apply brackets its whole GEMM region
  * (first phase-1 launch … last reduce) with one CUDA event pair on stream_main; the launches keep

@@ -268,3 +268,16 @@ def diagonal_blockwise(pb):
         dr = np.ones(out[kin].shape[1]) if Rb is None else np.diag(Rb)
         out[kin] += alpha * np.outer(dl, dr)
     return out
+
+
+def expectation_per_pair(pb, psi=None):
+    """e_k = ⟨ψ, c_k (op_L(k) P^{π_k} ⊗ op_R(k)) ψ⟩ for every operator pair k, each from the blockwise
+    definition applied to that pair alone (with the pair list {c†_i c_j} these are
+    the elements γ_ij of the one-particle reduced density matrix)."""
+    psi = pb.psi if psi is None else psi
+    out = np.zeros(len(pb.terms))
+    for k, term in enumerate(pb.terms):
+        one = Problem(pb.n_charges, pb.sectors_A, pb.sectors_B, pb.target, pb.ops, [term], psi, pb.name)
+        sig = sigma_blockwise(one)
+        out[k] = sum(float(np.sum(sig[key] * psi[key])) for key in psi)
+    return out

@@ -215,6 +215,7 @@ struct Chunk {
     int64_t p1_segs = 0, p2_segs = 0;
     int64_t d_block0 = 0, d_blocks = 0;
     std::vector<StageCopy> copies;
+    int64_t k_first = 0, k_count = 0;   // the chunk's range of operator pairs
     int ring_part = -1;   // which third of the staging ring holds this chunk's pinned operators
 };
 
@@ -246,6 +247,8 @@ struct dmrgk_heff {
     double flops_alg = 0, flops_exec = 0;
     int64_t op_bytes = 0;
     int64_t t_bytes = 0, partial_bytes = 0, ring_bytes = 0, ring_part_bytes = 0, workspace_bytes = 0;
+    int64_t pp_base = 0, pp_bytes = 0, pp_vec_bytes = 0;   // per-pair σ_k buffers + dot scratch (dmrgk_heff_expect)
+    int64_t K = 0;
     bool done_recorded[3] = {false, false, false};
     std::vector<dmrgk::Chunk> chunks;
     // device metadata (library-owned)

@@ -122,7 +122,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
     if (o.split_waves <= 0) o.split_waves = 32;   // units per CTA slot: the queue's tail is ≈ one unit long
-    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 3) || o.order_policy < 0 || o.order_policy > 2)
+    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 3) || o.order_policy < 0 || o.order_policy > 2 ||
+        (o.per_pair_output != 0 && o.per_pair_output != 1))
         return fail(DMRGK_EINVAL, "heff_create: bad options");
     const int64_t ring_part = (o.ring_bytes / 3) / 128 * 128;   // three parts: see dmrgk_heff_apply
 
@@ -192,7 +193,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     std::vector<DiagBlock> dblocks;
     std::vector<DiagTask> dtasks;
     const int64_t slots = int64_t(ctx->n_sm) * 3;
-    int64_t max_t_bytes = 0, max_partial_tiles = 0;
+    int64_t max_t_bytes = 0, max_partial_tiles = 0, max_pairs = 0;
+    const int64_t pp_vec_bytes = round_up(layout->n_padded * 8, 128);     // one σ_k buffer (per-pair mode)
 
     // Tasks of pair k (every ψ block whose L and R blocks exist and whose output block is in the layout)
     // and the bytes of their T intermediates.  Enumerated once for all pairs: the total decides the
@@ -335,6 +337,8 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             std::vector<Task>& mine = pair_tasks[k];
             const bool nonempty = !tasks.empty() || !staged.empty();
             if (nonempty && (t_bytes + tb > o.t_chunk_bytes || ring_used + need > ring_part)) break;
+            // per-pair outputs: one σ_k buffer per pair of the chunk
+            if (o.per_pair_output && k > k0 && (k - k0 + 1) * pp_vec_bytes > std::max<int64_t>(o.t_chunk_bytes, pp_vec_bytes)) break;
             // accept pair k into the chunk
             for (const dmrgk_op* op : {(const dmrgk_op*)L[k], (const dmrgk_op*)R[k]})
                 if (op && op->pinned && op->n_padded && !staged.count(op)) {
@@ -349,6 +353,9 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             }
             t_bytes += tb;
         }
+        ch.k_first = k0;
+        ch.k_count = k - k0;
+        max_pairs = std::max<int64_t>(max_pairs, k - k0);
         k0 = k;
         max_t_bytes = std::max(max_t_bytes, t_bytes);
 
@@ -422,33 +429,51 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
         ch.p2_seg0 = int64_t(segs.size());
         ch.r_unit0 = int64_t(runits.size());
         {
-            std::vector<std::vector<int>> by_ob(pb.size());
-            for (size_t i = 0; i < tasks.size(); ++i) by_ob[tasks[i].ob].push_back(int(i));
+            // a group = the tasks summed into one destination block: all tasks of an output block, or — with
+            // per-pair outputs (dmrgk_heff_expect) — the single task of (pair k, output block), which
+            // writes block ob of the pair's own σ_k buffer
+            struct Group {
+                int ob;
+                std::vector<int> idx;
+                long long c_extra;       // byte offset of the σ_k buffer inside the per-pair region
+            };
+            std::vector<Group> groups;
+            if (!o.per_pair_output) {
+                std::vector<std::vector<int>> by_ob(pb.size());
+                for (size_t i = 0; i < tasks.size(); ++i) by_ob[tasks[i].ob].push_back(int(i));
+                for (size_t ob = 0; ob < pb.size(); ++ob)
+                    if (!by_ob[ob].empty()) groups.push_back({int(ob), std::move(by_ob[ob]), 0});
+            } else {
+                for (size_t i = 0; i < tasks.size(); ++i)
+                    groups.push_back({tasks[i].ob, std::vector<int>(1, int(i)), (long long)(tasks[i].k - ch.k_first) * pp_vec_bytes});
+            }
             // total cost → target cost of a unit
             int64_t total_cost = 0;
-            for (size_t ob = 0; ob < pb.size(); ++ob) {
+            for (const Group& gr : groups) {
+                const int ob = gr.ob;
                 int64_t nkt = 0;
-                for (int i : by_ob[ob]) nkt += (tasks[i].s2.klen + TILE_K - 1) / TILE_K;
+                for (int i : gr.idx) nkt += (tasks[i].s2.klen + TILE_K - 1) / TILE_K;
                 for (int i0 = 0; i0 < pb[ob].rows; i0 += TILE_M)
                     for (int j0 = 0; j0 < pb[ob].ld; j0 += TILE_N)
                         total_cost += cost_of(std::min(TILE_M, pb[ob].rows - i0), std::min(TILE_N, pb[ob].ld - j0), nkt);
             }
-            const int64_t target = std::max<int64_t>(64 * 256 / TILE_K, total_cost / std::max<int64_t>(1, slots * o.split_waves));
+            const int64_t target = o.per_pair_output ? (int64_t(1) << 60)
+                                 : std::max<int64_t>(64 * 256 / TILE_K, total_cost / std::max<int64_t>(1, slots * o.split_waves));
             struct U2 {
                 int64_t cost;
                 Unit u;
             };
             std::vector<U2> tmp;
             int64_t partial_tiles = 0;
-            for (size_t ob = 0; ob < pb.size(); ++ob) {
-                if (by_ob[ob].empty()) continue;
+            for (const Group& gr : groups) {
+                const int ob = gr.ob;
                 const int seg0 = int(segs.size() - ch.p2_seg0);
                 std::vector<int64_t> prefix(1, 0);
-                for (int i : by_ob[ob]) {
+                for (int i : gr.idx) {
                     segs.push_back(tasks[i].s2);
                     prefix.push_back(prefix.back() + (tasks[i].s2.klen + TILE_K - 1) / TILE_K);
                 }
-                const int ns = int(by_ob[ob].size());
+                const int ns = int(gr.idx.size());
                 const int64_t nkt = prefix.back();
                 const Block& B = pb[ob];
                 for (int i0 = 0; i0 < B.rows; i0 += TILE_M)
@@ -467,7 +492,15 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                         u.ncols_st = B.ld;
                         const unsigned long long c_sigma = (unsigned long long)(B.off * 8);     // block origin in σ
                         u.c_rp = B.rows_pad;
-                        if (n_split == 1) {
+                        if (o.per_pair_output) {
+                            u.C = c_sigma + (unsigned long long)gr.c_extra;   // + base of the per-pair region (rebased below)
+                            u.seg_begin = seg0;
+                            u.seg_end = seg0 + ns;
+                            u.mode = BASE_WS << UNIT_C_SEL_SHIFT;             // the only writer of this block: no accumulation
+                            u.pad_[0] = 1;
+                            u.nkt = int32_t(nkt);
+                            tmp.push_back({c, u});
+                        } else if (n_split == 1) {
                             u.C = c_sigma;
                             u.seg_begin = seg0;
                             u.seg_end = seg0 + ns;
@@ -558,7 +591,10 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     h->ring_bytes = any_pinned ? 3 * ring_part : 0;
     h->ring_part_bytes = ring_part;
     // workspace layout: [T buffer 0 | T buffer 1 | partial tiles | ring part 0 | 1 | 2]
-    h->workspace_bytes = std::max<int64_t>(128, 2 * h->t_bytes + h->partial_bytes + h->ring_bytes);
+    h->pp_vec_bytes = pp_vec_bytes;
+    h->pp_bytes = o.per_pair_output ? max_pairs * pp_vec_bytes + round_up(dmrgk_vec_scratch_bytes(64), 128) : 0;
+    h->pp_base = 2 * h->t_bytes + h->partial_bytes + h->ring_bytes;
+    h->workspace_bytes = std::max<int64_t>(128, h->pp_base + h->pp_bytes);
     const unsigned long long part_base = (unsigned long long)(2 * h->t_bytes);
     const unsigned long long ring_base = part_base + (unsigned long long)h->partial_bytes;
 
@@ -580,6 +616,10 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             units[i].seg_begin += int32_t(c.p2_seg0);
             units[i].seg_end += int32_t(c.p2_seg0);
             if (units[i].mode & UNIT_C_PLAIN) units[i].C += part_base;
+            if (units[i].pad_[0]) {
+                units[i].C += (unsigned long long)h->pp_base;
+                units[i].pad_[0] = 0;
+            }
         }
         for (int64_t i = c.r_unit0; i < c.r_unit0 + c.r_units; ++i) runits[i].P += part_base;
         for (int64_t s = c.p1_seg0; s < c.p2_seg0 + c.p2_segs; ++s) {      // staged operator blocks (the two phases' segments are contiguous)
@@ -594,6 +634,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
     }
     if (int64_t(segs.size()) > 0x7fffffffLL) return bail(fail(DMRGK_EINVAL, "heff_create: too many segments"));
 
+    h->K = K;
     h->n_launches = 1;
     for (const Chunk& c : h->chunks) h->n_launches += (c.p1_units > 0) + (c.p2_units > 0) + (c.r_units > 0);
 
@@ -704,17 +745,17 @@ static int32_t chunk_done(dmrgk_heff* h, const Chunk& c, cudaStream_t main) {
 
 }  // namespace dmrgk
 
-extern "C" {
 
-int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev, void* workspace_dev,
-                         void* stream_main, void* stream_copy) {
-    if (!h) return fail(DMRGK_EINVAL, "heff_apply: heff is NULL");
+// σ = H_eff ψ (expect_dev == NULL) or the per-pair expectation values (sigma_dev == NULL)
+static int32_t run_plan(dmrgk_heff* h, const double* psi_dev, double* sigma_dev, double* expect_dev, void* workspace_dev,
+                        void* stream_main, void* stream_copy) {
     const int64_t n = h->layout->n_padded;
     if (n == 0) return DMRGK_OK;
-    if (!psi_dev || !sigma_dev) return fail(DMRGK_EINVAL, "heff_apply: NULL vector");
-    if (psi_dev == sigma_dev) return fail(DMRGK_EINVAL, "heff_apply: psi and sigma alias");
+    const bool expect = expect_dev != nullptr;
+    if (!psi_dev || (!expect && !sigma_dev)) return fail(DMRGK_EINVAL, "heff_apply: NULL vector");
+    if (!expect && psi_dev == sigma_dev) return fail(DMRGK_EINVAL, "heff_apply: psi and sigma alias");
     if (!workspace_dev && h->n_tasks) return fail(DMRGK_EINVAL, "heff_apply: NULL workspace");
-    if (!aligned128(psi_dev) || !aligned128(sigma_dev) || !aligned128(workspace_dev))
+    if (!aligned128(psi_dev) || (sigma_dev && !aligned128(sigma_dev)) || !aligned128(workspace_dev))
         return fail(DMRGK_EALIGN, "heff_apply: pointers must be 128-byte aligned");
     DMRGK_CUDA(cudaSetDevice(h->ctx->device));
     cudaStream_t main = (cudaStream_t)stream_main, copy = (cudaStream_t)stream_copy;
@@ -725,7 +766,7 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
     bases.b[BASE_WS] = (unsigned long long)(uintptr_t)workspace_dev;
     bases.b[BASE_PSI] = (unsigned long long)(uintptr_t)psi_dev;
     bases.b[BASE_SIGMA] = (unsigned long long)(uintptr_t)sigma_dev;
-    DMRGK_CUDA(cudaMemsetAsync(sigma_dev, 0, size_t(n) * 8, main));
+    if (!expect) DMRGK_CUDA(cudaMemsetAsync(sigma_dev, 0, size_t(n) * 8, main));
     DMRGK_CUDA(cudaMemsetAsync(h->counters_dev, 0, (2 * h->chunks.size() + 2) * sizeof(int), main));
     // Stream choreography (all ordering by events; s1 and s2 are library-owned, non-blocking):
     //   s1 (lowest priority)  : p1(0)            p1(1)              p1(2) …   phase 1 of chunk c → T buffer c mod 2
@@ -761,12 +802,24 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
             DMRGK_CUDA(cudaEventRecord(h->ev_p1[c & 1], s1));
             DMRGK_CUDA(cudaStreamWaitEvent(s2, h->ev_p1[c & 1], 0));
         }
+        if (expect && ch.k_count)       // blocks of σ_k that no task writes must read as zero
+            DMRGK_CUDA(cudaMemsetAsync((char*)workspace_dev + h->pp_base, 0, size_t(ch.k_count) * h->pp_vec_bytes, s2));
         if (serial && ch.p2_units) DMRGK_TRY(prof_begin(h, 1, s2, &slot));
         DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, s2, h->counters_dev + 2 * c + 1, h->ctx->n_sm));
         if (serial && ch.p2_units) DMRGK_TRY(prof_end(h, slot, s2));
         if (serial && ch.r_units) DMRGK_TRY(prof_begin(h, 2, s2, &slot));
         DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, s2));
         if (serial && ch.r_units) DMRGK_TRY(prof_end(h, slot, s2));
+        if (expect) {
+            // out[k] = ⟨σ_k, ψ⟩ for the pairs of this chunk, 64 at a time (fused, fixed-order dots)
+            char* pp = (char*)workspace_dev + h->pp_base;
+            void* scratch = pp + h->pp_bytes - round_up(dmrgk_vec_scratch_bytes(64), 128);
+            for (int64_t g0 = 0; g0 < ch.k_count; g0 += 64) {
+                const int cnt = int(std::min<int64_t>(64, ch.k_count - g0));
+                DMRGK_TRY(dmrgk_vec_multi_dot(h->ctx, n, cnt, reinterpret_cast<const double*>(pp + g0 * h->pp_vec_bytes),
+                                              h->pp_vec_bytes / 8, psi_dev, expect_dev + ch.k_first + g0, scratch, s2));
+            }
+        }
         DMRGK_CUDA(cudaEventRecord(h->ev_p2[c & 1], s2));
         DMRGK_TRY(chunk_done(h, ch, s2));
         if (c + 1 < nc) DMRGK_TRY(stage_chunk(h, h->chunks[c + 1], (char*)workspace_dev, main, copy, s1, s2));
@@ -800,6 +853,27 @@ int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev
         }
     }
     return DMRGK_OK;
+}
+
+extern "C" {
+
+int32_t dmrgk_heff_apply(dmrgk_heff* h, const double* psi_dev, double* sigma_dev, void* workspace_dev,
+                         void* stream_main, void* stream_copy) {
+    if (!h) return fail(DMRGK_EINVAL, "heff_apply: heff is NULL");
+    if (h->opts.per_pair_output) return fail(DMRGK_ESTATE, "heff_apply: the plan was created with per_pair_output (use heff_expect)");
+    if (h->layout->n_padded && !sigma_dev) return fail(DMRGK_EINVAL, "heff_apply: NULL vector");
+    return run_plan(h, psi_dev, sigma_dev, nullptr, workspace_dev, stream_main, stream_copy);
+}
+
+int32_t dmrgk_heff_expect(dmrgk_heff* h, const double* psi_dev, double* out_dev, void* workspace_dev,
+                          void* stream_main, void* stream_copy) {
+    if (!h) return fail(DMRGK_EINVAL, "heff_expect: heff is NULL");
+    if (!h->opts.per_pair_output) return fail(DMRGK_ESTATE, "heff_expect: the plan was not created with per_pair_output");
+    if (h->K == 0) return DMRGK_OK;
+    if (!out_dev) return fail(DMRGK_EINVAL, "heff_expect: out is NULL");
+    DMRGK_CUDA(cudaSetDevice(h->ctx->device));
+    DMRGK_CUDA(cudaMemsetAsync(out_dev, 0, size_t(h->K) * 8, (cudaStream_t)stream_main));     // pairs without any task
+    return run_plan(h, psi_dev, nullptr, out_dev, workspace_dev, stream_main, stream_copy);
 }
 
 int32_t dmrgk_heff_profile(dmrgk_heff* h, int32_t enable) {
@@ -843,6 +917,7 @@ int32_t dmrgk_heff_apply_host(dmrgk_heff* h, const double* psi_host, double* sig
 int32_t dmrgk_heff_diag(dmrgk_heff* h, double* diag_dev, void* workspace_dev, void* stream_main,
                         void* stream_copy) {
     if (!h) return fail(DMRGK_EINVAL, "heff_diag: heff is NULL");
+    if (h->opts.per_pair_output) return fail(DMRGK_ESTATE, "heff_diag: the plan was created with per_pair_output");
     const int64_t n = h->layout->n_padded;
     if (n == 0) return DMRGK_OK;
     if (!diag_dev) return fail(DMRGK_EINVAL, "heff_diag: NULL vector");

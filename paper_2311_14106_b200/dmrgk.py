@@ -33,7 +33,8 @@ class RenormOpts(C.Structure):
 
 class HeffOpts(C.Structure):
     _fields_ = [("t_chunk_bytes", C.c_int64), ("ring_bytes", C.c_int64), ("kernel", C.c_int32),
-                ("split_waves", C.c_int32), ("order_policy", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("split_waves", C.c_int32), ("order_policy", C.c_int32), ("per_pair_output", C.c_int32),
+                ("reserved", C.c_int32 * 2)]
 
 
 _p, _i32, _i64, _u64, _f64 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_double
@@ -71,6 +72,7 @@ SIGNATURES = {
     "dmrgk_heff_destroy": (None, [_p]),
     "dmrgk_heff_query": (_i32, [_p, _pi64, _pf64, _pf64, _pi64, _pi64, _pi64, _pi64]),
     "dmrgk_heff_apply": (_i32, [_p, _p, _p, _p, _p, _p]),
+    "dmrgk_heff_expect": (_i32, [_p, _p, _p, _p, _p, _p]),
     "dmrgk_heff_apply_host": (_i32, [_p, _p, _p, _p, _p, _p, _p, _p]),
     "dmrgk_heff_diag": (_i32, [_p, _p, _p, _p, _p]),
     "dmrgk_heff_profile": (_i32, [_p, _i32]),
@@ -437,7 +439,7 @@ class Renorm:
 class Heff:
     """dmrgk_heff: terms = [(L Op or None, R Op or None, coef, trans_L, trans_R)]."""
 
-    def __init__(self, ctx, layout, terms, t_chunk_bytes=0, ring_bytes=0, kernel=0, split_waves=0, order_policy=0):
+    def __init__(self, ctx, layout, terms, t_chunk_bytes=0, ring_bytes=0, kernel=0, split_waves=0, order_policy=0, per_pair_output=0):
         self.ctx, self.lib, self.layout = ctx, ctx.lib, layout
         K = len(terms)
         Larr = (C.c_void_p * max(K, 1))()
@@ -456,7 +458,7 @@ class Heff:
             flags[k] = ((TRANS_L if tL else 0) | (TRANS_R if tR else 0) |
                         (IDENT_L if L is None else 0) | (IDENT_R if R is None else 0))
             self._ops += [L, R]
-        opts = HeffOpts(int(t_chunk_bytes), int(ring_bytes), int(kernel), int(split_waves), int(order_policy))
+        opts = HeffOpts(int(t_chunk_bytes), int(ring_bytes), int(kernel), int(split_waves), int(order_policy), int(per_pair_output))
         h = C.c_void_p()
         check(self.lib.dmrgk_heff_create(ctx.h, layout.h, K, Larr, Rarr, coef.ctypes.data, flags.ctypes.data,
                                          C.byref(opts), C.byref(h)))
@@ -477,6 +479,11 @@ class Heff:
     def apply(self, psi, sigma, workspace, stream_main=None, stream_copy=None):
         check(self.lib.dmrgk_heff_apply(self.h, _dev(psi), _dev(sigma), _dev(workspace), _stream(stream_main),
                                         _stream(stream_copy)))
+
+    def expect(self, psi, out, workspace, stream_main=None, stream_copy=None):
+        """out[k] = ⟨ψ, c_k (L_k ⊗ R_k) ψ⟩ for every pair (plan created with per_pair_output=1)."""
+        check(self.lib.dmrgk_heff_expect(self.h, _dev(psi), _dev(out), _dev(workspace), _stream(stream_main),
+                                         _stream(stream_copy)))
 
     def apply_host(self, psi_host, sigma_host, psi, sigma, workspace, stream_main=None, stream_copy=None):
         check(self.lib.dmrgk_heff_apply_host(self.h, _dev(psi_host), _dev(sigma_host), _dev(psi), _dev(sigma),

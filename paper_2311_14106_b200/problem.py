@@ -155,6 +155,12 @@ class DeviceProblem:
         self.heff.apply(psi, sigma, self.workspace, self.stream, self.copy_stream)
         return sigma
 
+    def expect(self, psi, n_pairs):
+        """⟨ψ, c_k (L_k ⊗ R_k) ψ⟩ for the n_pairs pairs of a plan built with per_pair_output=1 (device tensor)."""
+        out = torch.empty(max(n_pairs, 1), dtype=torch.float64, device=self.device)
+        self.heff.expect(psi, out, self.workspace, self.stream, self.copy_stream)
+        return out[:n_pairs]
+
     def diag(self, out=None):
         out = self.new_vector(zero=False) if out is None else out
         self.heff.diag(out, self.workspace, self.stream, self.copy_stream)
