@@ -27,6 +27,8 @@ def rdm_pairs(d, space):
 
     for i in range(n_A + n_B):
         for j in range(i, n_A + n_B):
+            if q(i) != q(j):
+                continue            # c†_i c_j changes a conserved charge: γ_ij = 0 by symmetry, no operator pair
             if j < n_A:
                 L, R = add_op("A", a[i].T @ a[j], sub(q(i), q(j)), 0), None
             elif i >= n_A:

@@ -52,6 +52,8 @@ def test_one_particle_rdm_of_a_dmrg_bond(make, bond, N):
     dp = device_problem(pb, per_pair_output=1)
     got = dp.expect(dp.psi_from_host(pb.psi), len(pb.terms)).cpu().numpy()
     gamma = rdm_fock(d, space, x)
+    listed = set(labels)
+    assert all(abs(gamma[i, j]) <= 1e-12 for i in range(d.n) for j in range(i, d.n) if (i, j) not in listed)
     for (i, j), v in zip(labels, got):
         assert abs(v - gamma[i, j]) <= 1e-11, (i, j)
     assert abs(sum(v for (i, j), v in zip(labels, got) if i == j) - N) <= 1e-11

@@ -21,6 +21,8 @@ def test_one_particle_rdm_from_pair_expectations(make, bond, N):
     pb.psi = dmrg.vec_to_blocks(space, x)
     e = heff.expectation_per_pair(pb)
     gamma = rdm_fock(d, space, x)
+    listed = set(labels)
+    assert all(abs(gamma[i, j]) <= 1e-12 for i in range(d.n) for j in range(i, d.n) if (i, j) not in listed)
     for (i, j), v in zip(labels, e):
         assert abs(v - gamma[i, j]) <= 1e-12, (i, j)
     assert abs(sum(v for (i, j), v in zip(labels, e) if i == j) - N) <= 1e-12
