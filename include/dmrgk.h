@@ -338,15 +338,20 @@ int32_t dmrgk_renorm_apply(dmrgk_renorm* plan, void* workspace_dev, void* stream
  * block).  Which products make up which operator — the complementary-operator sums over t and V — is
  * host bookkeeping (paper_2311_14106_b200/blockops.py: "complementary operators built on the host").
  *
- * `enlarged` must be the sector-major product space: sector q′ holds, in the order of the kept space's
- * sectors, every kept sector k for which q′ − q_k is the charge of a site state; site_charges is
- * [d][n_charges], all distinct.  out[i] live on `enlarged` and are bound to DEVICE arenas, which
- * dmrgk_enlarge_apply overwrites completely (zero fill, then every sub-block once — contributions are
- * grouped by destination, no atomics).  Errors: DMRGK_ESHAPE (spaces / sector dimensions inconsistent),
- * DMRGK_ECHARGE (shift or parity of a product does not match its target), DMRGK_ESTATE (unbound), DMRGK_EINVAL. */
+ * site_major = 0 is this LEFT-block form.  site_major = 1 is the RIGHT block, B′ = (site) ⊗ (kept block) with
+ * the site's modes first: a product is (y · P_s^{π_x}) ⊗ X with the parity on the small SITE factor, which the
+ * caller folds into y (flag bit 1 must be clear; flag bit 2 marks a fermionic site factor for validation only).
+ *
+ * `enlarged` must be the sector-major product space: sector q′ holds every kept sector k for which q′ − q_k
+ * is the charge of a site state — ordered by kept sector (in the kept space's order) for the left block, by
+ * site state for the right block; site_charges is [d][n_charges], all distinct.  out[i] live on `enlarged`
+ * and are bound to DEVICE arenas, which dmrgk_enlarge_apply overwrites completely (zero fill, then every
+ * sub-block once — contributions are grouped by destination, no atomics).  Errors: DMRGK_ESHAPE (spaces /
+ * sector dimensions inconsistent), DMRGK_ECHARGE (shift or parity of a product does not match its target),
+ * DMRGK_ESTATE (unbound), DMRGK_EINVAL. */
 typedef struct dmrgk_enlarge dmrgk_enlarge;
 int32_t dmrgk_enlarge_create(dmrgk_ctx* ctx, const dmrgk_space* kept, const dmrgk_space* enlarged, int32_t d,
-                             const int32_t* site_charges, int64_t n_out, dmrgk_op* const* out,
+                             const int32_t* site_charges, int32_t site_major, int64_t n_out, dmrgk_op* const* out,
                              int64_t n_terms, const int32_t* t_out, dmrgk_op* const* t_x,
                              const uint32_t* t_flags, const double* t_coef, const double* t_y,
                              dmrgk_enlarge** plan);

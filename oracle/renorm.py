@@ -114,3 +114,38 @@ def enlarge_dense(terms, sectors_K, site_charges):
         O += coef * np.kron(Xd, np.asarray(y, dtype=np.float64))
     perm, _ = enlarged_order(sectors_K, site_charges)
     return O[np.ix_(perm, perm)]
+
+
+def enlarged_order_right(sectors_K, site_charges):
+    """As `enlarged_order` for the RIGHT block, product basis |σ⟩⊗|r⟩ with σ major: perm[new] = σ·M + r."""
+    qs = []
+    for q, dim in sectors_K:
+        qs += [tuple(q)] * dim
+    keys = [tuple(a + b for a, b in zip(tuple(site_charges[s]), qr)) for s in range(len(site_charges)) for qr in qs]
+    perm = sorted(range(len(keys)), key=lambda i: (keys[i], i))
+    sectors = []
+    for i in perm:
+        if sectors and sectors[-1][0] == keys[i]:
+            sectors[-1][1] += 1
+        else:
+            sectors.append([keys[i], 1])
+    return np.array(perm), [(k, n) for k, n in sectors]
+
+
+def enlarge_dense_right(terms, sectors_K, site_charges, site_parity):
+    """Σ_j coef_j · kron(y_j · P_s^{π_j}, X_j) for the right block B′ = site ⊗ kept (the site's modes precede
+    the block's, so the parity P_s = diag(site_parity) of the SITE multiplies y when the block operator
+    X_j is odd, π_j = 1), rows and columns in the sector-major order of B′.
+
+    terms: [(X dense or None for the identity, y dense d×d, coef, π)]."""
+    M = sum(dim for _, dim in sectors_K)
+    d = len(site_charges)
+    O = np.zeros((M * d, M * d))
+    for X, y, coef, pi in terms:
+        Xd = np.eye(M) if X is None else np.asarray(X, dtype=np.float64)
+        yd = np.asarray(y, dtype=np.float64)
+        if pi:
+            yd = yd * np.asarray(site_parity, dtype=np.float64)[None, :]
+        O += coef * np.kron(yd, Xd)
+    perm, _ = enlarged_order_right(sectors_K, site_charges)
+    return O[np.ix_(perm, perm)]

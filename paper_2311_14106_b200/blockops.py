@@ -234,3 +234,167 @@ def enlarge_left_lists(T, V, mode_charges, A, S, right):
                         a.add(0.25 * W[p, q, r, s], [("+", p), ("+", q), ("-", r), ("-", s)])
     out[("H",)] = a.terms()
     return site, out
+
+
+# ----------------------------------------------------------------------------
+# RIGHT block: B′ = (site s) ⊗ (kept B), the site's modes precede B's in the Jordan–Wigner string
+# ----------------------------------------------------------------------------
+# The right block carries the COMPLEMENTARY operators of the regrouping: for the modes
+# `left` to the left of the block
+#     ("H",)           H_{B}
+#     ("c+", p)        c†_p                                   p ∈ B
+#     ("S", p)         S^B_p  = ½ Σ_{q,r,s∈B} W_pqrs c†_q c_r c_s          p ∈ left   (no one-body part)
+#     ("P", p, q)      P^B_pq = Σ_{r<s∈B} W_pqrs c_r c_s                   p < q ∈ left
+#     ("Q", p, s)      Q^B_ps = Σ_{q,r∈B} W_pqrs c†_q c_r                  p ≤ s ∈ left  (Q_sp = Q_psᵀ)
+# With the site to the LEFT of the kept block a product "site operator left of block operator" is
+# (y · P_s^{π_x}) ⊗ X: the parity now sits on the small site factor (P_s = (−1)^{n_σ}, π_x = parity of the
+# block operator) and is folded into the d×d matrix on the host; the enlarged basis is ordered
+# |σ⟩ ⊗ |r⟩ with σ major.  Accumulating S, P and Q here is where the sums over the interaction live:
+#     P^{B′}_pq = P^B_pq + Σ_{(r,s) not both in B} ½ W_pqrs c_r c_s
+#     Q^{B′}_ps = Q^B_ps + Σ_{(q,r) not both in B} W_pqrs c†_q c_r
+#     S^{B′}_p  = S^B_p + Σ_{q∈s} c̃†_q ⊗ P^B_pq + Σ_{s∈s} c̃_s ⊗ Q^B_ps + (monomials with ≥ 2 site operators)
+#     H_{B′}    = H_B + H_s + Σ_{p∈s} [c̃†_p P_s ⊗ S^B_p − c̃_p P_s ⊗ (S^B_p)ᵀ] + Σ_{p<q∈s} [c̃†_p c̃†_q ⊗ P^B_pq + c̃_q c̃_p ⊗ (P^B_pq)ᵀ]
+#                 + Σ_{p,s∈s} c̃†_p c̃_s ⊗ Q^B_ps + (monomials with ≤ 1 block operator)
+# (second line of S^{B′}: the r∈s and s∈s placements of ½ W c†_q c_r c_s are equal by W_pqrs = −W_pqsr.)
+def right_block_keys(B, left):
+    left = list(left)
+    keys = [("H",)] + [("c+", p) for p in B] + [("S", p) for p in left]
+    keys += [("P", p, q) for i, p in enumerate(left) for q in left[i + 1:]]
+    keys += [("Q", p, s) for i, p in enumerate(left) for s in left[i:]]
+    return keys
+
+
+def right_operator_spec(key, mode_charges):
+    mc = np.asarray(mode_charges, dtype=np.int64)
+    kind = key[0]
+    if kind in ("H", "c+"):
+        return operator_spec(key, mode_charges)
+    if kind == "S":                                   # pairs with c†_p on the left block: shift −q_p
+        return tuple(int(x) for x in -mc[key[1]]), 1
+    if kind == "P":
+        return tuple(int(x) for x in -(mc[key[1]] + mc[key[2]])), 0
+    if kind == "Q":
+        return tuple(int(x) for x in -(mc[key[1]] - mc[key[2]])), 0
+    raise KeyError(key)
+
+
+def right_key_parity(key):
+    """Fermion parity of a stored right-block operator (None = identity)."""
+    return 1 if key is not None and key[0] in ("c+", "S") else 0
+
+
+def fold_site_parity(site, key, y):
+    """y · P_s^{π_x}: the form dmrgk_enlarge takes for the right block (site_major = 1)."""
+    return y * site.parity[None, :] if right_key_parity(key) else y
+
+
+class _RightAccumulator(_Accumulator):
+    """Monomials whose block part has at most one operator; the site part stays on the left."""
+
+    def add(self, coef, ops):
+        if coef == 0.0:
+            return
+        kept, sops, swaps, n_kept_seen = [], [], 0, 0
+        for op in ops:
+            if op[1] in self.in_site:
+                sops.append(op)
+                swaps += n_kept_seen                  # this site operator jumps left over the block operators before it
+            else:
+                kept.append(op)
+                n_kept_seen += 1
+        if len(kept) > 1:
+            raise ValueError("block part with more than one operator must be given as a stored sum")
+        key, trans, factor = _kept_part(kept)
+        sign = -1.0 if swaps % 2 else 1.0
+        self.add_product(key, trans, coef * sign * factor, sops, len(kept) % 2)
+
+    def add_product(self, key, trans, coef, sops, kept_parity):
+        """coef · (site string · P_s^{kept parity}) ⊗ (stored operator `key`, maybe transposed)."""
+        assert kept_parity == right_key_parity(key)
+        y = self.site.matrix(sops)                    # P_s^{kept parity} is applied by the consumer (fold_site_parity)
+        g = (key, trans, len(sops) % 2)
+        acc = self.groups.get(g)
+        if acc is None:
+            acc = self.groups[g] = np.zeros((self.site.d, self.site.d))
+        acc += coef * y
+
+
+def enlarge_right_lists(T, V, mode_charges, left, S, B):
+    """Product lists of every operator of the right block B′ = S ∪ B (S = the site's modes, all to the left
+    of B's), `left` = the modes to the left of B′.  Kept keys refer to right_block_keys(B, left + S).
+
+    Returns (site, {target key: [(kept key or None, transposed, y (d×d), site factor odd)]}); the product is
+    (y · P_s^{π_x}) ⊗ X with π_x = right_key_parity(kept key) — see fold_site_parity."""
+    T = np.asarray(T, dtype=np.float64)
+    W = antisymmetrise(np.asarray(V, dtype=np.float64))
+    left, S, B = list(left), list(S), list(B)
+    site = Site(S, mode_charges)
+    m = len(S)
+    site.parity = np.array([1.0 - 2.0 * (bin(i).count("1") % 2) for i in range(site.d)])
+    in_site, in_B = set(S), set(B)
+    Bp = S + B
+    out = {}
+
+    def acc():
+        return _RightAccumulator(site, in_site)
+
+    for p in Bp:
+        a = acc()
+        a.add(1.0, [("+", p)])
+        out[("c+", p)] = a.terms()
+    for i, p in enumerate(left):
+        # S^{B′}_p
+        a = acc()
+        a.add_product(("S", p), False, 1.0, [], 1)
+        for q in S:
+            a.add_product(("P", p, q), False, 1.0, [("+", q)], 0)
+            a.add_product(("Q", p, q), False, 1.0, [("-", q)], 0)
+        for q in Bp:
+            for r in Bp:
+                for s in Bp:
+                    if (q in in_site) + (r in in_site) + (s in in_site) >= 2:
+                        a.add(0.5 * W[p, q, r, s], [("+", q), ("-", r), ("-", s)])
+        out[("S", p)] = a.terms()
+        for q in left[i + 1:]:
+            a = acc()
+            a.add_product(("P", p, q), False, 1.0, [], 0)
+            for r in Bp:
+                for s in Bp:
+                    if r in in_site or s in in_site:
+                        a.add(0.5 * W[p, q, r, s], [("-", r), ("-", s)])
+            out[("P", p, q)] = a.terms()
+        for s in left[i:]:
+            a = acc()
+            a.add_product(("Q", p, s), False, 1.0, [], 0)
+            for q in Bp:
+                for r in Bp:
+                    if q in in_site or r in in_site:
+                        a.add(W[p, q, r, s], [("+", q), ("-", r)])
+            out[("Q", p, s)] = a.terms()
+    # H_{B′}
+    a = acc()
+    a.add_product(("H",), False, 1.0, [], 0)
+    for p in S:
+        a.add_product(("S", p), False, +1.0, [("+", p)], 1)
+        a.add_product(("S", p), True, -1.0, [("-", p)], 1)
+    for i, p in enumerate(S):
+        for q in S[i + 1:]:
+            a.add_product(("P", p, q), False, 1.0, [("+", p), ("+", q)], 0)
+            a.add_product(("P", p, q), True, 1.0, [("-", q), ("-", p)], 0)
+        for s in S:
+            if p <= s:
+                a.add_product(("Q", p, s), False, 1.0, [("+", p), ("-", s)], 0)
+            else:
+                a.add_product(("Q", s, p), True, 1.0, [("+", p), ("-", s)], 0)
+    for p in Bp:
+        for q in Bp:
+            if p in in_site or q in in_site:
+                a.add(T[p, q], [("+", p), ("-", q)])
+    for p in Bp:
+        for q in Bp:
+            for r in Bp:
+                for s in Bp:
+                    if (p in in_site) + (q in in_site) + (r in in_site) + (s in in_site) >= 3:
+                        a.add(0.25 * W[p, q, r, s], [("+", p), ("+", q), ("-", r), ("-", s)])
+    out[("H",)] = a.terms()
+    return site, out

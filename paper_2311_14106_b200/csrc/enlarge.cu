@@ -105,13 +105,13 @@ void dmrgk_enlarge_destroy(dmrgk_enlarge* e) {
 }
 
 int32_t dmrgk_enlarge_create(dmrgk_ctx* ctx, const dmrgk_space* kept, const dmrgk_space* enlarged, int32_t d,
-                             const int32_t* site_charges, int64_t n_out, dmrgk_op* const* out, int64_t n_terms,
+                             const int32_t* site_charges, int32_t site_major, int64_t n_out, dmrgk_op* const* out, int64_t n_terms,
                              const int32_t* t_out, dmrgk_op* const* t_x, const uint32_t* t_flags,
                              const double* t_coef, const double* t_y, dmrgk_enlarge** plan) {
     if (!plan) return fail(DMRGK_EINVAL, "enlarge_create: plan is NULL");
     *plan = nullptr;
-    if (!ctx || !kept || !enlarged || !site_charges || d < 1 || d > 16)
-        return fail(DMRGK_EINVAL, "enlarge_create: bad argument (d must be 1..16)");
+    if (!ctx || !kept || !enlarged || !site_charges || d < 1 || d > 16 || (site_major != 0 && site_major != 1))
+        return fail(DMRGK_EINVAL, "enlarge_create: bad argument (d must be 1..16, site_major 0 or 1)");
     if (n_out < 0 || n_terms < 0 || (n_out && !out) || (n_terms && (!t_out || !t_x || !t_flags || !t_coef || !t_y)))
         return fail(DMRGK_EINVAL, "enlarge_create: bad arrays");
     if (kept->n_charges != enlarged->n_charges) return fail(DMRGK_ESHAPE, "enlarge_create: spaces differ in the number of charges");
@@ -131,7 +131,10 @@ int32_t dmrgk_enlarge_create(dmrgk_ctx* ctx, const dmrgk_space* kept, const dmrg
             const int k = kept->find(enlarged->q[2 * e] - sq(s, 0), enlarged->q[2 * e + 1] - sq(s, 1));
             if (k >= 0 && kept->dim[k] > 0) parts.push_back({k, s});
         }
-        std::sort(parts.begin(), parts.end());
+        // left block (kept ⊗ site): by kept sector; right block (site ⊗ kept): by site state
+        std::sort(parts.begin(), parts.end(), [&](const std::pair<int, int>& a, const std::pair<int, int>& b) {
+            return site_major ? std::make_pair(a.second, a.first) < std::make_pair(b.second, b.first) : a < b;
+        });
         int off = 0;
         for (auto& p : parts) {
             sub_k[size_t(e) * d + p.second] = p.first;
@@ -157,8 +160,9 @@ int32_t dmrgk_enlarge_create(dmrgk_ctx* ctx, const dmrgk_space* kept, const dmrg
         if (o < 0 || o >= n_out) return fail(DMRGK_EINVAL, "enlarge_create: term %lld targets operator %lld", (long long)j, (long long)o);
         const dmrgk_op* X = t_x[j];
         const uint32_t f = t_flags[j];
-        if (f & ~3u) return fail(DMRGK_EINVAL, "enlarge_create: term %lld has unknown flag bits", (long long)j);
-        const bool trans = (f & 1u) != 0, site_odd = (f & 2u) != 0;
+        if (f & ~7u) return fail(DMRGK_EINVAL, "enlarge_create: term %lld has unknown flag bits", (long long)j);
+        if ((f & 2u) && site_major) return fail(DMRGK_EINVAL, "enlarge_create: term %lld: the kept-parity flag belongs to the left block form", (long long)j);
+        const bool trans = (f & 1u) != 0, kept_sign = (f & 2u) != 0, site_odd = (f & 6u) != 0;
         if (X) {
             if (X->space != kept) return fail(DMRGK_ESHAPE, "enlarge_create: term %lld: X is not on the kept space", (long long)j);
             if (X->n_padded && !X->dev) return fail(DMRGK_ESTATE, "enlarge_create: term %lld: X is not bound to a device arena", (long long)j);
@@ -181,7 +185,7 @@ int32_t dmrgk_enlarge_create(dmrgk_ctx* ctx, const dmrgk_space* kept, const dmrg
                     if (kr < 0 || kc < 0) continue;
                     ESrc s;
                     memset(&s, 0, sizeof(s));
-                    const double sign = (site_odd && kept->parity(kc)) ? -1.0 : 1.0;
+                    const double sign = (kept_sign && kept->parity(kc)) ? -1.0 : 1.0;
                     s.scale = t_coef[j] * yv * sign;
                     if (!X) {
                         if (kr != kc) continue;

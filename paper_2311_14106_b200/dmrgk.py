@@ -88,7 +88,7 @@ SIGNATURES = {
     "dmrgk_renorm_destroy": (None, [_p]),
     "dmrgk_renorm_query": (_i32, [_p, _pi64, _pf64, _pi64, _pi64]),
     "dmrgk_renorm_apply": (_i32, [_p, _p, _p]),
-    "dmrgk_enlarge_create": (_i32, [_p, _p, _p, _i32, _p, _i64, _p, _i64, _p, _p, _p, _p, _p, _pp]),
+    "dmrgk_enlarge_create": (_i32, [_p, _p, _p, _i32, _p, _i32, _i64, _p, _i64, _p, _p, _p, _p, _p, _pp]),
     "dmrgk_enlarge_destroy": (None, [_p]),
     "dmrgk_enlarge_query": (_i32, [_p, _pi64, _pi64, _pi64, _pi64]),
     "dmrgk_enlarge_apply": (_i32, [_p, _p]),
@@ -315,9 +315,11 @@ class Op(_Blocked):
 
 class Enlarge:
     """dmrgk_enlarge: out[i] = Σ_j coef_j (X_j P^π_j) ⊗ y_j.
-    terms = [(index into out_ops, X Op or None, transposed, site_odd, coef, y (d×d array))]."""
+    terms = [(index into out_ops, X Op or None, transposed, site_odd, coef, y (d×d array))].
+    site_major=False: left block, kept ⊗ site, the kept-parity sign is applied when site_odd;
+    site_major=True: right block, site ⊗ kept, y already carries P_s^{π_x} (blockops.fold_site_parity)."""
 
-    def __init__(self, ctx, kept, enlarged, site_charges, out_ops, terms):
+    def __init__(self, ctx, kept, enlarged, site_charges, out_ops, terms, site_major=False):
         self.lib, self.ctx = ctx.lib, ctx
         sc = np.ascontiguousarray(site_charges, dtype=np.int32).reshape(len(site_charges), -1)
         d = sc.shape[0]
@@ -331,11 +333,11 @@ class Enlarge:
         for j, (o, X, trans, odd, coef, y) in enumerate(terms):
             t_out[j], t_coef[j] = o, coef
             xarr[j] = X.h if X is not None else None
-            t_flags[j] = (1 if trans else 0) | (2 if odd else 0)
+            t_flags[j] = (1 if trans else 0) | ((4 if site_major else 2) if odd else 0)
             t_y[j] = np.asarray(y, dtype=np.float64)
         self._keep = (out_ops, [t[1] for t in terms], kept, enlarged)
         h = C.c_void_p()
-        check(self.lib.dmrgk_enlarge_create(ctx.h, kept.h, enlarged.h, d, sc.ctypes.data, n_out, oarr, n_terms,
+        check(self.lib.dmrgk_enlarge_create(ctx.h, kept.h, enlarged.h, d, sc.ctypes.data, int(bool(site_major)), n_out, oarr, n_terms,
                                             t_out.ctypes.data, xarr, t_flags.ctypes.data, t_coef.ctypes.data,
                                             t_y.ctypes.data, C.byref(h)))
         self.h = h

@@ -167,3 +167,104 @@ def test_bond_step_on_the_device(make, bond):
     dp.build(tms)
     sigma = dp.to_blocks(dp.apply(dp.psi_from_host(dmrg.vec_to_blocks(space2, x))))
     assert rel_max(sigma, dmrg.vec_to_blocks(space2, Heff @ x)) <= TOL_SIGMA
+
+
+@pytest.mark.parametrize("make,bond", [(spinless_3x3(64), 4), (spinless_3x3(6), 4), (hubbard_ring(16), 2)])
+def test_left_moving_bond_step_right_block_with_S_P_Q(make, bond):
+    """The mirror step of a right-to-left sweep: the right block's operators (H_B, c†_p and the
+    complementary S^B_p, P^B_pq, Q^B_ps) are renormalised with the kept basis of B, then B′ = site ⊗ B is
+    formed on the device — the S, P, Q accumulations of blockops.enlarge_right_lists — and the previous
+    bond's σ is applied with them as R operators."""
+    from paper_2311_14106_b200 import dmrgk, blockops, problem
+    from test_oracle_enlarge import fock_right_set
+    T, V, mc, site_modes, target, D = make
+    d = dmrg.SimpleDMRG(T, V, mc, site_modes, target, D=D, seed=2)
+    d.warmup_to(bond)
+    space = d.space_at(bond)                                   # bond i: B = enlarged right block
+    left = [m for s in site_modes[:bond] for m in s]
+    S = list(site_modes[bond])
+    B = [m for s in site_modes[bond + 1:] for m in s]
+    n_A = len(left) + len(S)
+    keys_B = blockops.right_block_keys(B, left + S)
+    YB = fock_right_set(T, V, mc, n_A)
+    d.step(bond, -1)
+    kept, sectors_K = dmrg.sector_major(d.R[bond + 1])
+    U = space.B.Phi.T @ kept.Phi
+    dev = torch.device("cuda", 0)
+    ctx = dmrgk.Ctx(0)
+    nc = d.mc.shape[1]
+    sp_B = dmrgk.Space(ctx, nc, space.sectors_B)
+    sp_K = dmrgk.Space(ctx, nc, sectors_K)
+    specs_B = [blockops.right_operator_spec(k, mc) for k in keys_B]
+    ops_B = DeviceOps(ctx, sp_B, specs_B, dev)
+    for i, k in enumerate(keys_B):
+        ops_B.upload(i, cut_blocks(space.B.Phi.T @ (YB[k] @ space.B.Phi), space.sectors_B, space.sectors_B, specs_B[i][0]))
+    phi = dmrgk.Iso(ctx, sp_B, sp_K)
+    pr, pc, _, _, _, _ = phi.blocks()
+    slB, slK = dmrg.sector_slices(space.sectors_B), dmrg.sector_slices(sectors_K)
+    phi_blocks = {(int(pr[b]), int(pc[b])): U[slB[pr[b]], slK[pc[b]]] for b in range(len(pr))}
+    phi_arena = torch.zeros(max(phi.n_padded, 16), dtype=torch.float64, device=dev)
+    phi_arena[:phi.n_padded].copy_(torch.from_numpy(phi.pack(problem._unpadded_from_blocks(phi.blocks(), phi_blocks))))
+    phi.bind_device(phi_arena)
+    ops_K = DeviceOps(ctx, sp_K, specs_B, dev)
+    plan = dmrgk.Renorm(ctx, phi, ops_B.ops, ops_K.ops)
+    ws = torch.empty(max(plan.workspace_bytes, 128), dtype=torch.uint8, device=dev)
+    plan.apply(ws, torch.cuda.current_stream())
+    # ---- enlarge to B′ = site ⊗ kept ----
+    site, lists = blockops.enlarge_right_lists(T, V, mc, left, S, B)
+    space2 = d.space_at(bond - 1)                              # bond i−1: A′ | B′
+    keys_Bp = blockops.right_block_keys(S + B, left)
+    specs_Bp = [blockops.right_operator_spec(k, mc) for k in keys_Bp]
+    sp_E = dmrgk.Space(ctx, nc, space2.sectors_B)
+    ops_E = DeviceOps(ctx, sp_E, specs_Bp, dev)
+    ops_E.arena.fill_(float("nan"))
+    index_K = {k: i for i, k in enumerate(keys_B)}
+    terms = []
+    for o, key in enumerate(keys_Bp):
+        for (k, tr, y, odd) in lists[key]:
+            terms.append((o, None if k is None else ops_K.ops[index_K[k]], tr, bool(odd), 1.0, blockops.fold_site_parity(site, k, y)))
+    enl = dmrgk.Enlarge(ctx, sp_K, sp_E, site.charges, ops_E.ops, terms, site_major=True)
+    enl.apply(torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    YBp = fock_right_set(T, V, mc, len(left))
+    for i, key in enumerate(keys_Bp):
+        ref = cut_blocks(space2.B.Phi.T @ (YBp[key] @ space2.B.Phi), space2.sectors_B, space2.sectors_B, specs_Bp[i][0])
+        got, pad_ok = ops_E.download(i)
+        assert pad_ok and set(got) == set(ref), key
+        scale = max(1.0, max((np.abs(v).max() for v in ref.values() if v.size), default=1.0))
+        err = max((np.abs(got[k] - ref[k]).max() for k in ref if ref[k].size), default=0.0)
+        assert err <= 1e-11 * scale, (key, err)
+    # ---- σ of bond i−1 with the device-formed R operators (L operators from the oracle) ----
+    Heff, P = d.heff_at(space2)
+    x = d.guess_at(space2, P)
+    ops, tms = [], []
+    index_E = {k: i for i, k in enumerate(keys_Bp)}
+    for key in keys_Bp:
+        dq, par = blockops.right_operator_spec(key, mc)
+        ops.append({"half": "B", "dq": dq, "parity": par, "blocks": {}})
+    for t in oterms.complementary_terms(T, V, len(left), mc, prune=False):
+        fam, lab = t.family, tuple(t.label)
+        Rk, tR = {"F1": (("c+",) + lab, False), "F1h": (("c+",) + lab, True), "F2": (("S",) + lab, False),
+                  "F2h": (("S",) + lab, True), "F3": (("P",) + lab, False), "F3h": (("P",) + lab, True)}.get(fam, (None, False))
+        if fam == "F0":
+            Rk = ("H",) if lab == ("B",) else None
+        if fam == "F4":
+            Rk, tR = (("Q",) + lab, False) if lab[0] <= lab[1] else (("Q", lab[1], lab[0]), True)
+        Li = None
+        if not (fam == "F0" and lab == ("B",)):
+            Xd = space2.A.Phi.T @ (t.X @ space2.A.Phi)
+            ops.append({"half": "A", "dq": tuple(t.dq_A), "parity": t.parity,
+                        "blocks": cut_blocks(Xd, space2.sectors_A, space2.sectors_A, tuple(t.dq_A))})
+            Li = len(ops) - 1
+        tms.append((Li, None if Rk is None else index_E[Rk], t.coef, False, tR))
+    dp = problem.DeviceProblem(nc, space2.sectors_A, space2.sectors_B, space2.target, ctx=ctx)
+    dp.create_ops([(o["half"], o["dq"], o["parity"]) for o in ops])
+    dp.alloc_resident()
+    for i, o in enumerate(ops):
+        if o["half"] == "A":
+            dp.set_op_host(i, o["blocks"])
+        elif dp.ops[i].n_padded:
+            dp.op_views[i].copy_(ops_E.views[i][:dp.ops[i].n_padded])
+    dp.build(tms)
+    sigma = dp.to_blocks(dp.apply(dp.psi_from_host(dmrg.vec_to_blocks(space2, x))))
+    assert rel_max(sigma, dmrg.vec_to_blocks(space2, Heff @ x)) <= TOL_SIGMA

@@ -103,3 +103,51 @@ def test_a_wrong_sign_is_caught():
                  for (k, tr, y, pi) in lists[key]]
         err = np.abs(renorm.enlarge_dense(terms, sectors_K, site.charges.tolist()) - ref).max()
         assert (err > 1e-3) == drop_parity
+
+
+# ---- right block: B′ = site ⊗ kept B, with the S, P, Q accumulations --------------------------------
+def fock_right_set(T, V, mc, n_A):
+    """{key: sparse operator on the Fock space of modes n_A..n−1 (B's own JW basis)}: the right-block set."""
+    out = {}
+    for t in oterms.complementary_terms(T, V, n_A, mc, prune=False):
+        if t.family == "F0" and t.label == ("B",):
+            out[("H",)] = t.Y
+        elif t.family == "F1":
+            out[("c+", t.label[0])] = t.Y
+        elif t.family == "F2":
+            out[("S", t.label[0])] = t.Y
+        elif t.family == "F3":
+            out[("P",) + tuple(t.label)] = t.Y
+        elif t.family == "F4" and t.label[0] <= t.label[1]:
+            out[("Q",) + tuple(t.label)] = t.Y
+    return out
+
+
+@pytest.mark.parametrize("make,bond", [(spinless_3x3(64), 4), (spinless_3x3(5), 4), (spinless_3x3(6, rotated=False), 3),
+                                       (hubbard_ring(6), 2), (hubbard_ring(16), 1)])
+def test_right_block_lists_reproduce_the_definition(make, bond):
+    T, V, mc, site_modes, target, D = make
+    d = dmrg.SimpleDMRG(T, V, mc, site_modes, target, D=D, seed=2)
+    d.warmup_to(bond)
+    d.step(bond, -1)                                   # sets d.R[bond + 1]: the kept basis of B = site(bond+1) ∪ …
+    kept, sectors_K = dmrg.sector_major(d.R[bond + 1])      # a relabelling: R's columns come in descending charge order
+    left = [m for s in site_modes[:bond] for m in s]
+    S = list(site_modes[bond])
+    B = [m for s in site_modes[bond + 1:] for m in s]
+    n_A = len(left) + len(S)
+    YB = fock_right_set(T, V, mc, n_A)
+    keptops = {k: kept.Phi.T @ (Y @ kept.Phi) for k, Y in YB.items()}
+    assert set(keptops) == set(blockops.right_block_keys(B, left + S))
+    site, lists = blockops.enlarge_right_lists(T, V, mc, left, S, B)
+    Bp, sectors_E = dmrg.sector_major(dmrg.kron_basis(dmrg.site_basis(d.mc[S]), kept))
+    perm, sectors_E2 = renorm.enlarged_order_right(sectors_K, site.charges.tolist())
+    assert sectors_E2 == sectors_E
+    YBp = fock_right_set(T, V, mc, len(left))
+    assert set(lists) == set(YBp) == set(blockops.right_block_keys(S + B, left))
+    for key, plist in lists.items():
+        terms = [(None if k is None else (keptops[k].T if tr else keptops[k]), y, 1.0, blockops.right_key_parity(k))
+                 for (k, tr, y, odd) in plist]
+        got = renorm.enlarge_dense_right(terms, sectors_K, site.charges.tolist(), site.parity)
+        ref = Bp.Phi.T @ (YBp[key] @ Bp.Phi)
+        scale = max(1.0, np.abs(ref).max())
+        assert np.abs(got - ref).max() <= 1e-12 * scale, key
