@@ -30,7 +30,8 @@ as a d×d matrix in the site's own Jordan–Wigner basis.  Kept parts with three
 expanded: summed with their coefficients they are S^A_p, which is stored.
 
 Host logic only: index bookkeeping and coefficient sums in NumPy; no arithmetic on operator blocks.
-The mirror image for the RIGHT block (site ⊗ kept B, with the P^B and Q^B accumulations) is not built.
+The RIGHT block (site ⊗ kept B), which carries the complementary operators S^B, P^B, Q^B and their
+accumulation, is the second half of this module (enlarge_right_lists).
 """
 import numpy as np
 
