@@ -223,7 +223,7 @@ def measure_fp64_ceiling(dp, local):
     # the register-only DMMA loop in two shapes: 3 CTAs × 4 warps per SM (the residency of the GEMM kernel) and
     # 4 CTAs × 8 warps per SM (round 1's probe, which reads ≈ 20 % low on this part: too many warps per scheduler)
     out["dmma_probe"] = {"what": "dmrgk_probe_fp64: register-only mma.sync.m8n8k4.f64 loop, full grid"}
-    for kind, shape, long_iters in ((4, "3x4_warps_per_sm", 2400000), (0, "4x8_warps_per_sm", 1200000)):
+    for kind, shape, long_iters in ((4, "3x4_warps_per_sm", 3200000), (0, "4x8_warps_per_sm", 1200000)):
         dmrgk.probe_fp64(dp.ctx, kind, 20000, sink, dp.stream)
         burst = 0.0
         for _ in range(5):
