@@ -459,13 +459,19 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             }
             const int64_t target = o.per_pair_output ? (int64_t(1) << 60)
                                  : std::max<int64_t>(64 * 256 / TILE_K, total_cost / std::max<int64_t>(1, slots * o.split_waves));
+            // Launch order = the queue order of the persistent kernel: longest first (LPT), and among units
+            // of equal cost those of one (output block, k-range) together, row tile by row tile — they run
+            // at the same time and share their T row tiles and R column tiles in L2.
             struct U2 {
                 int64_t cost;
                 Unit u;
+                int32_t grp, split;
             };
             std::vector<U2> tmp;
             int64_t partial_tiles = 0;
+            int32_t gi = -1;
             for (const Group& gr : groups) {
+                ++gi;
                 const int ob = gr.ob;
                 const int seg0 = int(segs.size() - ch.p2_seg0);
                 std::vector<int64_t> prefix(1, 0);
@@ -499,14 +505,14 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                             u.mode = BASE_WS << UNIT_C_SEL_SHIFT;             // the only writer of this block: no accumulation
                             u.pad_[0] = 1;
                             u.nkt = int32_t(nkt);
-                            tmp.push_back({c, u});
+                            tmp.push_back({c, u, gi, 0});
                         } else if (n_split == 1) {
                             u.C = c_sigma;
                             u.seg_begin = seg0;
                             u.seg_end = seg0 + ns;
                             u.mode = UNIT_ACCUM | (BASE_SIGMA << UNIT_C_SEL_SHIFT);
                             u.nkt = int32_t(nkt);
-                            tmp.push_back({c, u});
+                            tmp.push_back({c, u, gi, 0});
                         } else {
                             RUnit r;
                             r.C = c_sigma;
@@ -529,7 +535,7 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                                 u.seg_end = seg0 + se;
                                 u.mode = UNIT_C_PLAIN | (BASE_WS << UNIT_C_SEL_SHIFT);
                                 u.nkt = int32_t(prefix[se] - prefix[sb]);
-                                tmp.push_back({cost_of(rt, ct, u.nkt), u});
+                                tmp.push_back({cost_of(rt, ct, u.nkt), u, gi, made});
                                 ++made;
                                 sb = se;
                             }
@@ -539,7 +545,11 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                         }
                     }
             }
-            std::stable_sort(tmp.begin(), tmp.end(), [](const U2& a, const U2& b) { return a.cost > b.cost; });
+            std::stable_sort(tmp.begin(), tmp.end(), [](const U2& a, const U2& b) {
+                if (a.cost != b.cost) return a.cost > b.cost;
+                if (a.grp != b.grp) return a.grp < b.grp;
+                return a.split < b.split;                  // then generation order: i0, j0
+            });
             for (const U2& x : tmp) units.push_back(x.u);
             ch.p2_units = int64_t(tmp.size());
             ch.p2_segs = int64_t(segs.size()) - ch.p2_seg0;
