@@ -167,6 +167,18 @@ typedef struct dmrgk_heff_opts {
 int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                           dmrgk_op* const* L, dmrgk_op* const* R, const double* coef,
                           const uint32_t* flags, const dmrgk_heff_opts* opts, dmrgk_heff** out);
+/* As dmrgk_heff_create, with one extra scalar per (pair, INPUT ψ block): the task of pair k on input block
+ * ib gets coef[k] · block_coef[k·n_blocks + ib] (n_blocks and the block order are those of
+ * dmrgk_layout_blocks); a zero entry removes the task.  This is the slot for the SU(2) recoupling
+ * coefficients of spin-adapted DMRG (BASELINE.json north_star: "SU(2) recoupling folded
+ * into per-block-pair scalar coefficients"): with reduced matrix elements as the stored blocks, the sectors
+ * labelled by (N, 2j) — for a singlet target the B half by (N, −2j) so that charges add up to the target — and
+ * a rank-k operator split into one stored operator per Δ(2j), the 6j/9j factor of each block pair goes here
+ * (SURVEY §8(f) NEXT-3).  block_coef = NULL is dmrgk_heff_create. */
+int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
+                                    dmrgk_op* const* L, dmrgk_op* const* R, const double* coef,
+                                    const double* block_coef, const uint32_t* flags,
+                                    const dmrgk_heff_opts* opts, dmrgk_heff** out);
 void dmrgk_heff_destroy(dmrgk_heff* h);
 /* flops_alg = Σ_tasks min(2m′n(m+n′), 2mn′(n+m′)) (identity factor → one product),
  * flops_exec = flops of the products the kernels execute in the chosen GEMM order (= flops_alg with

@@ -32,6 +32,9 @@ class Problem:
     terms: list = field(default_factory=list)
     psi: dict = field(default_factory=dict)
     name: str = ""
+    block_coef: dict = None      # optional {(k, (a_idx, b_idx)): scalar}: an extra factor of pair k on INPUT block (a, b)
+                                 # — the per-block-pair recoupling scalar of SU(2)-adapted DMRG;
+                                 # a missing key means 1, a zero removes the task
 
     def psi_blocks(self):
         idxB = {q: i for i, (q, _) in enumerate(self.sectors_B)}
@@ -130,7 +133,7 @@ def dense_heff(pb):
     par = np.concatenate([np.full(d, 1.0 - 2.0 * sector_parity(q)) for q, d in pb.sectors_A])
     ia, ib = allowed_pairs(pb)
     H = np.zeros((len(ia), len(ia)))
-    for (L, R, coef, tL, tR) in pb.terms:
+    for k, (L, R, coef, tL, tR) in enumerate(pb.terms):
         X = np.eye(MA) if L is None else densify_op(pb.ops[L], pb.sectors_A, tL)
         Y = np.eye(MB) if R is None else densify_op(pb.ops[R], pb.sectors_B, tR)
         parity = 0
@@ -140,7 +143,14 @@ def dense_heff(pb):
             parity = pb.ops[R]["parity"]
         if parity:
             X = X * par[None, :]          # X · P : scales column a by (−1)^{N(q_a)}
-        H += coef * X[np.ix_(ia, ia)] * Y[np.ix_(ib, ib)]
+        term = coef * X[np.ix_(ia, ia)] * Y[np.ix_(ib, ib)]
+        if pb.block_coef is not None:     # the extra scalar belongs to the INPUT block: scale its columns
+            o = 0
+            for (ai, bi) in pb.psi_blocks():
+                n = pb.sectors_A[ai][1] * pb.sectors_B[bi][1]
+                term[:, o:o + n] *= pb.block_coef.get((k, (ai, bi)), 1.0)
+                o += n
+        H += term
     return H
 
 
@@ -204,7 +214,10 @@ def enumerate_tasks(pb):
             if (ao, bo) not in blocks:
                 continue
             sign = -1.0 if (parity and sector_parity(pb.sectors_A[ai][0])) else 1.0
-            tasks.append((k, (ai, bi), (ao, bo), Lb, Rb, coef * sign))
+            extra = 1.0 if pb.block_coef is None else pb.block_coef.get((k, (ai, bi)), 1.0)
+            if extra == 0.0:
+                continue
+            tasks.append((k, (ai, bi), (ao, bo), Lb, Rb, coef * sign * extra))
     return tasks
 
 

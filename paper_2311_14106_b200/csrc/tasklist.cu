@@ -89,6 +89,13 @@ void dmrgk_heff_destroy(dmrgk_heff* h) {
 int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
                           dmrgk_op* const* L_in, dmrgk_op* const* R_in, const double* coef,
                           const uint32_t* flags_in, const dmrgk_heff_opts* opts, dmrgk_heff** out) {
+    return dmrgk_heff_create_blockcoef(ctx, layout, K, L_in, R_in, coef, nullptr, flags_in, opts, out);
+}
+
+int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
+                                    dmrgk_op* const* L_in, dmrgk_op* const* R_in, const double* coef,
+                                    const double* block_coef, const uint32_t* flags_in,
+                                    const dmrgk_heff_opts* opts, dmrgk_heff** out) {
     if (!out) return fail(DMRGK_EINVAL, "heff_create: out is NULL");
     *out = nullptr;
     if (!ctx || !layout) return fail(DMRGK_EINVAL, "heff_create: NULL ctx or layout");
@@ -261,6 +268,10 @@ int32_t dmrgk_heff_create(dmrgk_ctx* ctx, const dmrgk_layout* layout, int64_t K,
             t.ob = ob;
             const int par = L[k] ? L[k]->parity : (R[k] ? R[k]->parity : 0);
             t.alpha = coef[k] * ((par && SA->parity(a)) ? -1.0 : 1.0);
+            if (block_coef) {                               // recoupling scalar of (pair k, input block ib)
+                t.alpha *= block_coef[size_t(k) * pb.size() + ib];
+                if (t.alpha == 0.0) continue;               // structurally forbidden (e.g. a triangle rule)
+            }
             t.diag = (ob == ib);
             // phase-1 B operand = ψ block (N-major), phase-2 A operand = T (K-major, set per chunk)
             t.s1.B = (unsigned long long)(pb[ib].off * 8);

@@ -69,6 +69,7 @@ SIGNATURES = {
     "dmrgk_op_bind_device": (_i32, [_p, _p]),
     "dmrgk_op_bind_pinned": (_i32, [_p, _p]),
     "dmrgk_heff_create": (_i32, [_p, _p, _i64, _p, _p, _p, _p, _p, _pp]),
+    "dmrgk_heff_create_blockcoef": (_i32, [_p, _p, _i64, _p, _p, _p, _p, _p, _p, _pp]),
     "dmrgk_heff_destroy": (None, [_p]),
     "dmrgk_heff_query": (_i32, [_p, _pi64, _pf64, _pf64, _pi64, _pi64, _pi64, _pi64]),
     "dmrgk_heff_apply": (_i32, [_p, _p, _p, _p, _p, _p]),
@@ -441,7 +442,8 @@ class Renorm:
 class Heff:
     """dmrgk_heff: terms = [(L Op or None, R Op or None, coef, trans_L, trans_R)]."""
 
-    def __init__(self, ctx, layout, terms, t_chunk_bytes=0, ring_bytes=0, kernel=0, split_waves=0, order_policy=0, per_pair_output=0):
+    def __init__(self, ctx, layout, terms, t_chunk_bytes=0, ring_bytes=0, kernel=0, split_waves=0, order_policy=0, per_pair_output=0,
+                 block_coef=None):
         self.ctx, self.lib, self.layout = ctx, ctx.lib, layout
         K = len(terms)
         Larr = (C.c_void_p * max(K, 1))()
@@ -462,8 +464,14 @@ class Heff:
             self._ops += [L, R]
         opts = HeffOpts(int(t_chunk_bytes), int(ring_bytes), int(kernel), int(split_waves), int(order_policy), int(per_pair_output))
         h = C.c_void_p()
-        check(self.lib.dmrgk_heff_create(ctx.h, layout.h, K, Larr, Rarr, coef.ctypes.data, flags.ctypes.data,
-                                         C.byref(opts), C.byref(h)))
+        if block_coef is None:
+            check(self.lib.dmrgk_heff_create(ctx.h, layout.h, K, Larr, Rarr, coef.ctypes.data, flags.ctypes.data,
+                                             C.byref(opts), C.byref(h)))
+        else:       # [K][n_blocks] recoupling scalars per (pair, input block)
+            bc = np.ascontiguousarray(block_coef, dtype=np.float64).reshape(max(K, 1), -1)
+            assert bc.shape[1] == layout.n_blocks
+            check(self.lib.dmrgk_heff_create_blockcoef(ctx.h, layout.h, K, Larr, Rarr, coef.ctypes.data, bc.ctypes.data,
+                                                       flags.ctypes.data, C.byref(opts), C.byref(h)))
         self.h = h
         q = self.query()
         self.n_tasks, self.flops_alg, self.flops_exec = q["n_tasks"], q["flops_alg"], q["flops_exec"]

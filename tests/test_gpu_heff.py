@@ -332,3 +332,44 @@ def test_edge_cases_and_errors():
     with pytest.raises(dmrgk.DmrgkError) as e:
         dp.heff.apply(v, v, dp.workspace)
     assert e.value.status == dmrgk.EINVAL
+
+
+def test_block_coefficients_su2_slot():
+    """dmrgk_heff_create_blockcoef: one extra scalar per (pair, input block) — the slot of the SU(2)
+    recoupling coefficients — against the oracle with random scalars (zeros remove
+    tasks), and the spin-singlet H_eff of the Hubbard dimer: σ and the Davidson energy against the
+    closed form (U − √(U² + 16t²))/2."""
+    from paper_2311_14106_b200 import problem
+    from _su2 import dimer_singlet_problem
+    from _util import golden_table
+
+    def on_device(pb, **opts):
+        dp = problem.DeviceProblem(pb.n_charges, pb.sectors_A, pb.sectors_B, pb.target)
+        dp.create_ops([(o["half"], o["dq"], o["parity"]) for o in pb.ops])
+        dp.alloc_resident()
+        for i, o in enumerate(pb.ops):
+            dp.set_op_host(i, o["blocks"])
+        r, c = dp.table[0], dp.table[1]
+        bc = np.ones((len(pb.terms), len(r)))
+        for (k, blk), v in pb.block_coef.items():
+            bc[k, [i for i in range(len(r)) if (int(r[i]), int(c[i])) == blk][0]] = v
+        dp.build(pb.terms, block_coef=bc, **opts)
+        return dp
+
+    pb = heff.problem_from_workload(medium_spinless())
+    rng = np.random.default_rng(5)
+    pb.block_coef = {(k, blk): (0.0 if rng.random() < 0.2 else float(rng.normal())) for k in range(len(pb.terms))
+                     for blk in pb.psi_blocks() if rng.random() < 0.7}
+    for opts in ({}, {"order_policy": 2}):
+        dp = on_device(pb, **opts)
+        assert rel_max(dp.to_blocks(dp.apply(dp.psi_from_host(pb.psi))), heff.sigma_blockwise(pb)) <= TOL_SIGMA
+        assert dp.heff.n_tasks == len(heff.enumerate_tasks(pb))
+    dim, H = dimer_singlet_problem()
+    dp = on_device(dim)
+    x = dp.psi_from_host(dim.psi)
+    assert rel_max(dp.to_blocks(dp.apply(x)), heff.sigma_dense(dim)) <= TOL_SIGMA
+    dav = dp.davidson(m_max=3, tol=1e-12, max_iter=50)
+    dav.start(x)
+    theta, rn, n_apply, ok = dav.solve(None)
+    E0 = float(golden_table("closed_forms.txt")["hubbard_dimer_E0_U4"])
+    assert ok and abs(theta - E0) <= 1e-9

@@ -136,3 +136,23 @@ def test_fermionic_sign_uses_input_A_parity():
     assert sig[(2, 0)][0, 0] == -1.0      # from input a-sector N=1 (odd)
     s2 = heff.sigma_dense(pb)
     assert s2[(1, 1)][0, 0] == +1.0 and s2[(2, 0)][0, 0] == -1.0
+
+
+def test_block_coefficients_blockwise_vs_kronecker_and_su2_dimer():
+    """The per-(pair, input block) scalar: T3 against T2 with random scalars incl.
+    zeros, and the spin-singlet H_eff of the Hubbard dimer against its closed form."""
+    import workloads as wlmod
+    from _su2 import dimer_singlet_problem
+    from _util import golden_table
+    pb = heff.problem_from_workload(wlmod.lattice_workload("spinless", 5, 24, seed=3))
+    rng = np.random.default_rng(5)
+    pb.block_coef = {(k, blk): (0.0 if rng.random() < 0.2 else float(rng.normal())) for k in range(len(pb.terms))
+                     for blk in pb.psi_blocks() if rng.random() < 0.7}
+    s2, s3 = heff.sigma_dense(pb), heff.sigma_blockwise(pb)
+    assert max(np.abs(s2[k] - s3[k]).max() for k in s2) < 1e-12
+    plain = heff.problem_from_workload(wlmod.lattice_workload("spinless", 5, 24, seed=3))
+    assert max(np.abs(heff.sigma_blockwise(plain)[k] - s3[k]).max() for k in s3) > 1e-3      # the scalars matter
+    dim, H = dimer_singlet_problem()
+    assert np.abs(heff.dense_heff(dim) - H).max() < 1e-14
+    E0 = float(golden_table("closed_forms.txt")["hubbard_dimer_E0_U4"])
+    assert abs(np.linalg.eigvalsh(heff.dense_heff(dim))[0] - E0) < 1e-12
