@@ -70,18 +70,20 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 //                                                                    [BK/16 k-panels × 64 rows × 16]
 //   MN-major (stored [k][i]): element (i, k) at (i >> 4)·16·BK + k·16 + ((i & 15) xor ((k & 3) << 2))
 //                                                                    [4 panels × BK k-rows × 16]
-// A lane (g = lane >> 2, t4 = lane & 3) of fragment f reads row i = w·32 + f·8 + g at k = 4·ks + t4:
-//   K-major : k0 + f·128 + (ks >> 2)·1024 + (((ks & 3) xor (g & 3)) << 2)    with k0 = (w·32 + g)·16 + t4
-//   MN-major: m[f & 1] + (f >> 1)·16·BK + ks·64     with m[h] = w·32·BK + t4·16 + ((8h + g) xor (t4 << 2))
+// A warp owns the 8-row fragments F0 … F0 + n − 1 of its operand tile (F0 = 0 for warp row/column 0, the
+// tile's fragments are split evenly over the two warp rows/columns, per unit).  A lane (g = lane >> 2,
+// t4 = lane & 3) of the warp's fragment f reads row i = (F0 + f)·8 + g at k = 4·ks + t4:
+//   K-major : k0 + f·128 + (ks >> 2)·1024 + (((ks & 3) xor (g & 3)) << 2)    with k0 = (F0·8 + g)·16 + t4
+//   MN-major: m[f & 1] + (f >> 1)·16·BK + ks·64     with m[h] = ((F0 + h) >> 1)·16·BK + t4·16 + ((8·((F0 + h) & 1) + g) xor (t4 << 2))
 // In both cases the 16 lanes of a half-warp hit 16 distinct 8-byte banks.
 struct FragBase {
     int k0, m0, m1;
 };
-__device__ __forceinline__ FragBase make_frag_base(int origin, int w, int g, int t4) {
+__device__ __forceinline__ FragBase make_frag_base(int origin, int F0, int g, int t4) {
     FragBase b;
-    b.k0 = origin + (w * 32 + g) * 16 + t4;
-    b.m0 = origin + w * 2 * MN_PANEL + t4 * 16 + (g ^ (t4 << 2));
-    b.m1 = origin + w * 2 * MN_PANEL + t4 * 16 + ((8 + g) ^ (t4 << 2));
+    b.k0 = origin + (F0 * 8 + g) * 16 + t4;
+    b.m0 = origin + (F0 >> 1) * MN_PANEL + t4 * 16 + ((8 * (F0 & 1) + g) ^ (t4 << 2));
+    b.m1 = origin + ((F0 + 1) >> 1) * MN_PANEL + t4 * 16 + ((8 * ((F0 + 1) & 1) + g) ^ (t4 << 2));
     return b;
 }
 template <bool MN>
@@ -222,10 +224,10 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
         };
         int4 s_lo = make_int4(0, 0, 0, 0), s_hi = make_int4(0, 0, 0, 0);
         while (cur < n_units) {
-            // fields of the unit (Unit layout: C, alpha | c_rp, i0, j0, mrows | ncols, ncols_st, seg_begin, seg_end | mode, nkt, -, -)
-            const int i0 = uw[1].y, j0 = uw[1].z, mrows = uw[1].w, ncols = uw[2].x;
+            // fields of the unit (Unit layout: C, alpha | c_rp, i0, j0, mrows | ncols, ncols_st, seg_begin, seg_end | mode, nkt, -, tile)
+            const int i0 = uw[1].y, j0 = uw[1].z, ncols = uw[2].x;
             const int seg_begin = uw[2].z, seg_end = uw[2].w;
-            const int rows_a = min(BM, mrows - i0), cols_b = min(BN, ncols - j0);
+            const int rows_a = int(uint32_t(uw[3].w) & 0xffffu), cols_b = min(int(uint32_t(uw[3].w) >> 16), ncols - j0);
             const int npa = (rows_a + 15) >> 4, npb = (cols_b + 15) >> 4;
             bool first = true;
             s_lo = __ldg(reinterpret_cast<const int4*>(segs + seg_begin));
@@ -307,7 +309,6 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
     // ================================ CONSUMERS ================================
     const int wm = warp >> 1, wn = warp & 1;
     const int g = lane >> 2, t4 = lane & 3, g3 = g & 3;
-    const FragBase fa = make_frag_base(0, wm, g, t4), fb = make_frag_base(OPER_DOUBLES, wn, g, t4);
     int stage = 0, ring_pos = 0;
     uint32_t ph = 0;
     while (true) {
@@ -315,11 +316,14 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
         const Unit u = ring[ring_pos];
         if (++ring_pos == RING) ring_pos = 0;
         if (u.nkt == 0) break;
-        const int rows_t = min(BM, u.mrows - u.i0);
-        const int cols_t = min(BN, u.ncols_st - u.j0);
-        const int cols_b = min(BN, u.ncols - u.j0);
-        const int nfm = max(0, min(4, (rows_t - wm * 32 + 7) >> 3));
-        const int nfn = max(0, min(4, (cols_b - wn * 32 + 7) >> 3));
+        // the tile's fragments, split evenly over the two warp rows and the two warp columns
+        const int rows_t = int(u.tile & 0xffffu), cols_t = int(u.tile >> 16);      // cols_t: stored columns (padded ld)
+        const int cols_b = min(cols_t, u.ncols - u.j0);                             // columns that hold data
+        const int fmt = (rows_t + 7) >> 3, fnt = (cols_b + 7) >> 3, fm0 = (fmt + 1) >> 1, fn0 = (fnt + 1) >> 1;
+        const int Fm = wm ? fm0 : 0, nfm = wm ? fmt - fm0 : fm0;
+        const int Fn = wn ? fn0 : 0, nfn = wn ? fnt - fn0 : fn0;
+        const int nfn_st = wn ? (cols_t >> 3) - fn0 : fn0;                          // incl. all-padding column fragments
+        const FragBase fa = make_frag_base(0, Fm, g, t4), fb = make_frag_base(OPER_DOUBLES, Fn, g, t4);
         const bool busy = nfm > 0 && nfn > 0;
         double acc[4][4][2];
 #pragma unroll
@@ -349,16 +353,17 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
         // epilogue: lane holds C[row g][cols 2·t4, 2·t4+1] of each 8×8 fragment
         double* C = reinterpret_cast<double*>(bases.b[(u.mode >> UNIT_C_SEL_SHIFT) & 3u] + u.C);
         const bool accum = (u.mode & UNIT_ACCUM) != 0, plain = (u.mode & UNIT_C_PLAIN) != 0;
-        const int rows_st = plain ? rows_t : min(BM, u.c_rp - u.i0);      // padding rows get zeros
+        // the block's last row tile also writes the padding rows (zeros)
+        const int rows_st = (plain || u.i0 + rows_t < u.mrows) ? rows_t : u.c_rp - u.i0;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            const int r = wm * 32 + i * 8 + g;
-            if (r >= rows_st) continue;
+            const int r = (Fm + i) * 8 + g;
+            if (i >= nfm || r >= rows_st) continue;
             const bool live = r < rows_t;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                const int c = wn * 32 + j * 8 + 2 * t4;
-                if (c >= cols_t) continue;
+                const int c = (Fn + j) * 8 + 2 * t4;
+                if (j >= nfn_st) continue;
                 double2* p = reinterpret_cast<double2*>(plain ? C + r * BN + c : C + panel_off(u.i0 + r, u.j0 + c, u.c_rp));
                 double2 v;
                 v.x = (live && u.j0 + c < u.ncols) ? u.alpha * acc[i][j][0] : 0.0;
@@ -380,8 +385,9 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
 __global__ void __launch_bounds__(NTHREADS)
 heff_gemm_scalar_kernel(const Unit* __restrict__ units, const Seg* __restrict__ segs, Bases bases) {
     const Unit u = units[blockIdx.x];
-    const int rows_t = (u.mode & UNIT_C_PLAIN) ? min(BM, u.mrows - u.i0) : min(BM, u.c_rp - u.i0);   // incl. padding rows
-    const int cols_t = min(BN, u.ncols_st - u.j0);
+    const int tr = int(u.tile & 0xffffu);
+    const int rows_t = ((u.mode & UNIT_C_PLAIN) || u.i0 + tr < u.mrows) ? tr : u.c_rp - u.i0;   // incl. padding rows
+    const int cols_t = int(u.tile >> 16);
     double* C = reinterpret_cast<double*>(bases.b[(u.mode >> UNIT_C_SEL_SHIFT) & 3u] + u.C);
     for (int e = threadIdx.x; e < rows_t * cols_t; e += NTHREADS) {
         const int r = e / cols_t, c = e % cols_t;

@@ -150,7 +150,8 @@ struct Seg {
 
 // One CTA work unit: a (≤64 × ≤64) tile of C summed over segments [seg_begin, seg_end).
 // C is a block in the panel layout (origin + rows_pad) or, with UNIT_C_PLAIN, a private row-major
-// 64×64 tile (split-k partial in the workspace).
+// 64×64 tile (split-k partial in the workspace).  Tiles of a block are BALANCED (tile_cuts): origins are
+// multiples of 16 and extents differ by at most 16, so the tile's explicit extent travels in `tile`.
 enum : uint32_t { UNIT_ACCUM = 1u, UNIT_C_PLAIN = 2u, UNIT_C_SEL_SHIFT = 4 };
 struct Unit {
     unsigned long long C;   // byte address / offset of the C block origin (or of the plain tile)
@@ -163,7 +164,8 @@ struct Unit {
     int32_t seg_begin, seg_end;
     uint32_t mode;      // UNIT_ACCUM | UNIT_C_PLAIN | selector << UNIT_C_SEL_SHIFT
     int32_t nkt;        // Σ over the unit's segments of ceil(klen/TILE_K); ≥ 1 (0 marks the stop sentinel)
-    int32_t pad_[2];
+    int32_t pad_;
+    uint32_t tile;      // tile rows | tile columns << 16 (columns over the padded ld: the STORED extent)
 };  // 64 B: four 16-byte words (the persistent kernel passes descriptors through shared memory)
 static_assert(sizeof(Unit) == 64, "Unit must be 64 bytes");
 
@@ -191,6 +193,29 @@ struct DiagBlock {
 
 constexpr int TILE_M = 64, TILE_N = 64;
 constexpr int TILE_K = 32;   // contraction depth of one pipeline stage (k-tile); Unit::nkt counts these
+
+// Balanced tiling of one block dimension: ceil(extent/64) tiles with origins at multiples of 16 (a panel
+// row group, so that an MN-major operand tile starts on a panel) and extents that differ by at most 16;
+// the larger tiles come first, the ragged end of the block falls into one of the smaller ones.  A tile's
+// 8-row fragments are then split evenly over the two warp rows (columns) of the CTA — the CTA advances at
+// the pace of its fullest warp, so 64 + 10 rows cost two full tiles, 48 + 26 cost 3/4 + 1/2
+// (profiles/r2_ragged.md).  `cuts` gets n + 1 entries, cuts[n] = extent.
+static inline void tile_cuts(int extent, std::vector<int>& cuts) {
+    cuts.clear();
+    const int panels = (extent + 15) / 16, n = (extent + TILE_M - 1) / TILE_M;
+    int p = 0;
+    for (int t = 0; t < n; ++t) {
+        cuts.push_back(p * 16);
+        p += panels / n + (t < panels % n ? 1 : 0);
+    }
+    cuts.push_back(extent);
+}
+static inline uint32_t pack_tile(int rows, int cols) { return uint32_t(rows) | (uint32_t(cols) << 16); }
+// cost of a tile per k-tile in fragment products of its fullest warp × 4 (a full 64×64 tile costs 64)
+static inline int64_t tile_cost(int rows, int cols) {
+    const int fm = (rows + 7) / 8, fn = (cols + 7) / 8;
+    return int64_t(4) * ((fm + 1) / 2) * ((fn + 1) / 2);
+}
 
 // kernel launchers (heff_kernels.cu)
 // `counter_dev`: a zeroed int the persistent kernel uses as its unit queue head (one per launch in flight)

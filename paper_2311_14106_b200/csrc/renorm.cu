@@ -22,7 +22,6 @@ struct RTask {
     const Block* outb;           // output block of out_i
 };
 
-int64_t tile_cost(int rows, int cols, int64_t nkt) { return int64_t((rows + 7) / 8) * ((cols + 7) / 8) * nkt; }
 
 template <class T>
 int32_t upload(const std::vector<T>& v, T** out) {
@@ -128,6 +127,7 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
             Unit u;
         };
         std::vector<CU> p1, p2;
+        std::vector<int> cut_r, cut_c;
         int64_t t_off = 0;
         for (const RTask& t : tasks) {
             const int e_r = t.ob->rows, e_c = t.ob->cols, n_c = t.pc->cols, n_r = t.pr->cols;
@@ -146,8 +146,11 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
             const int32_t si1 = int32_t(segs.size());
             segs.push_back(s1);
             const int64_t nkt1 = (e_c + TILE_K - 1) / TILE_K;
-            for (int r0 = 0; r0 < e_r; r0 += TILE_M)
-                for (int c0 = 0; c0 < ldt; c0 += TILE_N) {
+            tile_cuts(e_r, cut_r);
+            tile_cuts(ldt, cut_c);
+            for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
+                for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj) {
+                    const int r0 = cut_r[ti], c0 = cut_c[tj], rt = cut_r[ti + 1] - r0, ct = cut_c[tj + 1] - c0;
                     Unit u;
                     memset(&u, 0, sizeof(u));
                     u.C = (unsigned long long)t_off;            // block origin of T (e_r × n_c, panel layout)
@@ -162,7 +165,8 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
                     u.seg_end = si1 + 1;
                     u.mode = BASE_WS << UNIT_C_SEL_SHIFT;
                     u.nkt = int32_t(nkt1);
-                    p1.push_back({tile_cost(std::min(TILE_M, e_r - r0), std::min(TILE_N, ldt - c0), nkt1), u});
+                    u.tile = pack_tile(rt, ct);
+                    p1.push_back({tile_cost(rt, std::min(ct, n_c - c0)) * nkt1, u});
                 }
             // phase 2: out (n_r × n_c) = Φ[q+δ]ᵀ (M-major) · T (N-major)
             Seg s2;
@@ -177,8 +181,11 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
             segs.push_back(s2);
             const int64_t nkt2 = (e_r + TILE_K - 1) / TILE_K;
             const int ldo = t.outb->ld;
-            for (int r0 = 0; r0 < n_r; r0 += TILE_M)
-                for (int c0 = 0; c0 < ldo; c0 += TILE_N) {
+            tile_cuts(n_r, cut_r);
+            tile_cuts(ldo, cut_c);
+            for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
+                for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj) {
+                    const int r0 = cut_r[ti], c0 = cut_c[tj], rt = cut_r[ti + 1] - r0, ct = cut_c[tj + 1] - c0;
                     Unit u;
                     memset(&u, 0, sizeof(u));
                     u.C = (unsigned long long)(uintptr_t)(t.out + t.outb->off);     // block origin
@@ -193,7 +200,8 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
                     u.seg_end = si2 + 1;
                     u.mode = BASE_ABS << UNIT_C_SEL_SHIFT;
                     u.nkt = int32_t(nkt2);
-                    p2.push_back({tile_cost(std::min(TILE_M, n_r - r0), std::min(TILE_N, ldo - c0), nkt2), u});
+                    u.tile = pack_tile(rt, ct);
+                    p2.push_back({tile_cost(rt, std::min(ct, n_c - c0)) * nkt2, u});
                 }
             t_off += int64_t(pad_rows(e_r)) * ldt * 8;
         }

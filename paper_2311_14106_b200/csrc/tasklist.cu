@@ -43,9 +43,7 @@ struct OpRef {               // where an operator block lives
     int ld;
 };
 
-int64_t cost_of(int rows, int cols, int64_t nkt) {
-    return int64_t((rows + 7) / 8) * ((cols + 7) / 8) * nkt;
-}
+int64_t cost_of(int rows, int cols, int64_t nkt) { return tile_cost(rows, cols) * nkt; }
 
 template <class T>
 int32_t upload(const std::vector<T>& v, T** out) {
@@ -200,6 +198,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
     std::vector<DiagBlock> dblocks;
     std::vector<DiagTask> dtasks;
     const int64_t slots = int64_t(ctx->n_sm) * 3;
+    std::vector<int> cut_r, cut_c;                       // balanced tile boundaries of the block at hand (tile_cuts)
     int64_t max_t_bytes = 0, max_partial_tiles = 0, max_pairs = 0;
     const int64_t pp_vec_bytes = round_up(layout->n_padded * 8, 128);     // one σ_k buffer (per-pair mode)
 
@@ -410,8 +409,11 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                 (t.rfirst ? t.s2.B : t.s2.A) = (unsigned long long)t_off[i];
                 const int ldt = t.t_ld;
                 const int64_t nkt = (t.s1.klen + TILE_K - 1) / TILE_K;
-                for (int i0 = 0; i0 < t.t_rows; i0 += TILE_M)
-                    for (int j0 = 0; j0 < ldt; j0 += TILE_N) {
+                tile_cuts(t.t_rows, cut_r);
+                tile_cuts(ldt, cut_c);
+                for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
+                    for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj) {
+                        const int i0 = cut_r[ti], j0 = cut_c[tj], rt = cut_r[ti + 1] - i0, ct = cut_c[tj + 1] - j0;
                         Unit u;
                         memset(&u, 0, sizeof(u));
                         u.C = (unsigned long long)t_off[i];      // block origin of T_t
@@ -426,7 +428,8 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                         u.seg_end = int32_t(i) + 1;
                         u.mode = BASE_WS << UNIT_C_SEL_SHIFT;
                         u.nkt = int32_t(nkt);
-                        tmp.push_back({cost_of(std::min(TILE_M, t.t_rows - i0), std::min(TILE_N, ldt - j0), nkt), u});
+                        u.tile = pack_tile(rt, ct);
+                        tmp.push_back({cost_of(rt, std::min(ct, t.t_cols - j0), nkt), u});
                     }
             }
             std::stable_sort(tmp.begin(), tmp.end(), [](const U1& a, const U1& b) { return a.cost > b.cost; });
@@ -464,9 +467,11 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                 const int ob = gr.ob;
                 int64_t nkt = 0;
                 for (int i : gr.idx) nkt += (tasks[i].s2.klen + TILE_K - 1) / TILE_K;
-                for (int i0 = 0; i0 < pb[ob].rows; i0 += TILE_M)
-                    for (int j0 = 0; j0 < pb[ob].ld; j0 += TILE_N)
-                        total_cost += cost_of(std::min(TILE_M, pb[ob].rows - i0), std::min(TILE_N, pb[ob].ld - j0), nkt);
+                tile_cuts(pb[ob].rows, cut_r);
+                tile_cuts(pb[ob].ld, cut_c);
+                for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
+                    for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj)
+                        total_cost += cost_of(cut_r[ti + 1] - cut_r[ti], std::min(cut_c[tj + 1], pb[ob].cols) - cut_c[tj], nkt);
             }
             const int64_t target = o.per_pair_output ? (int64_t(1) << 60)
                                  : std::max<int64_t>(64 * 256 / TILE_K, total_cost / std::max<int64_t>(1, slots * o.split_waves));
@@ -493,10 +498,13 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                 const int ns = int(gr.idx.size());
                 const int64_t nkt = prefix.back();
                 const Block& B = pb[ob];
-                for (int i0 = 0; i0 < B.rows; i0 += TILE_M)
-                    for (int j0 = 0; j0 < B.ld; j0 += TILE_N) {
-                        const int rt = std::min(TILE_M, B.rows - i0), ct = std::min(TILE_N, B.ld - j0);
-                        const int64_t c = cost_of(rt, ct, nkt);
+                tile_cuts(B.rows, cut_r);
+                tile_cuts(B.ld, cut_c);
+                for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
+                    for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj) {
+                        const int i0 = cut_r[ti], j0 = cut_c[tj], rt = cut_r[ti + 1] - i0, ct = cut_c[tj + 1] - j0;
+                        const int cc = std::min(ct, B.cols - j0);      // columns that are computed (ct: stored)
+                        const int64_t c = cost_of(rt, cc, nkt);
                         int n_split = int(std::min<int64_t>(ns, (c + target - 1) / target));
                         if (n_split < 1) n_split = 1;
                         Unit u;
@@ -507,6 +515,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                         u.mrows = B.rows;
                         u.ncols = B.cols;
                         u.ncols_st = B.ld;
+                        u.tile = pack_tile(rt, ct);
                         const unsigned long long c_sigma = (unsigned long long)(B.off * 8);     // block origin in σ
                         u.c_rp = B.rows_pad;
                         if (o.per_pair_output) {
@@ -514,7 +523,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                             u.seg_begin = seg0;
                             u.seg_end = seg0 + ns;
                             u.mode = BASE_WS << UNIT_C_SEL_SHIFT;             // the only writer of this block: no accumulation
-                            u.pad_[0] = 1;
+                            u.pad_ = 1;
                             u.nkt = int32_t(nkt);
                             tmp.push_back({c, u, gi, 0});
                         } else if (n_split == 1) {
@@ -546,7 +555,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                                 u.seg_end = seg0 + se;
                                 u.mode = UNIT_C_PLAIN | (BASE_WS << UNIT_C_SEL_SHIFT);
                                 u.nkt = int32_t(prefix[se] - prefix[sb]);
-                                tmp.push_back({cost_of(rt, ct, u.nkt), u, gi, made});
+                                tmp.push_back({cost_of(rt, cc, u.nkt), u, gi, made});
                                 ++made;
                                 sb = se;
                             }
@@ -637,9 +646,9 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
             units[i].seg_begin += int32_t(c.p2_seg0);
             units[i].seg_end += int32_t(c.p2_seg0);
             if (units[i].mode & UNIT_C_PLAIN) units[i].C += part_base;
-            if (units[i].pad_[0]) {
+            if (units[i].pad_) {
                 units[i].C += (unsigned long long)h->pp_base;
-                units[i].pad_[0] = 0;
+                units[i].pad_ = 0;
             }
         }
         for (int64_t i = c.r_unit0; i < c.r_unit0 + c.r_units; ++i) runits[i].P += part_base;
