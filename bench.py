@@ -737,6 +737,56 @@ def run_loop_probe(args):
     print(json.dumps(out), flush=True)
 
 
+def flat_workload(dim_a, dim_b, n_half=8, seed=11):
+    """A lattice-shaped operator-pair list (families F0-F4 of n_half spinless modes per half) over FLAT sectors:
+    every A sector has dim_a states, every B sector dim_b — all blocks the same shape, so that the cost of ragged
+    tile edges can be read off by comparing shapes (--op ragged)."""
+    from workloads.configs import Workload, _family_builder, spinless_term_structure
+    sa = [((q,), dim_a) for q in range(n_half + 1)]
+    sb = [((q,), dim_b) for q in range(n_half + 1)]
+    wl = Workload(f"flat_{dim_a}x{dim_b}", seed, 1, sa, sb, (n_half,))
+    sh = spinless_term_structure(n_half, n_half)
+    return _family_builder(wl, sh[0], sh[1])
+
+
+def run_ragged(args):
+    """--op ragged: the product kernel on flat-sector workloads — multiples of the 64-wide tile against ragged
+    dims — with the phases timed one after the other (dmrgk_heff_profile(2)).  Phase 1 is m' x n with k = m,
+    phase 2 m' x n' with k = n (stacked); here m = m' = dim_a, n = n' = dim_b.  Not a product number: it is
+    the evidence for the balanced tiling of DESIGN.md §4.1 (profiles/r2_ragged.md)."""
+    import torch
+    import workloads as wlmod
+    from paper_2311_14106_b200 import dmrgk, problem
+    torch.cuda.set_device(0)
+    dmrgk.load()
+    rows = []
+    for da, db in ((512, 512), (500, 512), (512, 500), (500, 500), (640, 640), (650, 650), (256, 256), (250, 250), (128, 128), (120, 120)):
+        wl = flat_workload(da, db)
+        opts = {"kernel": args.kernel} if args.kernel else {}
+        dp = problem.from_workload(wl, device=0, **opts)
+        psi = dp.psi_fill(wl.seed, wlmod.PSI_STREAM)
+        sig = dp.new_vector(zero=False)
+        for _ in range(3):
+            dp.apply(psi, sig)
+        ms = min(timed(dp.stream, lambda: dp.apply(psi, sig)) for _ in range(10))
+        h = dp.heff
+        h.profile(2)
+        for _ in range(5):
+            dp.apply(psi, sig)
+        torch.cuda.synchronize()
+        pm, _ = h.profile_read()
+        h.profile(0)
+        f1 = 2.0 * da * da * db * h.n_tasks      # identity factors of F0 included: approximate split of flops_alg
+        f2 = 2.0 * da * db * db * h.n_tasks
+        rows.append({"dim_a": da, "dim_b": db, "tasks": h.n_tasks, "chunks": h.n_chunks, "apply_ms": round(ms, 3),
+                     "apply_tflops": round(h.flops_alg / ms / 1e9, 2),
+                     "phase1_ms": round(pm["p1"] / 5, 3), "phase2_ms": round(pm["p2"] / 5, 3),
+                     "phase1_tflops": round(f1 / (pm["p1"] / 5) / 1e9, 2), "phase2_tflops": round(f2 / (pm["p2"] / 5) / 1e9, 2)})
+        del dp, psi, sig
+        torch.cuda.empty_cache()
+    print(json.dumps({"op": "ragged", "source_hash": dmrgk.source_hash(), "kernel_variant": args.kernel, "rows": rows}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -754,7 +804,7 @@ def main():
     ap.add_argument("--shard", default="none", choices=["none", "k"],
                     help="N > 1 only: 'none' = independent replicas (the scope of BASELINE.json), 'k' = split the operator-pair "
                          "list over the ranks and all-reduce sigma (SURVEY §8(f) NEXT-2)")
-    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "enlarge", "loop_probe"],
+    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "enlarge", "loop_probe", "ragged"],
                     help="davidson (default, the headline hot path) or renorm (NEXT-1 row, its own metric)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -765,6 +815,8 @@ def main():
         run_enlarge(args)
     elif args.op == "loop_probe":
         run_loop_probe(args)
+    elif args.op == "ragged":
+        run_ragged(args)
     else:
         run_ours(args)
 
