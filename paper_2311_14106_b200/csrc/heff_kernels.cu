@@ -21,13 +21,14 @@
 
 namespace dmrgk {
 
-constexpr int BM = TILE_M, BN = TILE_N, BK = TILE_K;
-constexpr int NTHREADS = 128;           // 4 warps as 2×2, each a 32×32 warp tile = 4×4 DMMA frags
-constexpr int KP = BK / 16;              // 16-column k-panels per k-tile
-constexpr int OPER_DOUBLES = BM * BK;    // one operand tile, dense 128-byte rows
-constexpr int STAGE_DOUBLES = 2 * OPER_DOUBLES;
+// The kernel is a template on WM, the 8-row fragments a warp holds along M: WM = 4 gives the 64×64 CTA
+// tile (2×2 warps of 32×32), WM = 8 the tall 128×64 tile (2×2 warps of 64×32).
+constexpr int BN = TILE_N, BK = TILE_K;
+constexpr int NTHREADS = 128;
+constexpr int B_DOUBLES = BN * BK;       // the B operand tile, dense 128-byte rows
 constexpr int MN_PANEL = BK * 16;        // doubles of one 16-column panel of an MN-major tile (BK k-rows)
-constexpr int smem_bytes(int stages) { return stages * STAGE_DOUBLES * 8; }
+constexpr int stage_doubles(int wm) { return wm * 16 * BK + B_DOUBLES; }
+constexpr int smem_bytes(int wm, int stages) { return stages * stage_doubles(wm) * 8; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -67,7 +68,7 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 // ---- consumer ----------------------------------------------------------------------------------
 // Shared image of an operand tile (doubles from the operand's origin in the stage):
 //   K-major  (stored [i][k]): element (i, k) at (k >> 4)·1024 + i·16 + ((k & 15) xor ((i & 3) << 2))
-//                                                                    [BK/16 k-panels × 64 rows × 16]
+//                                                            [BK/16 k-panels × tile rows (64 | 128) × 16]
 //   MN-major (stored [k][i]): element (i, k) at (i >> 4)·16·BK + k·16 + ((i & 15) xor ((k & 3) << 2))
 //                                                                    [4 panels × BK k-rows × 16]
 // A warp owns the 8-row fragments F0 … F0 + n − 1 of its operand tile (F0 = 0 for warp row/column 0, the
@@ -86,25 +87,27 @@ __device__ __forceinline__ FragBase make_frag_base(int origin, int F0, int g, in
     b.m1 = origin + ((F0 + 1) >> 1) * MN_PANEL + t4 * 16 + ((8 * ((F0 + 1) & 1) + g) ^ (t4 << 2));
     return b;
 }
-template <bool MN>
+// KSTRIDE: doubles between the 16-column k-panels of a K-major operand tile (its rows × 16)
+template <bool MN, int KSTRIDE>
 __device__ __forceinline__ double frag(const double* __restrict__ st, const FragBase& b, int g3, int f, int ks) {
     if (MN) return st[((f & 1) ? b.m1 : b.m0) + (f >> 1) * MN_PANEL + ks * 64];
-    return st[b.k0 + f * 128 + (ks >> 2) * 1024 + (((ks & 3) ^ g3) << 2)];
+    return st[b.k0 + f * 128 + (ks >> 2) * KSTRIDE + (((ks & 3) ^ g3) << 2)];
 }
 
 // One k-tile (BK = 16, `nks` steps of 4) of a warp tile of FM × FN fragments.  FM, FN and the operand
 // layouts are compile-time: accumulator indices are static and no DMMA carries a guard.
-template <int FM, int FN, bool AM, bool BN_, bool FULLK>
+template <int WM, int FM, int FN, bool AM, bool BN_, bool FULLK>
 __device__ __forceinline__ void mma_ktile(const double* __restrict__ st, const FragBase& fa, const FragBase& fb, int g3,
-                                          int nks, double (&acc)[4][4][2]) {
+                                          int nks, double (&acc)[WM][4][2]) {
+    constexpr int KA = WM * 256, KB = 1024;
     if (FULLK) {
 #pragma unroll
         for (int ks = 0; ks < BK / 4; ++ks) {
             double af[FM], bf[FN];
 #pragma unroll
-            for (int f = 0; f < FM; ++f) af[f] = frag<AM>(st, fa, g3, f, ks);
+            for (int f = 0; f < FM; ++f) af[f] = frag<AM, KA>(st, fa, g3, f, ks);
 #pragma unroll
-            for (int f = 0; f < FN; ++f) bf[f] = frag<BN_>(st, fb, g3, f, ks);
+            for (int f = 0; f < FN; ++f) bf[f] = frag<BN_, KB>(st, fb, g3, f, ks);
 #pragma unroll
             for (int i = 0; i < FM; ++i)
 #pragma unroll
@@ -115,9 +118,9 @@ __device__ __forceinline__ void mma_ktile(const double* __restrict__ st, const F
         for (int ks = 0; ks < nks; ++ks) {
             double af[FM], bf[FN];
 #pragma unroll
-            for (int f = 0; f < FM; ++f) af[f] = frag<AM>(st, fa, g3, f, ks);
+            for (int f = 0; f < FM; ++f) af[f] = frag<AM, KA>(st, fa, g3, f, ks);
 #pragma unroll
-            for (int f = 0; f < FN; ++f) bf[f] = frag<BN_>(st, fb, g3, f, ks);
+            for (int f = 0; f < FN; ++f) bf[f] = frag<BN_, KB>(st, fb, g3, f, ks);
 #pragma unroll
             for (int i = 0; i < FM; ++i)
 #pragma unroll
@@ -126,29 +129,42 @@ __device__ __forceinline__ void mma_ktile(const double* __restrict__ st, const F
     }
 }
 
-template <int FM, bool AM, bool BN_>
+template <int WM, int FM, bool AM, bool BN_>
 __device__ __forceinline__ void mma_ktile_n(int nfn, const double* st, const FragBase& fa, const FragBase& fb, int g3,
-                                            int nks, double (&acc)[4][4][2]) {
+                                            int nks, double (&acc)[WM][4][2]) {
     switch (nfn) {
-        case 1: mma_ktile<FM, 1, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
-        case 2: mma_ktile<FM, 2, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
-        case 3: mma_ktile<FM, 3, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
-        default: mma_ktile<FM, 4, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
+        case 1: mma_ktile<WM, FM, 1, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
+        case 2: mma_ktile<WM, FM, 2, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
+        case 3: mma_ktile<WM, FM, 3, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
+        default: mma_ktile<WM, FM, 4, AM, BN_, false>(st, fa, fb, g3, nks, acc); break;
     }
 }
 
 // All fragment shapes of one operand-layout combination; branches are warp-uniform.
-template <bool AM, bool BN_>
+template <int WM, bool AM, bool BN_>
 __device__ __forceinline__ void mma_layout(int nfm, int nfn, int nks, const double* st, const FragBase& fa,
-                                           const FragBase& fb, int g3, double (&acc)[4][4][2]) {
-    if (nfm == 4 && nfn == 4 && nks == BK / 4) {
-        mma_ktile<4, 4, AM, BN_, true>(st, fa, fb, g3, BK / 4, acc);
+                                           const FragBase& fb, int g3, double (&acc)[WM][4][2]) {
+    if (nfm == WM && nfn == 4 && nks == BK / 4) {
+        mma_ktile<WM, WM, 4, AM, BN_, true>(st, fa, fb, g3, BK / 4, acc);
     } else {
-        switch (nfm) {
-            case 1: mma_ktile_n<1, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
-            case 2: mma_ktile_n<2, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
-            case 3: mma_ktile_n<3, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
-            default: mma_ktile_n<4, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+        if constexpr (WM > 4) {
+            switch (nfm) {
+                case 1: mma_ktile_n<WM, 1, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                case 2: mma_ktile_n<WM, 2, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                case 3: mma_ktile_n<WM, 3, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                case 4: mma_ktile_n<WM, 4, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                case 5: mma_ktile_n<WM, 5, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                case 6: mma_ktile_n<WM, 6, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                case 7: mma_ktile_n<WM, 7, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                default: mma_ktile_n<WM, 8, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+            }
+        } else {
+            switch (nfm) {
+                case 1: mma_ktile_n<WM, 1, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                case 2: mma_ktile_n<WM, 2, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                case 3: mma_ktile_n<WM, 3, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+                default: mma_ktile_n<WM, 4, AM, BN_>(nfn, st, fa, fb, g3, nks, acc); break;
+            }
         }
     }
 }
@@ -171,11 +187,12 @@ struct StageNote {
 // The stop signal is a descriptor with nkt = 0 published through the same ring on a data-less tile.
 constexpr int P_NTHREADS = 160;
 
-template <int STAGES, int MIN_CTAS>
+template <int WM, int STAGES, int MIN_CTAS>
 __global__ void __launch_bounds__(P_NTHREADS, MIN_CTAS)
 heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __restrict__ segs, int n_units,
                                  int* __restrict__ queue_head, Bases bases) {
     constexpr int RING = STAGES + 1;       // a unit has ≥ 1 tile, the producer runs ≤ STAGES tiles ahead
+    constexpr int A_DOUBLES = WM * 16 * BK, STAGE_DOUBLES = A_DOUBLES + B_DOUBLES;
     extern __shared__ __align__(128) double smem[];
     __shared__ __align__(8) unsigned long long bars[2 * STAGES];   // full[0..S), empty[S..2S)
     __shared__ StageNote notes[STAGES];
@@ -264,10 +281,10 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                     // one is ceil(extent/16) panels of (nk4 × 128 B); the elected lane issues them one by one
                     // (UBLKCP takes uniform operands, so spreading them over lanes would be serialised anyway)
                     if (lane == 0) {
-                        const uint32_t dA = smem_base + stage * (STAGE_DOUBLES * 8), dB = dA + OPER_DOUBLES * 8;
+                        const uint32_t dA = smem_base + stage * (STAGE_DOUBLES * 8), dB = dA + A_DOUBLES * 8;
                         if (!am) {
                             for (int kp = 0; kp < nkp; ++kp)
-                                bulk_g2s(dA + kp * 8192, A + (int64_t((k0 >> 4) + kp) * a_rp + i0) * 128, uint32_t(rows_a * 128), full);
+                                bulk_g2s(dA + kp * (WM * 2048), A + (int64_t((k0 >> 4) + kp) * a_rp + i0) * 128, uint32_t(rows_a * 128), full);
                         } else {
                             for (int pp = 0; pp < npa; ++pp)
                                 bulk_g2s(dA + pp * (MN_PANEL * 8), A + (int64_t((i0 >> 4) + pp) * a_rp + k0) * 128, uint32_t(nk4 * 128), full);
@@ -323,11 +340,11 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
         const int Fm = wm ? fm0 : 0, nfm = wm ? fmt - fm0 : fm0;
         const int Fn = wn ? fn0 : 0, nfn = wn ? fnt - fn0 : fn0;
         const int nfn_st = wn ? (cols_t >> 3) - fn0 : fn0;                          // incl. all-padding column fragments
-        const FragBase fa = make_frag_base(0, Fm, g, t4), fb = make_frag_base(OPER_DOUBLES, Fn, g, t4);
+        const FragBase fa = make_frag_base(0, Fm, g, t4), fb = make_frag_base(A_DOUBLES, Fn, g, t4);
         const bool busy = nfm > 0 && nfn > 0;
-        double acc[4][4][2];
+        double acc[WM][4][2];
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < WM; ++i)
 #pragma unroll
             for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 #pragma unroll 1
@@ -337,10 +354,10 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                 const StageNote note = notes[stage];
                 const double* st = smem + stage * STAGE_DOUBLES;
                 switch (note.flags & (SEG_A_MMAJOR | SEG_B_NMAJOR)) {
-                    case 0: mma_layout<false, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
-                    case SEG_A_MMAJOR: mma_layout<true, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
-                    case SEG_B_NMAJOR: mma_layout<false, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
-                    default: mma_layout<true, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                    case 0: mma_layout<WM, false, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                    case SEG_A_MMAJOR: mma_layout<WM, true, false>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                    case SEG_B_NMAJOR: mma_layout<WM, false, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
+                    default: mma_layout<WM, true, true>(nfm, nfn, note.nks, st, fa, fb, g3, acc); break;
                 }
             }
             __syncwarp();
@@ -356,7 +373,7 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
         // the block's last row tile also writes the padding rows (zeros)
         const int rows_st = (plain || u.i0 + rows_t < u.mrows) ? rows_t : u.c_rp - u.i0;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < WM; ++i) {
             const int r = (Fm + i) * 8 + g;
             if (i >= nfm || r >= rows_st) continue;
             const bool live = r < rows_t;
@@ -413,13 +430,13 @@ heff_gemm_scalar_kernel(const Unit* __restrict__ units, const Seg* __restrict__ 
 }
 
 // a7: fixed-order sum of split-k partial tiles, σ_tile += Σ_s P_s (s ascending).  Eight CTAs per tile
-// (one 8-row slab each, one double2 per thread) so that even a handful of output tiles fills the GPU;
+// (one 8-row slab each, one double2 per thread; 16 for the tall tile) so that even a handful of output tiles fills the GPU;
 // the partial loads of four splits are issued together, the additions stay in split order.
-constexpr int RED_SLABS = BM / 8;
 __global__ void __launch_bounds__(256)
-heff_reduce_kernel(const RUnit* __restrict__ runits, Bases bases) {
-    const RUnit u = runits[blockIdx.x / RED_SLABS];
-    const int r = (blockIdx.x % RED_SLABS) * 8 + (threadIdx.x >> 5);
+heff_reduce_kernel(const RUnit* __restrict__ runits, Bases bases, int slabs) {      // slabs = tile rows / 8
+    const RUnit u = runits[blockIdx.x / slabs];
+    const int r = (blockIdx.x % slabs) * 8 + (threadIdx.x >> 5);
+    const int64_t tile_d2 = int64_t(slabs) * 8 * BN / 2;                             // double2s per partial tile
     const int c = (threadIdx.x & 31) * 2;
     if (r >= u.rows || c >= u.cols) return;   // cols is even (multiple of 16 or the tile width 64)
     double2* p = reinterpret_cast<double2*>(reinterpret_cast<double*>(bases.b[BASE_SIGMA] + u.C) + panel_off(u.i0 + r, u.j0 + c, u.c_rp));
@@ -429,7 +446,7 @@ heff_reduce_kernel(const RUnit* __restrict__ runits, Bases bases) {
     for (; s + 4 <= u.n_split; s += 4) {
         double2 q[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) q[j] = P[int64_t(s + j) * (BM * BN / 2)];
+        for (int j = 0; j < 4; ++j) q[j] = P[int64_t(s + j) * tile_d2];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             v.x += q[j].x;
@@ -437,7 +454,7 @@ heff_reduce_kernel(const RUnit* __restrict__ runits, Bases bases) {
         }
     }
     for (; s < u.n_split; ++s) {
-        const double2 q = P[int64_t(s) * (BM * BN / 2)];
+        const double2 q = P[int64_t(s) * tile_d2];
         v.x += q.x;
         v.y += q.y;
     }
@@ -485,30 +502,36 @@ heff_diag_kernel(const DiagBlock* __restrict__ blocks, const DiagTask* __restric
 static int g_gemm_ctas_per_sm = 0;
 int gemm_ctas_per_sm() { return g_gemm_ctas_per_sm; }
 
-// Kernel variants (dmrgk_heff_opts.kernel): 0 = product path, 3 CTAs per SM with 64 KB of stages each;
-// 1 = scalar check kernel; 2 = 2 CTAs per SM with 96 KB of stages; 3 = 2 CTAs per SM with 64 KB — other
-// residencies of the same persistent kernel, kept for measurement (profiles/r2_tma_summary.md).
-constexpr int ST64 = 65536 / (STAGE_DOUBLES * 8), ST96 = 98304 / (STAGE_DOUBLES * 8);
+// Kernel variants (dmrgk_heff_opts.kernel): 0 = 64×64 tiles, 3 CTAs per SM with 64 KB of stages each;
+// 1 = scalar check kernel; 2 = 64×64, 2 CTAs per SM with 96 KB of stages; 3 = 64×64, 2 CTAs per SM with
+// 64 KB; 4 = the tall 128×64 tile (2×2 warps of 64×32: 128 accumulator registers), 2 CTAs per SM with 96 KB
+// of stages — a CTA of 5 warps at 2 CTAs per SM is capped at 168 registers, so this variant spills and is
+// slower than variant 0 on every shape measured (profiles/r2_ragged.md); kept, like 2 and 3, for measurement.
+constexpr int ST64 = 65536 / (stage_doubles(4) * 8), ST96 = 98304 / (stage_doubles(4) * 8), ST96T = 98304 / (stage_doubles(8) * 8);
 template <class K>
-static int32_t setup_kernel(K* fn, int threads, int stages, int min_ctas, int* resident) {
-    DMRGK_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes(stages)));
+static int32_t setup_kernel(K* fn, int threads, int smem, int min_ctas, int* resident) {
+    DMRGK_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     // the L1/shared split must leave room for min_ctas CTAs: ask for the largest shared-memory carve-out
     // and verify the residency instead of trusting the driver's heuristic
     DMRGK_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     int n = 0;
-    DMRGK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, threads, smem_bytes(stages)));
+    DMRGK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, threads, smem));
     if (resident) *resident = n;
     if (n < min_ctas)
-        return fail(DMRGK_ECUDA, "gemm kernel <%d stages, %d CTAs>: only %d CTA(s) per SM resident", stages, min_ctas, n);
+        return fail(DMRGK_ECUDA, "gemm kernel <%d B of stages, %d CTAs>: only %d CTA(s) per SM resident", smem, min_ctas, n);
     return DMRGK_OK;
 }
 
 int32_t gemm_kernel_setup() {
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<ST64, 3>, P_NTHREADS, ST64, 3, &g_gemm_ctas_per_sm));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<ST96, 2>, P_NTHREADS, ST96, 2, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<ST64, 2>, P_NTHREADS, ST64, 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3>, P_NTHREADS, smem_bytes(4, ST64), 3, &g_gemm_ctas_per_sm));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST96, 2>, P_NTHREADS, smem_bytes(4, ST96), 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 2>, P_NTHREADS, smem_bytes(4, ST64), 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<8, ST96T, 2>, P_NTHREADS, smem_bytes(8, ST96T), 2, nullptr));
     return DMRGK_OK;
 }
+
+int gemm_tile_m(int kernel) { return kernel == 4 ? 128 : 64; }
+int gemm_ctas(int kernel) { return (kernel == 0 || kernel == 1) ? 3 : 2; }
 
 int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
                           const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm) {
@@ -519,18 +542,20 @@ int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev
     if (kernel != 1 && !counter_dev) return fail(DMRGK_EINVAL, "launch_gemm_units: the persistent kernel needs a queue counter");
     switch (kernel) {
         case 1: heff_gemm_scalar_kernel<<<unsigned(n_units), NTHREADS, 0, st>>>(units_dev, segs_dev, bases); break;
-        case 2: heff_gemm_dmma_persistent_kernel<ST96, 2><<<pgrid(2), P_NTHREADS, smem_bytes(ST96), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        case 3: heff_gemm_dmma_persistent_kernel<ST64, 2><<<pgrid(2), P_NTHREADS, smem_bytes(ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        default: heff_gemm_dmma_persistent_kernel<ST64, 3><<<pgrid(3), P_NTHREADS, smem_bytes(ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 2: heff_gemm_dmma_persistent_kernel<4, ST96, 2><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST96), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 3: heff_gemm_dmma_persistent_kernel<4, ST64, 2><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 4: heff_gemm_dmma_persistent_kernel<8, ST96T, 2><<<pgrid(2), P_NTHREADS, smem_bytes(8, ST96T), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        default: heff_gemm_dmma_persistent_kernel<4, ST64, 3><<<pgrid(3), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
     }
     count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;
 }
 
-int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cudaStream_t st) {
+int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cudaStream_t st, int tile_m) {
     if (n <= 0) return DMRGK_OK;
-    heff_reduce_kernel<<<unsigned(n * RED_SLABS), 256, 0, st>>>(runits_dev, bases);
+    const int slabs = tile_m / 8;
+    heff_reduce_kernel<<<unsigned(n * slabs), 256, 0, st>>>(runits_dev, bases, slabs);
     count_launch();
     DMRGK_CUDA(cudaGetLastError());
     return DMRGK_OK;

@@ -194,15 +194,15 @@ struct DiagBlock {
 constexpr int TILE_M = 64, TILE_N = 64;
 constexpr int TILE_K = 32;   // contraction depth of one pipeline stage (k-tile); Unit::nkt counts these
 
-// Balanced tiling of one block dimension: ceil(extent/64) tiles with origins at multiples of 16 (a panel
+// Balanced tiling of one block dimension: ceil(extent/tile_max) tiles (tile_max = 64, or 128 rows for the tall tile) with origins at multiples of 16 (a panel
 // row group, so that an MN-major operand tile starts on a panel) and extents that differ by at most 16;
 // the larger tiles come first, the ragged end of the block falls into one of the smaller ones.  A tile's
 // 8-row fragments are then split evenly over the two warp rows (columns) of the CTA — the CTA advances at
 // the pace of its fullest warp, so 64 + 10 rows cost two full tiles, 48 + 26 cost 3/4 + 1/2
 // (profiles/r2_ragged.md).  `cuts` gets n + 1 entries, cuts[n] = extent.
-static inline void tile_cuts(int extent, std::vector<int>& cuts) {
+static inline void tile_cuts(int extent, int tile_max, std::vector<int>& cuts) {
     cuts.clear();
-    const int panels = (extent + 15) / 16, n = (extent + TILE_M - 1) / TILE_M;
+    const int panels = (extent + 15) / 16, n = (extent + tile_max - 1) / tile_max;
     int p = 0;
     for (int t = 0; t < n; ++t) {
         cuts.push_back(p * 16);
@@ -221,7 +221,9 @@ static inline int64_t tile_cost(int rows, int cols) {
 // `counter_dev`: a zeroed int the persistent kernel uses as its unit queue head (one per launch in flight)
 int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
                           const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm);
-int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cudaStream_t st);
+int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cudaStream_t st, int tile_m);
+int gemm_tile_m(int kernel);   // rows of the CTA tile of a kernel variant (64, or 128 for the tall tile)
+int gemm_ctas(int kernel);     // CTAs per SM the variant is launched with
 int32_t launch_diag(const DiagBlock* blocks_dev, const DiagTask* tasks_dev, int64_t n_blocks,
                     double* diag, const Bases& bases, cudaStream_t st);
 int32_t gemm_kernel_setup();   // opt-in shared memory attribute, once

@@ -64,7 +64,7 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
     const bool default_chunk = o.t_chunk_bytes <= 0;
-    if (o.kernel < 0 || o.kernel > 3) return fail(DMRGK_EINVAL, "renorm_create: bad options");
+    if (o.kernel < 0 || o.kernel > 4) return fail(DMRGK_EINVAL, "renorm_create: bad options");
     for (int64_t i = 0; i < n_ops; ++i) {
         if (!in[i] || !out[i]) return fail(DMRGK_EINVAL, "renorm_create: operator %lld is NULL", (long long)i);
         if (in[i]->space != phi->enl) return fail(DMRGK_ESHAPE, "renorm_create: in[%lld] is not on phi's enlarged space", (long long)i);
@@ -128,6 +128,7 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
         };
         std::vector<CU> p1, p2;
         std::vector<int> cut_r, cut_c;
+        const int tile_m = gemm_tile_m(o.kernel);
         int64_t t_off = 0;
         for (const RTask& t : tasks) {
             const int e_r = t.ob->rows, e_c = t.ob->cols, n_c = t.pc->cols, n_r = t.pr->cols;
@@ -146,8 +147,8 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
             const int32_t si1 = int32_t(segs.size());
             segs.push_back(s1);
             const int64_t nkt1 = (e_c + TILE_K - 1) / TILE_K;
-            tile_cuts(e_r, cut_r);
-            tile_cuts(ldt, cut_c);
+            tile_cuts(e_r, tile_m, cut_r);
+            tile_cuts(ldt, TILE_N, cut_c);
             for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
                 for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj) {
                     const int r0 = cut_r[ti], c0 = cut_c[tj], rt = cut_r[ti + 1] - r0, ct = cut_c[tj + 1] - c0;
@@ -181,8 +182,8 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
             segs.push_back(s2);
             const int64_t nkt2 = (e_r + TILE_K - 1) / TILE_K;
             const int ldo = t.outb->ld;
-            tile_cuts(n_r, cut_r);
-            tile_cuts(ldo, cut_c);
+            tile_cuts(n_r, tile_m, cut_r);
+            tile_cuts(ldo, TILE_N, cut_c);
             for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
                 for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj) {
                     const int r0 = cut_r[ti], c0 = cut_c[tj], rt = cut_r[ti + 1] - r0, ct = cut_c[tj + 1] - c0;

@@ -127,7 +127,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
     if (o.split_waves <= 0) o.split_waves = 32;   // units per CTA slot: the queue's tail is ≈ one unit long
-    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 3) || o.order_policy < 0 || o.order_policy > 2 ||
+    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 4) || o.order_policy < 0 || o.order_policy > 2 ||
         (o.per_pair_output != 0 && o.per_pair_output != 1))
         return fail(DMRGK_EINVAL, "heff_create: bad options");
     const int64_t ring_part = (o.ring_bytes / 3) / 128 * 128;   // three parts: see dmrgk_heff_apply
@@ -197,7 +197,8 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
     std::vector<RUnit> runits;
     std::vector<DiagBlock> dblocks;
     std::vector<DiagTask> dtasks;
-    const int64_t slots = int64_t(ctx->n_sm) * 3;
+    const int tile_m = gemm_tile_m(o.kernel);            // rows of the CTA tile: 64, or 128 for the tall-tile variant
+    const int64_t slots = int64_t(ctx->n_sm) * gemm_ctas(o.kernel);
     std::vector<int> cut_r, cut_c;                       // balanced tile boundaries of the block at hand (tile_cuts)
     int64_t max_t_bytes = 0, max_partial_tiles = 0, max_pairs = 0;
     const int64_t pp_vec_bytes = round_up(layout->n_padded * 8, 128);     // one σ_k buffer (per-pair mode)
@@ -409,8 +410,8 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                 (t.rfirst ? t.s2.B : t.s2.A) = (unsigned long long)t_off[i];
                 const int ldt = t.t_ld;
                 const int64_t nkt = (t.s1.klen + TILE_K - 1) / TILE_K;
-                tile_cuts(t.t_rows, cut_r);
-                tile_cuts(ldt, cut_c);
+                tile_cuts(t.t_rows, tile_m, cut_r);
+                tile_cuts(ldt, TILE_N, cut_c);
                 for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
                     for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj) {
                         const int i0 = cut_r[ti], j0 = cut_c[tj], rt = cut_r[ti + 1] - i0, ct = cut_c[tj + 1] - j0;
@@ -467,8 +468,8 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                 const int ob = gr.ob;
                 int64_t nkt = 0;
                 for (int i : gr.idx) nkt += (tasks[i].s2.klen + TILE_K - 1) / TILE_K;
-                tile_cuts(pb[ob].rows, cut_r);
-                tile_cuts(pb[ob].ld, cut_c);
+                tile_cuts(pb[ob].rows, tile_m, cut_r);
+                tile_cuts(pb[ob].ld, TILE_N, cut_c);
                 for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
                     for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj)
                         total_cost += cost_of(cut_r[ti + 1] - cut_r[ti], std::min(cut_c[tj + 1], pb[ob].cols) - cut_c[tj], nkt);
@@ -498,8 +499,8 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                 const int ns = int(gr.idx.size());
                 const int64_t nkt = prefix.back();
                 const Block& B = pb[ob];
-                tile_cuts(B.rows, cut_r);
-                tile_cuts(B.ld, cut_c);
+                tile_cuts(B.rows, tile_m, cut_r);
+                tile_cuts(B.ld, TILE_N, cut_c);
                 for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
                     for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj) {
                         const int i0 = cut_r[ti], j0 = cut_c[tj], rt = cut_r[ti + 1] - i0, ct = cut_c[tj + 1] - j0;
@@ -536,7 +537,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                         } else {
                             RUnit r;
                             r.C = c_sigma;
-                            r.P = (unsigned long long)(partial_tiles * TILE_M * TILE_N * 8);   // rebased below
+                            r.P = (unsigned long long)(partial_tiles * tile_m * TILE_N * 8);   // rebased below
                             r.c_rp = B.rows_pad;
                             r.i0 = i0;
                             r.j0 = j0;
@@ -550,7 +551,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                                 while (se < ns && prefix[se] < want) ++se;
                                 if (s == n_split - 1) se = ns;
                                 if (se == sb) continue;
-                                u.C = (unsigned long long)((partial_tiles + made) * TILE_M * TILE_N * 8);
+                                u.C = (unsigned long long)((partial_tiles + made) * tile_m * TILE_N * 8);
                                 u.seg_begin = seg0 + sb;
                                 u.seg_end = seg0 + se;
                                 u.mode = UNIT_C_PLAIN | (BASE_WS << UNIT_C_SEL_SHIFT);
@@ -614,7 +615,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
 
     // ---- workspace layout: [T | partial tiles | ring half 0 | ring half 1] --------------------
     h->t_bytes = round_up(max_t_bytes, 128);
-    h->partial_bytes = max_partial_tiles * TILE_M * TILE_N * 8;
+    h->partial_bytes = max_partial_tiles * tile_m * TILE_N * 8;
     bool any_pinned = false;
     for (const Chunk& c : h->chunks) any_pinned |= !c.copies.empty();
     h->has_pinned = any_pinned;
@@ -838,7 +839,7 @@ static int32_t run_plan(dmrgk_heff* h, const double* psi_dev, double* sigma_dev,
         DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, s2, h->counters_dev + 2 * c + 1, h->ctx->n_sm));
         if (serial && ch.p2_units) DMRGK_TRY(prof_end(h, slot, s2));
         if (serial && ch.r_units) DMRGK_TRY(prof_begin(h, 2, s2, &slot));
-        DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, s2));
+        DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, s2, gemm_tile_m(h->opts.kernel)));
         if (serial && ch.r_units) DMRGK_TRY(prof_end(h, slot, s2));
         if (expect) {
             // out[k] = ⟨σ_k, ψ⟩ for the pairs of this chunk, 64 at a time (fused, fixed-order dots)

@@ -55,9 +55,11 @@ def test_sigma_vs_dense_kronecker(make, kernel):
 
 
 @pytest.mark.parametrize("make", [medium_config2, medium_spinless, medium_hubbard])
-@pytest.mark.parametrize("opts", [{}, {"split_waves": 4}, {"t_chunk_bytes": 1 << 20}, {"order_policy": 1}, {"order_policy": 2}])
+@pytest.mark.parametrize("opts", [{}, {"split_waves": 4}, {"t_chunk_bytes": 1 << 20}, {"order_policy": 1}, {"order_policy": 2},
+                                  {"kernel": 4}, {"kernel": 4, "split_waves": 64}])
 def test_sigma_vs_blockwise_medium(make, opts):
-    """T3 at sizes spanning several tiles and ragged tails; split-k and chunking variants."""
+    """T3 at sizes spanning several tiles and ragged tails; split-k and chunking variants, and the
+    tall-tile (128×64) variant of the GEMM kernel."""
     pb = heff.problem_from_workload(make())
     ref = heff.sigma_blockwise(pb)
     dp = device_problem(pb, **opts)
@@ -100,6 +102,11 @@ def test_gemm_order_is_chosen_per_task_on_skewed_shapes():
         execd[policy] = dp.heff.flops_exec
         assert dp.heff.flops_alg == heff.flops_alg(pb)
     assert execd[0] == heff.flops_alg(pb) and execd[1] > execd[0] and execd[2] > execd[0]     # both orders are in use
+    for kern in (2, 3, 4):                                  # the other residencies and the tall tile, same lists
+        dp = device_problem(pb, kernel=kern)
+        sigma = dp.apply(dp.psi_from_host(pb.psi))
+        assert rel_max(dp.to_blocks(sigma), ref) <= TOL_SIGMA, kern
+        assert padding_is_zero(dp, sigma)
     stg = problem.from_workload(wl, pinned=[1, 2, 6, 9], ring_bytes=64 << 20)
     got = stg.apply(stg.psi_fill(wl.seed, wlmod.PSI_STREAM))
     res = problem.from_workload(wl)
@@ -373,3 +380,29 @@ def test_block_coefficients_su2_slot():
     theta, rn, n_apply, ok = dav.solve(None)
     E0 = float(golden_table("closed_forms.txt")["hubbard_dimer_E0_U4"])
     assert ok and abs(theta - E0) <= 1e-9
+
+
+@pytest.mark.parametrize("kernel", [0, 4])
+def test_balanced_tiles_at_edge_dims(kernel):
+    """Sector sizes on both sides of every tile-count boundary (64/65, 128/129, one row, a 16-multiple, a
+    4-multiple that is no 8-multiple …): the balanced tiling (tile origins at multiples of 16, a tile's
+    fragments split evenly over the warp rows/columns, internal.h tile_cuts) must cover each block exactly
+    once, padding rows and columns included."""
+    dims_a = [1, 64, 65, 129, 12, 100, 128, 200, 17]
+    dims_b = [130, 16, 1, 63, 192, 66, 20, 127, 72]
+    secA = [((q,), d) for q, d in enumerate(dims_a)]
+    secB = [((q,), d) for q, d in enumerate(dims_b)]
+    wl = wlmod.Workload("edge_dims", 23, 1, secA, secB, (8,))
+    for k, dlt in enumerate([0, 1, -1, 2, -2, 3, -3, 1]):
+        wl.ops.append(wlmod.OpSpec("A", (dlt,), dlt & 1, False, "one", f"L{k}"))
+        wl.ops.append(wlmod.OpSpec("B", (-dlt,), dlt & 1, False, "one", f"R{k}"))
+        wl.terms.append(wlmod.TermSpec(2 * k, 2 * k + 1, 0.5 - 0.1 * k, False, False, "syn"))
+        wl.terms.append(wlmod.TermSpec(2 * k, 2 * k + 1, 0.25 + 0.1 * k, True, True, "syn^T"))
+    pb = heff.problem_from_workload(wl)
+    ref = heff.sigma_blockwise(pb)
+    for opts in ({}, {"split_waves": 64}, {"order_policy": 2}):
+        dp = device_problem(pb, kernel=kernel, **opts)
+        sigma = dp.apply(dp.psi_from_host(pb.psi))
+        assert rel_max(dp.to_blocks(sigma), ref) <= TOL_SIGMA, opts
+        assert padding_is_zero(dp, sigma)
+        assert rel_max(dp.to_blocks(dp.diag()), heff.diagonal_blockwise(pb)) <= 1e-13
