@@ -346,7 +346,7 @@ def reduced_problem(T, V, n_sites_A, N_target, keep=None, seed=0):
     sa, sb = sector_lists(multA, multB, N_target)
     ia = {q: i for i, (q, _) in enumerate(sa)}
     ib = {q: i for i, (q, _) in enumerate(sb)}
-    ops, tlist, bcoef = [], [], {}
+    ops, tlist, bcoef, ranks = [], [], {}, []
     defects = {"tensor_A": 0.0, "tensor_B": 0.0, "wigner_eckart": 0.0}
     psi_blocks = [(ia[(N, tS)], ib[(N_target - N, -tS)]) for (N, tS), _ in sa if (N_target - N, -tS) in ib]
     for g in groups:
@@ -356,6 +356,7 @@ def reduced_problem(T, V, n_sites_A, N_target, keep=None, seed=0):
             defects["wigner_eckart"] = max(defects["wigner_eckart"], d)
             ops.append({"half": "A", "dq": (0, 0), "parity": 0, "blocks": {(ia[o], ia[i]): m for (o, i), m in red.items()}})
             tlist.append((len(ops) - 1, None, 1.0, False, False))
+            ranks.append(0)
             continue
         if g.ident == "A":      # 1 ⊗ H_B
             defects["tensor_B"] = max(defects["tensor_B"], tensor_defect(g.Ut, 0, n_sites_B))
@@ -364,6 +365,7 @@ def reduced_problem(T, V, n_sites_A, N_target, keep=None, seed=0):
             ops.append({"half": "B", "dq": (0, 0), "parity": 0,
                         "blocks": {(ib[(o[0], -o[1])], ib[(i[0], -i[1])]): m for (o, i), m in red.items()}})
             tlist.append((None, len(ops) - 1, 1.0, False, False))
+            ranks.append(0)
             continue
         U = g.U()
         defects["tensor_A"] = max(defects["tensor_A"], tensor_defect(g.T, g.k2, n_sites_A))
@@ -381,6 +383,7 @@ def reduced_problem(T, V, n_sites_A, N_target, keep=None, seed=0):
             ops.append({"half": "B", "dq": (-g.dN_A, -d2), "parity": g.parity, "blocks": RB})
             k = len(tlist)
             tlist.append((len(ops) - 2, len(ops) - 1, 1.0, False, False))
+            ranks.append(g.k2)
             for (a_idx, b_idx) in psi_blocks:
                 N, tS = sa[a_idx][0]
                 tS2 = tS + d2
@@ -390,4 +393,5 @@ def reduced_problem(T, V, n_sites_A, N_target, keep=None, seed=0):
                 sign = -1.0 if (g.parity and N % 2) else 1.0       # Jordan–Wigner string of the B operator over A
                 bcoef[(k, (a_idx, b_idx))] = sign * recoupling_singlet(tS, tS2, g.k2)
     pb = Problem(2, sa, sb, (N_target, 0), ops, tlist, {}, f"su2_singlet_N{N_target}", bcoef)
+    pb.ranks = ranks            # doubled tensor rank of every pair (an input of the library's host code)
     return pb, multA, multB, groups, defects

@@ -1,0 +1,52 @@
+"""-m gpu parity of the SU(2) spin-adapted H_eff for a singlet target.
+
+The oracle (oracle/su2.py) hands over what a spin-adapted DMRG would: sector lists in multiplets, the reduced
+matrix elements of the tensor-operator pairs, the pair list with each pair's rank.  The recoupling scalars are
+the LIBRARY side's (paper_2311_14106_b200/su2.py, closed form) — the oracle's brute-force table is not passed
+in.  σ is compared with the oracle's blockwise tier and with the definition Cᵀ H C ψ at 1e-11, the Davidson
+energy with the lowest singlet level of the Fock-space Hamiltonian at 1e-9."""
+import numpy as np
+import pytest
+
+from oracle import su2 as osu2, heff, fock
+from _gpu import rel_max, padding_is_zero, TOL_SIGMA, TOL_ENERGY
+from test_oracle_su2 import hubbard, singlet_spectrum_from_S2
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+@pytest.mark.parametrize("R,Cn,nA,rotated,keep", [(2, 2, 2, True, None), (2, 3, 3, False, None), (2, 3, 3, True, None),
+                                                   (2, 3, 2, True, None), (2, 3, 3, True, 0.6)])
+def test_singlet_heff_sigma_and_energy(R, Cn, nA, rotated, keep):
+    from paper_2311_14106_b200 import su2
+    T, V, mc = hubbard(R, Cn, rotated)
+    n = R * Cn
+    pb, multA, multB, groups, defects = osu2.reduced_problem(T, V, nA, n, keep=keep, seed=5)
+    rng = np.random.default_rng(8)
+    pb.psi = {(a, b): rng.normal(size=(pb.sectors_A[a][1], pb.sectors_B[b][1])) for (a, b) in pb.psi_blocks()}
+    pairs = [(L, Rr, c, k2) for (L, Rr, c, _, _), k2 in zip(pb.terms, pb.ranks)]
+    for opts in ({}, {"order_policy": 2}):
+        dp = su2.singlet_problem(pb.sectors_A, pb.sectors_B, n, pb.ops, pairs, **opts)
+        sigma = dp.apply(dp.psi_from_host(pb.psi))
+        got = dp.to_blocks(sigma)
+        assert rel_max(got, heff.sigma_blockwise(pb)) <= TOL_SIGMA            # the method, step by step
+        C = osu2.singlet_isometry(multA, multB, n)
+        H_def = C.T @ (fock.hamiltonian(T, V) @ C)                             # the definition
+        ref = heff.vec_to_psi(pb, H_def @ heff.psi_to_vec(pb))
+        assert rel_max(got, ref) <= TOL_SIGMA
+        assert padding_is_zero(dp, sigma)
+        assert rel_max(dp.to_blocks(dp.diag()), heff.vec_to_psi(pb, np.diag(H_def).copy())) <= 1e-12
+    # spin-adapted dimension: multiplets, fewer than the U(1) states of the same half
+    assert sum(d for _, d in pb.sectors_A) < 4 ** nA
+    dav = dp.davidson(m_max=16, tol=1e-9, max_iter=3000)
+    dav.start(dp.psi_from_host(pb.psi))
+    theta, rn, n_apply, ok = dav.solve(None)
+    assert ok
+    E = np.linalg.eigvalsh(H_def)[0]
+    assert abs(theta - E) <= TOL_ENERGY * max(1.0, abs(E))
+    E_singlet = singlet_spectrum_from_S2(T, V, n, n)[0]
+    if keep is None:
+        assert abs(theta - E_singlet) <= TOL_ENERGY * max(1.0, abs(E_singlet))
+    else:
+        assert theta >= E_singlet - 1e-9                                        # variational
