@@ -223,13 +223,26 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                 for (int q = 0; q < 4; ++q) w[q] = __ldg(p + q);
             }
         };
-        // two claims ahead: cur is being produced, nxt's descriptor is in flight, nx2's index is in flight
-        int cur = claim(), nxt = claim(), nx2 = claim();
-        int4 uw[4], nw[4];
+        // Three levels of look-ahead, each one unit apart, so that no global-memory latency sits between two
+        // units (short units — two or three k-tiles — would otherwise pay it every time): the queue index
+        // of the unit three ahead, the descriptor of the units one and two ahead, the first segment
+        // descriptor of the unit one ahead.
+        auto load_seg = [&](int idx, int seg, int4& lo, int4& hi) {
+            if (idx < n_units) {
+                lo = __ldg(reinterpret_cast<const int4*>(segs + seg));
+                hi = __ldg(reinterpret_cast<const int4*>(segs + seg) + 1);
+            }
+        };
+        int cur = claim(), nxt = claim(), nx2 = claim(), nx3 = claim();
+        int4 uw[4], nw[4], n2w[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) uw[q] = nw[q] = make_int4(0, 0, 0, 0);
+        for (int q = 0; q < 4; ++q) uw[q] = nw[q] = n2w[q] = make_int4(0, 0, 0, 0);
         load_unit(cur, uw);
         load_unit(nxt, nw);
+        load_unit(nx2, n2w);
+        int4 s_lo = make_int4(0, 0, 0, 0), s_hi = make_int4(0, 0, 0, 0), ns_lo = s_lo, ns_hi = s_hi;
+        load_seg(cur, uw[2].z, s_lo, s_hi);
+        load_seg(nxt, nw[2].z, ns_lo, ns_hi);
         int T = 0, stage = 0, ring_pos = 0;
         uint32_t eph = 1;                                 // parity to wait for on empty[stage]: (T/S − 1) & 1
         auto advance_stage = [&]() {
@@ -239,7 +252,6 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                 eph ^= 1u;
             }
         };
-        int4 s_lo = make_int4(0, 0, 0, 0), s_hi = make_int4(0, 0, 0, 0);
         while (cur < n_units) {
             // fields of the unit (Unit layout: C, alpha | c_rp, i0, j0, mrows | ncols, ncols_st, seg_begin, seg_end | mode, nkt, -, tile)
             const int i0 = uw[1].y, j0 = uw[1].z, ncols = uw[2].x;
@@ -247,9 +259,7 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
             const int rows_a = int(uint32_t(uw[3].w) & 0xffffu), cols_b = min(int(uint32_t(uw[3].w) >> 16), ncols - j0);
             const int npa = (rows_a + 15) >> 4, npb = (cols_b + 15) >> 4;
             bool first = true;
-            s_lo = __ldg(reinterpret_cast<const int4*>(segs + seg_begin));
-            s_hi = __ldg(reinterpret_cast<const int4*>(segs + seg_begin) + 1);
-            for (int sg = seg_begin; sg < seg_end; ++sg) {
+            for (int sg = seg_begin; sg < seg_end; ++sg) {       // (s_lo, s_hi) hold segment sg
                 const unsigned long long sA = (unsigned long long)(unsigned)s_lo.x | ((unsigned long long)(unsigned)s_lo.y << 32);
                 const unsigned long long sB = (unsigned long long)(unsigned)s_lo.z | ((unsigned long long)(unsigned)s_lo.w << 32);
                 const int a_rp = s_hi.x, b_rp = s_hi.y, klen = s_hi.z;
@@ -304,13 +314,20 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                     advance_stage();
                 }
             }
-            // next unit: its descriptor was requested one unit ago, its successor's index two units ago
+            // rotate the look-ahead chain
             cur = nxt;
+            s_lo = ns_lo;
+            s_hi = ns_hi;
 #pragma unroll
-            for (int q = 0; q < 4; ++q) uw[q] = nw[q];
+            for (int q = 0; q < 4; ++q) {
+                uw[q] = nw[q];
+                nw[q] = n2w[q];
+            }
             nxt = nx2;
-            load_unit(nxt, nw);
-            nx2 = claim();
+            load_seg(nxt, nw[2].z, ns_lo, ns_hi);
+            nx2 = nx3;
+            load_unit(nx2, n2w);
+            nx3 = claim();
         }
         // stop sentinel on a data-less tile
         if (T >= STAGES) mbar_wait(bar0 + (STAGES + stage) * 8, eph);

@@ -211,10 +211,14 @@ static inline void tile_cuts(int extent, int tile_max, std::vector<int>& cuts) {
     cuts.push_back(extent);
 }
 static inline uint32_t pack_tile(int rows, int cols) { return uint32_t(rows) | (uint32_t(cols) << 16); }
-// cost of a tile per k-tile in fragment products of its fullest warp × 4 (a full 64×64 tile costs 64)
+// cost of a tile per k-tile: the fragment products of its fullest warp × 4 (a full 64×64 tile costs 64), but
+// never less than TILE_COST_FLOOR — a thin tile turns its stages over faster than the copies arrive, so its
+// k-tile costs a latency, not its flops (profiles/r2_ragged.md).  Used for LPT ordering and the split-k plan.
+constexpr int TILE_COST_FLOOR = 24;
 static inline int64_t tile_cost(int rows, int cols) {
     const int fm = (rows + 7) / 8, fn = (cols + 7) / 8;
-    return int64_t(4) * ((fm + 1) / 2) * ((fn + 1) / 2);
+    const int64_t c = int64_t(4) * ((fm + 1) / 2) * ((fn + 1) / 2);
+    return c < TILE_COST_FLOOR ? TILE_COST_FLOOR : c;
 }
 
 // kernel launchers (heff_kernels.cu)
