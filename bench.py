@@ -796,7 +796,7 @@ def main():
     ap.add_argument("--config", default="4", choices=["2", "3", "3b", "4", "5", "5r"])
     ap.add_argument("--m-max", dest="m_max", type=int, default=16)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
-    ap.add_argument("--kernel", type=int, default=0, choices=[0, 2, 3, 4],
+    ap.add_argument("--kernel", type=int, default=0, choices=[0, 2, 3, 4, 5],
                     help="GEMM kernel variant (dmrgk_heff_opts.kernel): 0 = product path; 2, 3, 4 = other (stages, CTAs/SM) "
                          "instantiations kept for measurement")
     ap.add_argument("--no-extras", dest="no_extras", action="store_true",

@@ -186,8 +186,9 @@ struct StageNote {
 // warp stores its own fragment rows and moves on (no CTA-wide barrier anywhere after the prologue).
 // The stop signal is a descriptor with nkt = 0 published through the same ring on a data-less tile.
 constexpr int P_NTHREADS = 160;
+constexpr int EAGER = 1 << 30;           // LOOKAHEAD value: claim units as soon as a look-ahead slot is free
 
-template <int WM, int STAGES, int MIN_CTAS>
+template <int WM, int STAGES, int MIN_CTAS, int LOOKAHEAD>
 __global__ void __launch_bounds__(P_NTHREADS, MIN_CTAS)
 heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __restrict__ segs, int n_units,
                                  int* __restrict__ queue_head, Bases bases) {
@@ -211,38 +212,135 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
 
     if (warp == 4) {
         // ================================ PRODUCER ================================
-        auto claim = [&]() -> int {
+        auto load_unit = [&](int idx, int4 (&w)[4]) {
+            const int4* p = reinterpret_cast<const int4*>(units + idx);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) w[q] = __ldg(p + q);
+        };
+        auto load_seg = [&](int seg, int4& lo, int4& hi) {
+            lo = __ldg(reinterpret_cast<const int4*>(segs + seg));
+            hi = __ldg(reinterpret_cast<const int4*>(segs + seg) + 1);
+        };
+        auto claim_async = [&]() -> int {      // only lane 0 holds the result until it is broadcast
             int v = 0;
             if (lane == 0) v = atomicAdd(queue_head, 1);
-            return __shfl_sync(0xffffffffu, v, 0);
+            return v;
         };
-        auto load_unit = [&](int idx, int4 (&w)[4]) {
-            if (idx < n_units) {
-                const int4* p = reinterpret_cast<const int4*>(units + idx);
+        // Look-ahead: the dependent loads between two units — queue index (atomic), unit descriptor, first
+        // segment descriptor — are requested ahead of time so that no global-memory latency sits between
+        // units, however short.  Two schemes (template parameter LOOKAHEAD):
+        //  * EAGER, the product path, works in whole units: the index of the unit three ahead, the descriptors
+        //    of the units one and two ahead and the first segment of the unit one ahead are in flight, each
+        //    requested one unit before it is used, so nothing in the chain ever blocks.
+        //  * LATE (variant 5) works in k-tiles: a unit is claimed only when fewer than LOOKAHEAD tiles are
+        //    left to issue (current unit + claimed units; up to three claimed units A, B, C; the chain
+        //    advances one step per issued tile).  A unit then starts a few tile times after its claim, so
+        //    queue neighbours — the tiles of one (output block, k-range), which read the same T row tiles and
+        //    R column tiles — run at the same time on different SMs and share those reads in L2: DRAM
+        //    traffic halves (23 → 11.5 GB per launch on config 4), but the chain now has to be advanced
+        //    inside the tile loop and the kernel, which is bound by the DMMA pipe and not by HBM, is 2 %
+        //    slower (profiles/r2_final_summary.md).  Kept for measurement.
+        int4 uw[4];
+        int4 s_lo = make_int4(0, 0, 0, 0), s_hi = s_lo, ns_lo = s_lo, ns_hi = s_lo;
+        int nxt = 0, nx2 = 0, nx3 = 0;                  // EAGER: queue indices of the units one, two, three ahead
+        int4 nw[4], n2w[4];                              //        descriptors of the units one and two ahead
+        int idA = 0, idB = 0, idC = 0;                  // LATE:  claimed units A (runs next), B, C
+        int stA = 0, stB = 0, stC = 0;                  //        0 empty, 1 claimed, 2 descriptor requested, 3 descriptor
+        bool ended = false;                              //        readable, 4 first segment requested (A), 5 end of queue
+        int4 wA[4], wB[4], wC[4];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) w[q] = __ldg(p + q);
+        for (int q = 0; q < 4; ++q) uw[q] = nw[q] = n2w[q] = wA[q] = wB[q] = wC[q] = s_lo;
+        auto step = [&](int& st, int& id, int4 (&w)[4]) {
+            if (st == 1) {
+                id = __shfl_sync(0xffffffffu, id, 0);
+                if (id >= n_units) {
+                    st = 5;
+                    ended = true;
+                } else {
+                    load_unit(id, w);
+                    st = 2;
+                }
+            } else if (st == 2) {
+                st = 3;
             }
         };
-        // Three levels of look-ahead, each one unit apart, so that no global-memory latency sits between two
-        // units (short units — two or three k-tiles — would otherwise pay it every time): the queue index
-        // of the unit three ahead, the descriptor of the units one and two ahead, the first segment
-        // descriptor of the unit one ahead.
-        auto load_seg = [&](int idx, int seg, int4& lo, int4& hi) {
-            if (idx < n_units) {
-                lo = __ldg(reinterpret_cast<const int4*>(segs + seg));
-                hi = __ldg(reinterpret_cast<const int4*>(segs + seg) + 1);
+        auto feed = [&](int tiles_left) {              // LATE only: once per issued tile
+            if (stA == 3) {
+                load_seg(wA[2].z, ns_lo, ns_hi);
+                stA = 4;
+            }
+            step(stA, idA, wA);
+            step(stB, idB, wB);
+            step(stC, idC, wC);
+            if (ended || stC != 0) return;
+            int ahead = tiles_left;                     // an entry whose length is not known yet holds further claims back
+            if (stA != 0) ahead += stA >= 3 ? wA[3].y : LOOKAHEAD;
+            if (stB != 0) ahead += stB >= 3 ? wB[3].y : LOOKAHEAD;
+            if (ahead < LOOKAHEAD) {
+                const int v = claim_async();
+                if (stA == 0) {
+                    idA = v;
+                    stA = 1;
+                } else if (stB == 0) {
+                    idB = v;
+                    stB = 1;
+                } else {
+                    idC = v;
+                    stC = 1;
+                }
             }
         };
-        int cur = claim(), nxt = claim(), nx2 = claim(), nx3 = claim();
-        int4 uw[4], nw[4], n2w[4];
+        // make the next unit current (uw, s_lo, s_hi); false at the end of the queue
+        auto rotate = [&]() -> bool {
+            if constexpr (LOOKAHEAD == EAGER) {
+                const int cur = nxt;
+                if (cur >= n_units) return false;
+                s_lo = ns_lo;
+                s_hi = ns_hi;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) uw[q] = nw[q] = n2w[q] = make_int4(0, 0, 0, 0);
-        load_unit(cur, uw);
-        load_unit(nxt, nw);
-        load_unit(nx2, n2w);
-        int4 s_lo = make_int4(0, 0, 0, 0), s_hi = make_int4(0, 0, 0, 0), ns_lo = s_lo, ns_hi = s_hi;
-        load_seg(cur, uw[2].z, s_lo, s_hi);
-        load_seg(nxt, nw[2].z, ns_lo, ns_hi);
+                for (int q = 0; q < 4; ++q) {
+                    uw[q] = nw[q];
+                    nw[q] = n2w[q];
+                }
+                nxt = nx2;
+                if (nxt < n_units) load_seg(nw[2].z, ns_lo, ns_hi);
+                nx2 = nx3;
+                if (nx2 < n_units) load_unit(nx2, n2w);
+                nx3 = __shfl_sync(0xffffffffu, claim_async(), 0);
+                return true;
+            } else {
+                if (stA == 0) {
+                    if (ended) return false;
+                    idA = claim_async();
+                    stA = 1;
+                }
+                if (stA == 1) step(stA, idA, wA);
+                if (stA == 5) return false;
+                if (stA <= 3) load_seg(wA[2].z, ns_lo, ns_hi);
+                s_lo = ns_lo;
+                s_hi = ns_hi;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    uw[q] = wA[q];
+                    wA[q] = wB[q];
+                    wB[q] = wC[q];
+                }
+                stA = stB;
+                idA = idB;
+                stB = stC;
+                idB = idC;
+                stC = 0;
+                return true;
+            }
+        };
+        if constexpr (LOOKAHEAD == EAGER) {             // prime the chain: units 0, 1, 2 of this CTA and the index of the fourth
+            nxt = __shfl_sync(0xffffffffu, claim_async(), 0);
+            nx2 = __shfl_sync(0xffffffffu, claim_async(), 0);
+            nx3 = __shfl_sync(0xffffffffu, claim_async(), 0);
+            if (nxt < n_units) load_unit(nxt, nw);
+            if (nx2 < n_units) load_unit(nx2, n2w);
+            if (nxt < n_units) load_seg(nw[2].z, ns_lo, ns_hi);
+        }
         int T = 0, stage = 0, ring_pos = 0;
         uint32_t eph = 1;                                 // parity to wait for on empty[stage]: (T/S − 1) & 1
         auto advance_stage = [&]() {
@@ -252,12 +350,14 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                 eph ^= 1u;
             }
         };
-        while (cur < n_units) {
+        bool more = rotate();
+        while (more) {
             // fields of the unit (Unit layout: C, alpha | c_rp, i0, j0, mrows | ncols, ncols_st, seg_begin, seg_end | mode, nkt, -, tile)
             const int i0 = uw[1].y, j0 = uw[1].z, ncols = uw[2].x;
             const int seg_begin = uw[2].z, seg_end = uw[2].w;
             const int rows_a = int(uint32_t(uw[3].w) & 0xffffu), cols_b = min(int(uint32_t(uw[3].w) >> 16), ncols - j0);
             const int npa = (rows_a + 15) >> 4, npb = (cols_b + 15) >> 4;
+            int tiles_left = uw[3].y;                            // nkt of the unit
             bool first = true;
             for (int sg = seg_begin; sg < seg_end; ++sg) {       // (s_lo, s_hi) hold segment sg
                 const unsigned long long sA = (unsigned long long)(unsigned)s_lo.x | ((unsigned long long)(unsigned)s_lo.y << 32);
@@ -312,22 +412,10 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                         if (++ring_pos == RING) ring_pos = 0;
                     }
                     advance_stage();
+                    if constexpr (LOOKAHEAD != EAGER) feed(--tiles_left);
                 }
             }
-            // rotate the look-ahead chain
-            cur = nxt;
-            s_lo = ns_lo;
-            s_hi = ns_hi;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                uw[q] = nw[q];
-                nw[q] = n2w[q];
-            }
-            nxt = nx2;
-            load_seg(nxt, nw[2].z, ns_lo, ns_hi);
-            nx2 = nx3;
-            load_unit(nx2, n2w);
-            nx3 = claim();
+            more = rotate();
         }
         // stop sentinel on a data-less tile
         if (T >= STAGES) mbar_wait(bar0 + (STAGES + stage) * 8, eph);
@@ -523,7 +611,8 @@ int gemm_ctas_per_sm() { return g_gemm_ctas_per_sm; }
 // 1 = scalar check kernel; 2 = 64×64, 2 CTAs per SM with 96 KB of stages; 3 = 64×64, 2 CTAs per SM with
 // 64 KB; 4 = the tall 128×64 tile (2×2 warps of 64×32: 128 accumulator registers), 2 CTAs per SM with 96 KB
 // of stages — a CTA of 5 warps at 2 CTAs per SM is capped at 168 registers, so this variant spills and is
-// slower than variant 0 on every shape measured (profiles/r2_ragged.md); kept, like 2 and 3, for measurement.
+// slower than variant 0 on every shape measured (profiles/r2_ragged.md); kept, like 2 and 3, for measurement;
+// 5 = variant 0 with LATE unit claims (see the producer's look-ahead comment).
 constexpr int ST64 = 65536 / (stage_doubles(4) * 8), ST96 = 98304 / (stage_doubles(4) * 8), ST96T = 98304 / (stage_doubles(8) * 8);
 template <class K>
 static int32_t setup_kernel(K* fn, int threads, int smem, int min_ctas, int* resident) {
@@ -540,15 +629,16 @@ static int32_t setup_kernel(K* fn, int threads, int smem, int min_ctas, int* res
 }
 
 int32_t gemm_kernel_setup() {
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3>, P_NTHREADS, smem_bytes(4, ST64), 3, &g_gemm_ctas_per_sm));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST96, 2>, P_NTHREADS, smem_bytes(4, ST96), 2, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 2>, P_NTHREADS, smem_bytes(4, ST64), 2, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<8, ST96T, 2>, P_NTHREADS, smem_bytes(8, ST96T), 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3, EAGER>, P_NTHREADS, smem_bytes(4, ST64), 3, &g_gemm_ctas_per_sm));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST96, 2, EAGER>, P_NTHREADS, smem_bytes(4, ST96), 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 2, EAGER>, P_NTHREADS, smem_bytes(4, ST64), 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<8, ST96T, 2, EAGER>, P_NTHREADS, smem_bytes(8, ST96T), 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3, 8>, P_NTHREADS, smem_bytes(4, ST64), 3, nullptr));
     return DMRGK_OK;
 }
 
 int gemm_tile_m(int kernel) { return kernel == 4 ? 128 : 64; }
-int gemm_ctas(int kernel) { return (kernel == 0 || kernel == 1) ? 3 : 2; }
+int gemm_ctas(int kernel) { return (kernel == 0 || kernel == 1 || kernel == 5) ? 3 : 2; }
 
 int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
                           const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm) {
@@ -559,10 +649,11 @@ int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev
     if (kernel != 1 && !counter_dev) return fail(DMRGK_EINVAL, "launch_gemm_units: the persistent kernel needs a queue counter");
     switch (kernel) {
         case 1: heff_gemm_scalar_kernel<<<unsigned(n_units), NTHREADS, 0, st>>>(units_dev, segs_dev, bases); break;
-        case 2: heff_gemm_dmma_persistent_kernel<4, ST96, 2><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST96), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        case 3: heff_gemm_dmma_persistent_kernel<4, ST64, 2><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        case 4: heff_gemm_dmma_persistent_kernel<8, ST96T, 2><<<pgrid(2), P_NTHREADS, smem_bytes(8, ST96T), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        default: heff_gemm_dmma_persistent_kernel<4, ST64, 3><<<pgrid(3), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 2: heff_gemm_dmma_persistent_kernel<4, ST96, 2, EAGER><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST96), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 3: heff_gemm_dmma_persistent_kernel<4, ST64, 2, EAGER><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 4: heff_gemm_dmma_persistent_kernel<8, ST96T, 2, EAGER><<<pgrid(2), P_NTHREADS, smem_bytes(8, ST96T), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 5: heff_gemm_dmma_persistent_kernel<4, ST64, 3, 8><<<pgrid(3), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        default: heff_gemm_dmma_persistent_kernel<4, ST64, 3, EAGER><<<pgrid(3), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
     }
     count_launch();
     DMRGK_CUDA(cudaGetLastError());

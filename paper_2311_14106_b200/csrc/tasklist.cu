@@ -127,7 +127,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
     if (o.split_waves <= 0) o.split_waves = 32;   // units per CTA slot: the queue's tail is ≈ one unit long
-    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 4) || o.order_policy < 0 || o.order_policy > 2 ||
+    if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 5) || o.order_policy < 0 || o.order_policy > 2 ||
         (o.per_pair_output != 0 && o.per_pair_output != 1))
         return fail(DMRGK_EINVAL, "heff_create: bad options");
     const int64_t ring_part = (o.ring_bytes / 3) / 128 * 128;   // three parts: see dmrgk_heff_apply
@@ -480,7 +480,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
             // of equal cost those of one (output block, k-range) together, row tile by row tile — they run
             // at the same time and share their T row tiles and R column tiles in L2.
             struct U2 {
-                int64_t cost;
+                int64_t cost;            // queue key: the cost of the LARGEST tile of the unit's (group, split)
                 Unit u;
                 int32_t grp, split;
             };
@@ -501,13 +501,17 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                 const Block& B = pb[ob];
                 tile_cuts(B.rows, tile_m, cut_r);
                 tile_cuts(B.ld, TILE_N, cut_c);
+                // One split plan per GROUP, taken from its largest tile (the first one): every tile of the block
+                // is cut at the same segment boundaries, and all units of a (group, split) carry the same queue
+                // key, so they are claimed together and stream the same T row tiles and R column tiles through
+                // L2 at the same time (profiles/r2_final_summary.md: DRAM traffic).
+                const int rt0 = cut_r[1] - cut_r[0], cc0 = std::min(cut_c[1] - cut_c[0], B.cols);
+                const int64_t c = cost_of(rt0, cc0, nkt);
+                int n_split = int(std::min<int64_t>(ns, (c + target - 1) / target));
+                if (n_split < 1) n_split = 1;
                 for (size_t ti = 0; ti + 1 < cut_r.size(); ++ti)
                     for (size_t tj = 0; tj + 1 < cut_c.size(); ++tj) {
                         const int i0 = cut_r[ti], j0 = cut_c[tj], rt = cut_r[ti + 1] - i0, ct = cut_c[tj + 1] - j0;
-                        const int cc = std::min(ct, B.cols - j0);      // columns that are computed (ct: stored)
-                        const int64_t c = cost_of(rt, cc, nkt);
-                        int n_split = int(std::min<int64_t>(ns, (c + target - 1) / target));
-                        if (n_split < 1) n_split = 1;
                         Unit u;
                         memset(&u, 0, sizeof(u));
                         u.alpha = 1.0;
@@ -556,7 +560,7 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
                                 u.seg_end = seg0 + se;
                                 u.mode = UNIT_C_PLAIN | (BASE_WS << UNIT_C_SEL_SHIFT);
                                 u.nkt = int32_t(prefix[se] - prefix[sb]);
-                                tmp.push_back({cost_of(rt, cc, u.nkt), u, gi, made});
+                                tmp.push_back({cost_of(rt0, cc0, u.nkt), u, gi, made});
                                 ++made;
                                 sb = se;
                             }
