@@ -149,7 +149,7 @@ typedef struct dmrgk_heff_opts {
                                1 = scalar check kernel (same task lists; debugging aid),
                                2, 3 = the DMMA kernel at other residencies (measurement aid),
                                4 = the DMMA kernel with a tall 128×64 CTA tile,
-                               5 = variant 0 claiming work units late (L2 sharing experiment)  */
+                               5 = variant 0 claiming work units eagerly (L2 sharing experiment) */
     int32_t split_waves;    /* phase-2 split-k target: units per CTA slot (0 = default 32)  */
     int32_t order_policy;   /* GEMM order per task: 0 = the cheaper of (Lψ)Rᵀ and
                                L(ψRᵀ) by flop count, 1 = always (Lψ)Rᵀ, 2 = always L(ψRᵀ); tasks

@@ -186,7 +186,8 @@ struct StageNote {
 // warp stores its own fragment rows and moves on (no CTA-wide barrier anywhere after the prologue).
 // The stop signal is a descriptor with nkt = 0 published through the same ring on a data-less tile.
 constexpr int P_NTHREADS = 160;
-constexpr int EAGER = 1 << 30;           // LOOKAHEAD value: claim units as soon as a look-ahead slot is free
+constexpr int EAGER = 1 << 30;           // LOOKAHEAD value: claim whole units ahead (variant 5)
+constexpr int LATE = 8;                  // LOOKAHEAD of the product path, in k-tiles
 
 template <int WM, int STAGES, int MIN_CTAS, int LOOKAHEAD>
 __global__ void __launch_bounds__(P_NTHREADS, MIN_CTAS)
@@ -228,66 +229,55 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
         };
         // Look-ahead: the dependent loads between two units — queue index (atomic), unit descriptor, first
         // segment descriptor — are requested ahead of time so that no global-memory latency sits between
-        // units, however short.  Two schemes (template parameter LOOKAHEAD):
-        //  * EAGER, the product path, works in whole units: the index of the unit three ahead, the descriptors
-        //    of the units one and two ahead and the first segment of the unit one ahead are in flight, each
-        //    requested one unit before it is used, so nothing in the chain ever blocks.
-        //  * LATE (variant 5) works in k-tiles: a unit is claimed only when fewer than LOOKAHEAD tiles are
-        //    left to issue (current unit + claimed units; up to three claimed units A, B, C; the chain
-        //    advances one step per issued tile).  A unit then starts a few tile times after its claim, so
-        //    queue neighbours — the tiles of one (output block, k-range), which read the same T row tiles and
-        //    R column tiles — run at the same time on different SMs and share those reads in L2: DRAM
-        //    traffic halves (23 → 11.5 GB per launch on config 4), but the chain now has to be advanced
-        //    inside the tile loop and the kernel, which is bound by the DMMA pipe and not by HBM, is 2 %
-        //    slower (profiles/r2_final_summary.md).  Kept for measurement.
+        // units.  Two schemes (template parameter LOOKAHEAD):
+        //  * LATE, the product path, works in k-tiles: the next unit is claimed only when fewer than
+        //    LOOKAHEAD tiles of the current one are left to issue, its descriptor follows two and its first
+        //    segment four tiles later (a unit shorter than that pays the latencies).  A unit then starts a
+        //    few tile times after its claim, so queue neighbours — the tiles of one (output block, k-range),
+        //    which read the same T row tiles and R column tiles — run at the same time on different SMs and
+        //    share those reads in L2.
+        //  * EAGER (variant 5, kept for measurement) works in whole units: the index of the unit three
+        //    ahead, the descriptors of the units one and two ahead and the first segment of the unit one
+        //    ahead are in flight, each requested one unit before it is used.  Nothing ever blocks, but a
+        //    CTA runs queue neighbours one after the other instead of next to other CTAs: same speed on
+        //    config 4 (bound by the DMMA pipe), 1.6× the DRAM traffic (23 against 14 GB per launch,
+        //    profiles/r2_final_summary.md).
         int4 uw[4];
         int4 s_lo = make_int4(0, 0, 0, 0), s_hi = s_lo, ns_lo = s_lo, ns_hi = s_lo;
         int nxt = 0, nx2 = 0, nx3 = 0;                  // EAGER: queue indices of the units one, two, three ahead
         int4 nw[4], n2w[4];                              //        descriptors of the units one and two ahead
-        int idA = 0, idB = 0, idC = 0;                  // LATE:  claimed units A (runs next), B, C
-        int stA = 0, stB = 0, stC = 0;                  //        0 empty, 1 claimed, 2 descriptor requested, 3 descriptor
-        bool ended = false;                              //        readable, 4 first segment requested (A), 5 end of queue
-        int4 wA[4], wB[4], wC[4];
+        int idA = 0, stA = 0;                           // LATE:  the claimed next unit; 0 none, 1 claimed, 2 descriptor
+        bool ended = false;                              //        requested, 4 first segment requested, 5 end of queue
+        int4 wA[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) uw[q] = nw[q] = n2w[q] = wA[q] = wB[q] = wC[q] = s_lo;
-        auto step = [&](int& st, int& id, int4 (&w)[4]) {
-            if (st == 1) {
-                id = __shfl_sync(0xffffffffu, id, 0);
-                if (id >= n_units) {
-                    st = 5;
-                    ended = true;
-                } else {
-                    load_unit(id, w);
-                    st = 2;
-                }
-            } else if (st == 2) {
-                st = 3;
+        for (int q = 0; q < 4; ++q) uw[q] = nw[q] = n2w[q] = wA[q] = s_lo;
+        // LATE only, once per issued tile: one chain step when its trigger point is reached — claim with
+        // LOOKAHEAD tiles left, descriptor two tiles later, first segment two tiles after that
+        auto chain_claim = [&]() {
+            idA = claim_async();
+            stA = 1;
+        };
+        auto chain_desc = [&]() {
+            idA = __shfl_sync(0xffffffffu, idA, 0);
+            if (idA >= n_units) {
+                stA = 5;
+                ended = true;
+            } else {
+                load_unit(idA, wA);
+                stA = 2;
             }
         };
-        auto feed = [&](int tiles_left) {              // LATE only: once per issued tile
-            if (stA == 3) {
-                load_seg(wA[2].z, ns_lo, ns_hi);
-                stA = 4;
-            }
-            step(stA, idA, wA);
-            step(stB, idB, wB);
-            step(stC, idC, wC);
-            if (ended || stC != 0) return;
-            int ahead = tiles_left;                     // an entry whose length is not known yet holds further claims back
-            if (stA != 0) ahead += stA >= 3 ? wA[3].y : LOOKAHEAD;
-            if (stB != 0) ahead += stB >= 3 ? wB[3].y : LOOKAHEAD;
-            if (ahead < LOOKAHEAD) {
-                const int v = claim_async();
-                if (stA == 0) {
-                    idA = v;
-                    stA = 1;
-                } else if (stB == 0) {
-                    idB = v;
-                    stB = 1;
-                } else {
-                    idC = v;
-                    stC = 1;
-                }
+        auto chain_seg = [&]() {
+            load_seg(wA[2].z, ns_lo, ns_hi);
+            stA = 4;
+        };
+        auto feed = [&](int tiles_left) {
+            if (stA == 0) {
+                if (!ended && tiles_left < LOOKAHEAD) chain_claim();
+            } else if (stA == 1) {
+                if (tiles_left < LOOKAHEAD - 2) chain_desc();
+            } else if (stA == 2) {
+                if (tiles_left < LOOKAHEAD - 4) chain_seg();
             }
         };
         // make the next unit current (uw, s_lo, s_hi); false at the end of the queue
@@ -309,27 +299,18 @@ heff_gemm_dmma_persistent_kernel(const Unit* __restrict__ units, const Seg* __re
                 nx3 = __shfl_sync(0xffffffffu, claim_async(), 0);
                 return true;
             } else {
-                if (stA == 0) {
+                if (stA == 0) {                        // finish whatever is missing, synchronously
                     if (ended) return false;
-                    idA = claim_async();
-                    stA = 1;
+                    chain_claim();
                 }
-                if (stA == 1) step(stA, idA, wA);
+                if (stA == 1) chain_desc();
                 if (stA == 5) return false;
-                if (stA <= 3) load_seg(wA[2].z, ns_lo, ns_hi);
+                if (stA == 2) chain_seg();
                 s_lo = ns_lo;
                 s_hi = ns_hi;
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    uw[q] = wA[q];
-                    wA[q] = wB[q];
-                    wB[q] = wC[q];
-                }
-                stA = stB;
-                idA = idB;
-                stB = stC;
-                idB = idC;
-                stC = 0;
+                for (int q = 0; q < 4; ++q) uw[q] = wA[q];
+                stA = 0;
                 return true;
             }
         };
@@ -612,7 +593,7 @@ int gemm_ctas_per_sm() { return g_gemm_ctas_per_sm; }
 // 64 KB; 4 = the tall 128×64 tile (2×2 warps of 64×32: 128 accumulator registers), 2 CTAs per SM with 96 KB
 // of stages — a CTA of 5 warps at 2 CTAs per SM is capped at 168 registers, so this variant spills and is
 // slower than variant 0 on every shape measured (profiles/r2_ragged.md); kept, like 2 and 3, for measurement;
-// 5 = variant 0 with LATE unit claims (see the producer's look-ahead comment).
+// 5 = variant 0 with EAGER unit claims (see the producer's look-ahead comment).
 constexpr int ST64 = 65536 / (stage_doubles(4) * 8), ST96 = 98304 / (stage_doubles(4) * 8), ST96T = 98304 / (stage_doubles(8) * 8);
 template <class K>
 static int32_t setup_kernel(K* fn, int threads, int smem, int min_ctas, int* resident) {
@@ -629,11 +610,11 @@ static int32_t setup_kernel(K* fn, int threads, int smem, int min_ctas, int* res
 }
 
 int32_t gemm_kernel_setup() {
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3, EAGER>, P_NTHREADS, smem_bytes(4, ST64), 3, &g_gemm_ctas_per_sm));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST96, 2, EAGER>, P_NTHREADS, smem_bytes(4, ST96), 2, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 2, EAGER>, P_NTHREADS, smem_bytes(4, ST64), 2, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<8, ST96T, 2, EAGER>, P_NTHREADS, smem_bytes(8, ST96T), 2, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3, 8>, P_NTHREADS, smem_bytes(4, ST64), 3, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3, LATE>, P_NTHREADS, smem_bytes(4, ST64), 3, &g_gemm_ctas_per_sm));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST96, 2, LATE>, P_NTHREADS, smem_bytes(4, ST96), 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 2, LATE>, P_NTHREADS, smem_bytes(4, ST64), 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<8, ST96T, 2, LATE>, P_NTHREADS, smem_bytes(8, ST96T), 2, nullptr));
+    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3, EAGER>, P_NTHREADS, smem_bytes(4, ST64), 3, nullptr));
     return DMRGK_OK;
 }
 
@@ -641,19 +622,20 @@ int gemm_tile_m(int kernel) { return kernel == 4 ? 128 : 64; }
 int gemm_ctas(int kernel) { return (kernel == 0 || kernel == 1 || kernel == 5) ? 3 : 2; }
 
 int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
-                          const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm) {
+                          const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm, bool short_units) {
     if (n_units <= 0) return DMRGK_OK;
+    if (kernel == 0 && short_units) kernel = 5;      // units too short for the late look-ahead chain: claim eagerly
     if (n_units > 0x7fffffffLL) return fail(DMRGK_EINVAL, "too many work units in one launch: %lld", (long long)n_units);
     const int nu = int(n_units);
     auto pgrid = [&](int ctas) { return unsigned(std::min<int64_t>(n_units, int64_t(n_sm) * ctas)); };
     if (kernel != 1 && !counter_dev) return fail(DMRGK_EINVAL, "launch_gemm_units: the persistent kernel needs a queue counter");
     switch (kernel) {
         case 1: heff_gemm_scalar_kernel<<<unsigned(n_units), NTHREADS, 0, st>>>(units_dev, segs_dev, bases); break;
-        case 2: heff_gemm_dmma_persistent_kernel<4, ST96, 2, EAGER><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST96), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        case 3: heff_gemm_dmma_persistent_kernel<4, ST64, 2, EAGER><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        case 4: heff_gemm_dmma_persistent_kernel<8, ST96T, 2, EAGER><<<pgrid(2), P_NTHREADS, smem_bytes(8, ST96T), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        case 5: heff_gemm_dmma_persistent_kernel<4, ST64, 3, 8><<<pgrid(3), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
-        default: heff_gemm_dmma_persistent_kernel<4, ST64, 3, EAGER><<<pgrid(3), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 2: heff_gemm_dmma_persistent_kernel<4, ST96, 2, LATE><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST96), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 3: heff_gemm_dmma_persistent_kernel<4, ST64, 2, LATE><<<pgrid(2), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 4: heff_gemm_dmma_persistent_kernel<8, ST96T, 2, LATE><<<pgrid(2), P_NTHREADS, smem_bytes(8, ST96T), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        case 5: heff_gemm_dmma_persistent_kernel<4, ST64, 3, EAGER><<<pgrid(3), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
+        default: heff_gemm_dmma_persistent_kernel<4, ST64, 3, LATE><<<pgrid(3), P_NTHREADS, smem_bytes(4, ST64), st>>>(units_dev, segs_dev, nu, counter_dev, bases); break;
     }
     count_launch();
     DMRGK_CUDA(cudaGetLastError());

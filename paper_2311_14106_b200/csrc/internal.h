@@ -223,8 +223,10 @@ static inline int64_t tile_cost(int rows, int cols) {
 
 // kernel launchers (heff_kernels.cu)
 // `counter_dev`: a zeroed int the persistent kernel uses as its unit queue head (one per launch in flight)
+// `short_units`: the launch's units average fewer k-tiles than the late look-ahead needs (variant 0 then claims eagerly)
 int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
-                          const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm);
+                          const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm, bool short_units);
+constexpr int SHORT_UNIT_TILES = 8;   // = the late look-ahead of the GEMM kernel, in k-tiles
 int32_t launch_reduce(const RUnit* runits_dev, int64_t n, const Bases& bases, cudaStream_t st, int tile_m);
 int gemm_tile_m(int kernel);   // rows of the CTA tile of a kernel variant (64, or 128 for the tall tile)
 int gemm_ctas(int kernel);     // CTAs per SM the variant is launched with
@@ -242,6 +244,7 @@ struct StageCopy {
 struct Chunk {
     int64_t p1_unit0 = 0, p1_units = 0, p1_seg0 = 0;
     int64_t p2_unit0 = 0, p2_units = 0, p2_seg0 = 0;
+    bool p1_short = false, p2_short = false;   // mean unit length below SHORT_UNIT_TILES k-tiles
     int64_t r_unit0 = 0, r_units = 0;
     int64_t p1_segs = 0, p2_segs = 0;
     int64_t d_block0 = 0, d_blocks = 0;
@@ -259,6 +262,7 @@ struct dmrgk_renorm {
     double flops = 0;
     struct RChunk {
         int64_t p1_unit0 = 0, p1_units = 0, p2_unit0 = 0, p2_units = 0;
+        bool p1_short = false, p2_short = false;
     };
     std::vector<RChunk> chunks;
     dmrgk::Unit* units_dev = nullptr;

@@ -212,6 +212,13 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
         ch.p1_unit0 = int64_t(units.size());
         for (const CU& x : p1) units.push_back(x.u);
         ch.p1_units = int64_t(p1.size());
+        {
+            int64_t k1 = 0, k2 = 0;
+            for (const CU& x : p1) k1 += x.u.nkt;
+            for (const CU& x : p2) k2 += x.u.nkt;
+            ch.p1_short = k1 < SHORT_UNIT_TILES * int64_t(p1.size());
+            ch.p2_short = k2 < SHORT_UNIT_TILES * int64_t(p2.size());
+        }
         ch.p2_unit0 = int64_t(units.size());
         for (const CU& x : p2) units.push_back(x.u);
         ch.p2_units = int64_t(p2.size());
@@ -292,10 +299,10 @@ int32_t dmrgk_renorm_apply(dmrgk_renorm* r, void* workspace_dev, void* stream) {
         for (size_t c = 0; c < r->chunks.size(); ++c) {
             const auto& ch = r->chunks[c];
             if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(r->s1, r->ev_p2[c & 1], 0));     // T buffer re-use
-            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p1_unit0, r->segs_dev, ch.p1_units, bases, r->s1, r->counters_dev + 2 * c, r->ctx->n_sm));
+            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p1_unit0, r->segs_dev, ch.p1_units, bases, r->s1, r->counters_dev + 2 * c, r->ctx->n_sm, ch.p1_short));
             DMRGK_CUDA(cudaEventRecord(r->ev_p1[c & 1], r->s1));
             DMRGK_CUDA(cudaStreamWaitEvent(r->s2, r->ev_p1[c & 1], 0));
-            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p2_unit0, r->segs_dev, ch.p2_units, bases, r->s2, r->counters_dev + 2 * c + 1, r->ctx->n_sm));
+            DMRGK_TRY(launch_gemm_units(r->kernel, r->units_dev + ch.p2_unit0, r->segs_dev, ch.p2_units, bases, r->s2, r->counters_dev + 2 * c + 1, r->ctx->n_sm, ch.p2_short));
             DMRGK_CUDA(cudaEventRecord(r->ev_p2[c & 1], r->s2));
         }
         return DMRGK_OK;

@@ -436,6 +436,11 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
             std::stable_sort(tmp.begin(), tmp.end(), [](const U1& a, const U1& b) { return a.cost > b.cost; });
             for (const U1& x : tmp) units.push_back(x.u);
             ch.p1_units = int64_t(tmp.size());
+            {
+                int64_t kt = 0;
+                for (const U1& x : tmp) kt += x.u.nkt;
+                ch.p1_short = kt < SHORT_UNIT_TILES * ch.p1_units;
+            }
             ch.p1_segs = int64_t(tasks.size());
         }
 
@@ -577,6 +582,11 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
             });
             for (const U2& x : tmp) units.push_back(x.u);
             ch.p2_units = int64_t(tmp.size());
+            {
+                int64_t kt = 0;
+                for (const U2& x : tmp) kt += x.u.nkt;
+                ch.p2_short = kt < SHORT_UNIT_TILES * ch.p2_units;
+            }
             ch.p2_segs = int64_t(segs.size()) - ch.p2_seg0;
             ch.r_units = int64_t(runits.size()) - ch.r_unit0;
             max_partial_tiles = std::max(max_partial_tiles, partial_tiles);
@@ -832,7 +842,7 @@ static int32_t run_plan(dmrgk_heff* h, const double* psi_dev, double* sigma_dev,
         if (ch.p1_units) {
             if (c >= 2) DMRGK_CUDA(cudaStreamWaitEvent(s1, h->ev_p2[c & 1], 0));
             if (serial) DMRGK_TRY(prof_begin(h, 0, s1, &slot));
-            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, s1, h->counters_dev + 2 * c, h->ctx->n_sm));
+            DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p1_unit0, h->segs_dev, ch.p1_units, bases, s1, h->counters_dev + 2 * c, h->ctx->n_sm, ch.p1_short));
             if (serial) DMRGK_TRY(prof_end(h, slot, s1));
             DMRGK_CUDA(cudaEventRecord(h->ev_p1[c & 1], s1));
             DMRGK_CUDA(cudaStreamWaitEvent(s2, h->ev_p1[c & 1], 0));
@@ -840,7 +850,7 @@ static int32_t run_plan(dmrgk_heff* h, const double* psi_dev, double* sigma_dev,
         if (expect && ch.k_count)       // blocks of σ_k that no task writes must read as zero
             DMRGK_CUDA(cudaMemsetAsync((char*)workspace_dev + h->pp_base, 0, size_t(ch.k_count) * h->pp_vec_bytes, s2));
         if (serial && ch.p2_units) DMRGK_TRY(prof_begin(h, 1, s2, &slot));
-        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, s2, h->counters_dev + 2 * c + 1, h->ctx->n_sm));
+        DMRGK_TRY(launch_gemm_units(h->opts.kernel, h->units_dev + ch.p2_unit0, h->segs_dev, ch.p2_units, bases, s2, h->counters_dev + 2 * c + 1, h->ctx->n_sm, ch.p2_short));
         if (serial && ch.p2_units) DMRGK_TRY(prof_end(h, slot, s2));
         if (serial && ch.r_units) DMRGK_TRY(prof_begin(h, 2, s2, &slot));
         DMRGK_TRY(launch_reduce(h->runits_dev + ch.r_unit0, ch.r_units, bases, s2, gemm_tile_m(h->opts.kernel)));
