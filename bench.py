@@ -787,6 +787,92 @@ def run_ragged(args):
     print(json.dumps({"op": "ragged", "source_hash": dmrgk.source_hash(), "kernel_variant": args.kernel, "rows": rows}), flush=True)
 
 
+def run_su2(args):
+    """--op su2: one step = one apply of the SU(2) spin-adapted singlet H_eff
+    on the synthetic spin-adapted workload `workloads.su2_singlet_workload()`: 18 orbitals per half, 190 sectors
+    (N, 2S) holding M = 12288 multiplets (D = 4096 kept multiplets × 3 site multiplets), K = 2702 pairs of reduced
+    operators, recoupling scalars from paper_2311_14106_b200/su2.py.  Its own metric, not the headline."""
+    import torch
+    import workloads as wlmod
+    from paper_2311_14106_b200 import dmrgk, problem, su2
+    torch.cuda.set_device(0)
+    dmrgk.load()
+    wl = wlmod.su2_singlet_workload()
+    terms = [(t.L, t.R, t.coef, t.trans_L, t.trans_R) for t in wl.terms]
+    psi_a = [a for (a, _, _, _, _) in wlmod.psi_block_table(wl.sectors_A, wl.sectors_B, wl.target)]
+    table = su2.block_coef_table(wl.sectors_A, psi_a, su2.pair_meta(wl.ops, terms, wl.ranks))
+    opts = {"kernel": args.kernel} if args.kernel else {}
+    dp = problem.from_workload(wl, block_coef=table, **opts)
+    h = dp.heff
+    psi = dp.psi_fill(wl.seed, wlmod.PSI_STREAM)
+    sig = dp.new_vector(zero=False)
+    for _ in range(max(args.warmup, 3)):
+        dp.apply(psi, sig)
+    burst = min(timed(dp.stream, lambda: dp.apply(psi, sig)) for _ in range(5))
+    clocks = ClockSampler(0)
+    clocks.start()
+    dmrgk.launch_count(reset=True)
+    ms = timed(dp.stream, lambda: dp.apply(psi, sig), reps=args.steps) / args.steps
+    launches = dmrgk.launch_count()
+    clk = clocks.stop()
+    n_sm = dp.ctx.query()[0]
+    peak = n_sm * 128 * (clk.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+    val = h.flops_alg / ms / 1e9
+    print(json.dumps({
+        "metric": "su2_singlet_heff_apply_fp64_tflops", "value": val, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "sectors": len(wl.sectors_A), "largest_sector": max(d for _, d in wl.sectors_A),
+                   "M_multiplets": wl.M_A, "K_pairs": len(wl.terms), "tasks": h.n_tasks, "psi_blocks": len(psi_a),
+                   "zero_scalars": int((table == 0).sum()), "flops_alg_per_apply": h.flops_alg,
+                   "op_bytes_resident": int(dp.op_arena.numel() * 8), "chunks": h.n_chunks, "source_hash": dmrgk.source_hash(),
+                   "l2": "operator arena (>> 126 MB L2) is streamed once per step"},
+        "apply_burst": {"ms": burst, "tflops": h.flops_alg / burst / 1e9},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "tensor", "kernel": "heff_gemm_dmma_kernel (spin-adapted work lists)", "achieved": val, "peak": peak,
+                     "unit": UNIT, "frac": val / peak, "traffic": None, "peak_source": f"of derived: {n_sm} SMs x 128 FP64 flop/clk x max SM clock"},
+        "clocks": clk}), flush=True)
+
+
+def run_expect(args):
+    """--op expect: one step = the per-pair expectation values e_k = <psi, c_k (L_k x R_k) psi> of EVERY operator pair
+    of the workload (dmrgk_heff_expect: the reduced density matrices are such lists
+    with the pairs {c+_i c_j}, {c+_i c+_j c_k c_l}): phase 1 as in the matvec, phase 2 per pair, fused dots.
+    Default workload: config 3.  Its own metric."""
+    import torch
+    import workloads as wlmod
+    from paper_2311_14106_b200 import dmrgk, problem
+    torch.cuda.set_device(0)
+    dmrgk.load()
+    wl = make_workload(args.config if args.config != "4" else "3")
+    dp = problem.from_workload(wl, per_pair_output=1)
+    h = dp.heff
+    psi = dp.psi_fill(wl.seed, wlmod.PSI_STREAM)
+    K = len(wl.terms)
+    for _ in range(max(args.warmup, 2)):
+        out = dp.expect(psi, K)
+    clocks = ClockSampler(0)
+    clocks.start()
+    dmrgk.launch_count(reset=True)
+    ms = timed(dp.stream, lambda: dp.expect(psi, K), reps=args.steps) / args.steps
+    launches = dmrgk.launch_count()
+    clk = clocks.stop()
+    n_sm = dp.ctx.query()[0]
+    peak = n_sm * 128 * (clk.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+    val = h.flops_alg / ms / 1e9
+    print(json.dumps({
+        "metric": "per_pair_expectation_fp64_tflops", "value": val, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": max(args.warmup, 2), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "K_pairs": K, "pairs_per_second": K / ms * 1e3, "tasks": h.n_tasks,
+                   "flops_alg_per_step": h.flops_alg, "chunks": h.n_chunks, "workspace_bytes": int(h.workspace_bytes),
+                   "source_hash": dmrgk.source_hash()},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "tensor", "kernel": "heff_gemm_dmma_kernel (per-pair work lists)", "achieved": val, "peak": peak,
+                     "unit": UNIT, "frac": val / peak, "traffic": None, "peak_source": f"of derived: {n_sm} SMs x 128 FP64 flop/clk x max SM clock"},
+        "sum_check": float(out.sum().item()), "clocks": clk}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -804,7 +890,7 @@ def main():
     ap.add_argument("--shard", default="none", choices=["none", "k"],
                     help="N > 1 only: 'none' = independent replicas (the scope of BASELINE.json), 'k' = split the operator-pair "
                          "list over the ranks and all-reduce sigma (SURVEY §8(f) NEXT-2)")
-    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "enlarge", "loop_probe", "ragged"],
+    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "enlarge", "loop_probe", "ragged", "su2", "expect"],
                     help="davidson (default, the headline hot path) or renorm (NEXT-1 row, its own metric)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -817,6 +903,10 @@ def main():
         run_loop_probe(args)
     elif args.op == "ragged":
         run_ragged(args)
+    elif args.op == "su2":
+        run_su2(args)
+    elif args.op == "expect":
+        run_expect(args)
     else:
         run_ours(args)
 

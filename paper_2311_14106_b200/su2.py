@@ -88,3 +88,18 @@ def singlet_problem(sectors_A, sectors_B, n_target, ops, pairs, device=0, ctx=No
     bc = block_coef_table(sectors_A, psi_a, meta)
     dp.build([(L, R, coef, False, False) for (L, R, coef, _) in pairs], block_coef=bc, **opts)
     return dp
+
+
+def pair_meta(ops, terms, ranks):
+    """[(two_k, parity, Δ2S of the APPLIED left operator)] for `block_coef_table`, from operator specs with `.dq`,
+    `.parity` (or dicts), terms (L, R, coef, trans_L, trans_R) and the doubled rank of every pair.  A pair applied
+    through the transpose flags (the h.c. partner of a stored pair) shifts 2S the other way."""
+    get = lambda o, k: o[k] if isinstance(o, dict) else getattr(o, k)
+    meta = []
+    for (L, R, _, trans_L, _), two_k in zip(terms, ranks):
+        if L is None or R is None:
+            meta.append((0, 0, 0))
+        else:
+            d2 = get(ops[L], "dq")[1]
+            meta.append((two_k, get(ops[L], "parity"), -d2 if trans_L else d2))
+    return meta

@@ -50,3 +50,44 @@ def test_singlet_heff_sigma_and_energy(R, Cn, nA, rotated, keep):
         assert abs(theta - E_singlet) <= TOL_ENERGY * max(1.0, abs(E_singlet))
     else:
         assert theta >= E_singlet - 1e-9                                        # variational
+
+
+def oracle_block_coef(wl, pb):
+    """The oracle's recoupling table of a spin-adapted workload: brute-force Clebsch–Gordan sums
+    (oracle.su2.recoupling_singlet) times the Jordan–Wigner sign, per (pair, input ψ block)."""
+    table = {}
+    for k, ((L, R, c, tL, tR), k2) in enumerate(zip(pb.terms, wl.ranks)):
+        for (a, b) in pb.psi_blocks():
+            N, tS = pb.sectors_A[a][0]
+            if L is None or R is None:
+                table[(k, (a, b))] = 1.0
+                continue
+            d2 = pb.ops[L]["dq"][1] * (-1 if tL else 1)
+            x = osu2.recoupling_singlet(tS, tS + d2, k2) if tS + d2 >= 0 else 0.0
+            table[(k, (a, b))] = (-x if (pb.ops[L]["parity"] and N % 2) else x)
+    return table
+
+
+@pytest.mark.parametrize("opts", [{}, {"split_waves": 64}, {"order_policy": 2}, {"kernel": 5}])
+def test_su2_structured_workload_vs_oracle(opts):
+    """The spin-adapted workload of `bench.py --op su2`, scaled down (6 orbitals per half, 900 multiplets, synthetic
+    reduced matrix elements, sectors up to 2S = 6, all families, h.c. partners through the transpose flags): σ with the
+    library's closed-form recoupling table against the oracle's blockwise tier with the brute-force table."""
+    import workloads as wlmod
+    from paper_2311_14106_b200 import problem, su2
+    thin = lambda fam, i: fam in ("F1", "F2") or i % 3 == 0
+    wl = wlmod.su2_singlet_workload(6, 900, seed=16, keep=thin)
+    pb = heff.problem_from_workload(wl)
+    pb.block_coef = oracle_block_coef(wl, pb)
+    assert any(v == 0.0 for v in pb.block_coef.values())            # triangle rule: S = 0 → S′ = 0 through a rank-1 pair
+    ref = heff.sigma_blockwise(pb)
+    terms = [(t.L, t.R, t.coef, t.trans_L, t.trans_R) for t in wl.terms]
+    psi_a = [a for (a, _, _, _, _) in wlmod.psi_block_table(wl.sectors_A, wl.sectors_B, wl.target)]
+    table = su2.block_coef_table(wl.sectors_A, psi_a, su2.pair_meta(wl.ops, terms, wl.ranks))
+    dp = problem.from_workload(wl, block_coef=table, **opts)
+    psi = dp.psi_fill(wl.seed, wlmod.PSI_STREAM)
+    sigma = dp.apply(psi)
+    assert rel_max(dp.to_blocks(sigma), ref) <= TOL_SIGMA
+    assert padding_is_zero(dp, sigma)
+    assert dp.heff.n_tasks == len(heff.enumerate_tasks(pb))
+    assert dp.heff.flops_alg == heff.flops_alg(pb)

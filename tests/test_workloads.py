@@ -64,3 +64,24 @@ def test_symmetric_ops_are_symmetric():
     i = next(i for i, o in enumerate(wl.ops) if o.symmetric)
     for blk in w.fill_op_host(wl, i).values():
         assert np.array_equal(blk, blk.T)
+
+
+def test_su2_singlet_workload_structure():
+    """The spin-adapted input recipe: multiplet counts against the Fock-space dimension,
+    sector labels, one stored operator per Δ(2S), ranks."""
+    import workloads as wlmod
+    for n in (1, 2, 3, 5):      # Σ (2S+1)·#multiplets = 4^n
+        tot = sum((t + 1) * wlmod.su2_multiplet_count(n, N, t) for N in range(2 * n + 1) for t in range(0, n + 1))
+        assert tot == 4 ** n
+    assert [wlmod.su2_multiplet_count(1, N, t) for (N, t) in ((0, 0), (1, 1), (2, 0), (1, 0), (2, 2))] == [1, 1, 1, 0, 0]
+    wl = wlmod.su2_singlet_workload(6, 900, seed=16)
+    assert sum(d for _, d in wl.sectors_A) == 900 == sum(d for _, d in wl.sectors_B)
+    assert all((N + t) % 2 == 0 and t >= 0 for (N, t), _ in wl.sectors_A)          # N + 2S even: the library's sign never fires
+    assert [(N, -t) for (N, t), _ in wl.sectors_A] == [q for q, _ in wl.sectors_B]
+    assert len(wl.ranks) == len(wl.terms) == 2 + 4 * 12 + 2 * 66 + 2 * 66 + 12      # the U(1)×U(1) count of 12 spin-orbitals per half
+    for t, k2 in zip(wl.terms, wl.ranks):
+        if t.L is not None and t.R is not None:
+            dl, dr = wl.ops[t.L].dq, wl.ops[t.R].dq
+            assert dl[0] == -dr[0] and dl[1] == -dr[1] and abs(dl[1]) <= k2 and (dl[1] - k2) % 2 == 0
+    blocks = wlmod.psi_block_table(wl.sectors_A, wl.sectors_B, wl.target)
+    assert len(blocks) == len(wl.sectors_A)                                          # every A sector has its singlet partner

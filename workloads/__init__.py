@@ -13,5 +13,5 @@ from .configs import (  # noqa: F401
     spinless_term_structure, hubbard_term_structure, op_block_table,
     psi_block_table, fill_op_host, fill_psi_host, op_stream_id, op_stream_of, sub_workload, PSI_STREAM,
     config3, config4, config4_realspace, config5, config5_keep, config5_staged_ops,
-    renorm_basis, fill_phi_host, PHI_STREAM,
+    renorm_basis, fill_phi_host, PHI_STREAM, su2_singlet_workload, su2_multiplet_count,
 )

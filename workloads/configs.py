@@ -354,6 +354,63 @@ def config5_staged_ops(wl):
     return [i for i in range(len(wl.ops)) if i % 7 == 3]
 
 
+# ----------------------------------------------------------------------------
+# SU(2) spin-adapted singlet workload: structure only
+# ----------------------------------------------------------------------------
+def su2_multiplet_count(n_orb, N, two_s):
+    """Number of spin-S multiplets with N electrons in n_orb orbitals: dim(S_z = S) − dim(S_z = S + 1)."""
+    if (N + two_s) % 2 or two_s < 0:
+        return 0
+    up, dn = (N + two_s) // 2, (N - two_s) // 2
+    c = lambda a, b: binom(n_orb, a) * binom(n_orb, b) if 0 <= a <= n_orb and 0 <= b <= n_orb else 0
+    return c(up, dn) - c(up + 1, dn - 1)
+
+
+def su2_singlet_workload(n_half=18, M=12288, seed=6, name=None, keep=None, width_n=8.0, width_s=6.0):
+    """The operator-pair list of a Hubbard-type lattice half with n_half orbitals per side in SPIN-ADAPTED form,
+    for a spin-singlet target at half filling — sector structure and term structure only, values synthetic (r17).
+
+    Sectors: A labelled (N, 2S), B labelled (N, −2S) (for total spin 0 both halves of a ψ block carry the same S,
+    so the labels add up to the target (2·n_half, 0)); dims count MULTIPLETS, ∝ (2S+1)·exp(−(N−n_half)²/width_n
+    − S(S+1)/width_s), capped by the number of multiplets that exist, M in total (M = 3·D: a site has three
+    multiplets).  Terms: the families F0-F4 over the orbitals, every rank-k tensor operator stored once per
+    Δ(2S) ∈ {−2k … 2k} — which is the U(1)×U(1) list with the two spin components of an orbital replaced by the two
+    "virtual modes" of label shift (1, +1) and (1, −1).  ``wl.ranks[k]`` is the doubled tensor rank of pair k (an
+    input of the recoupling table): ½ for F1/F2, 1 for the Δ(2S) = ±2 pairs of F3/F4, and of the two Δ(2S) = 0 pairs of
+    an orbital pair one is the triplet's and one the singlet's."""
+    import re
+    qs = []
+    for N in range(2 * n_half + 1):
+        for two_s in range(N % 2, min(N, 2 * n_half - N) + 1, 2):
+            if su2_multiplet_count(n_half, N, two_s) > 0:
+                qs.append((N, two_s))
+    w = [(t + 1) * math.exp(-((N - n_half) ** 2) / width_n - (t / 2.0) * (t / 2.0 + 1.0) / width_s) for N, t in qs]
+    caps = [su2_multiplet_count(n_half, N, t) for N, t in qs]
+    dims = gaussian_sectors(M, w, caps)
+    sectors_A = [(q, d) for q, d in zip(qs, dims)]
+    sectors_B = [((N, -t), d) for (N, t), d in zip(qs, dims)]
+    wl = Workload(name or f"su2_singlet_n{n_half}_M{M}", seed, 2, sectors_A, sectors_B, (2 * n_half, 0))
+    shifts_A = [(1, 1), (1, -1)] * n_half
+    shifts_B = [(1, -1), (1, 1)] * n_half
+    _family_builder(wl, shifts_A, shifts_B, keep=keep)
+    wl.ranks = []
+    for t in wl.terms:
+        fam = t.family.replace("^hc", "")
+        if fam == "F0":
+            wl.ranks.append(0)
+        elif fam in ("F1", "F2"):
+            wl.ranks.append(1)
+        else:
+            op = wl.ops[t.L]
+            if op.dq[1] != 0:
+                wl.ranks.append(abs(op.dq[1]))
+            else:
+                idx = [int(x) for x in re.findall(r"\d+", op.tag)]
+                same_orbital = len(idx) == 2 and idx[0] // 2 == idx[1] // 2 and fam == "F3"
+                wl.ranks.append(0 if same_orbital or idx[0] % 2 else 2)
+    return wl
+
+
 def sub_workload(wl, term_ids, name=None):
     """The workload restricted to the operator pairs ``term_ids`` (a shard of the k list):
     same sectors and target, only the stored operators those pairs touch, re-indexed, each keeping the
