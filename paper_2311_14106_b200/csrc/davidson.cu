@@ -9,7 +9,8 @@
 //          t = r/(θ − d) guarded ; t ← t − V(Vᵀt) twice ; v = t/‖t‖ ; w = H v ; append
 //
 // Everything ψ-sized stays on the device; only the Rayleigh matrix entries (2(m+1) doubles), ‖r‖²,
-// ‖t‖² come back and (y, θ) go up per step.  G is kept on the host and extended by one row and
+// ‖t‖² come back and (y, θ) go up per step — two host synchronisations per step: after the residual (the
+// convergence decision precedes the expensive apply) and after the Rayleigh entries.  G is kept on the host and extended by one row and
 // column per step: its entries v_i·w_j never change while the basis is only appended to.
 #include "internal.h"
 #include <cmath>
@@ -118,11 +119,13 @@ int32_t orthogonalise(dmrgk_davidson* d, double* t) {
 }
 
 // Rayleigh-matrix entries of the newest basis vector (index j = m): G[i][j] = v_i·w_j, G[j][i] = w_i·v_j.
+// The read-back also brings ‖t‖² of the step (slot TT_SLOT of `out`), so a step has two host syncs, not three.
+constexpr int TT_SLOT = 160;
 int32_t extend_G(dmrgk_davidson* d) {
     const int j = d->m, mm = d->m_max;
     DMRGK_TRY(dmrgk_vec_multi_dot(d->ctx, d->n, j + 1, d->V, d->n, d->W + int64_t(j) * d->n, d->out, d->scratch, d->main));
     DMRGK_TRY(dmrgk_vec_multi_dot(d->ctx, d->n, j + 1, d->W, d->n, d->V + int64_t(j) * d->n, d->out + 64, d->scratch, d->main));
-    DMRGK_TRY(read_back(d, 128));
+    DMRGK_TRY(read_back(d, TT_SLOT + 1));
     for (int i = 0; i <= j; ++i) {
         d->G[size_t(i) * mm + j] = d->host[64 + i];
         d->G[size_t(j) * mm + i] = d->host[128 + i];
@@ -249,20 +252,27 @@ int32_t dmrgk_davidson_step(dmrgk_davidson* d, double* theta, double* resnorm, i
     }
     DMRGK_TRY(dmrgk_vec_precond(d->ctx, d->n, d->r, d->diag, theta_dev, d->t, d->main));
     DMRGK_TRY(orthogonalise(d, d->t));
-    DMRGK_TRY(dmrgk_vec_multi_dot(d->ctx, d->n, 1, d->t, d->n, d->t, d->out, d->scratch, d->main));
-    DMRGK_TRY(read_back(d, 1));
-    if (!(std::sqrt(d->host[64]) >= 1e-14 * d->rho)) {   // correction vanished: fall back to the residual
-        DMRGK_CUDA(cudaMemcpyAsync(d->t, d->r, size_t(d->n) * 8, cudaMemcpyDeviceToDevice, d->main));
-        DMRGK_TRY(orthogonalise(d, d->t));
-        DMRGK_TRY(dmrgk_vec_multi_dot(d->ctx, d->n, 1, d->t, d->n, d->t, d->out, d->scratch, d->main));
-        DMRGK_TRY(read_back(d, 1));
-        if (!(d->host[64] > 0.0)) return fail(DMRGK_ENOTCONV, "davidson_step: the search space is exhausted (‖t‖ = 0)");
-    }
+    // ‖t‖² stays on the device: the new basis vector, its image and the Rayleigh entries are computed without
+    // waiting for it, and it comes back with them; a vanished correction (rare) is detected then and redone
+    double* tt_dev = d->out + TT_SLOT;
+    DMRGK_TRY(dmrgk_vec_multi_dot(d->ctx, d->n, 1, d->t, d->n, d->t, tt_dev, d->scratch, d->main));
     double* v = d->V + int64_t(d->m) * d->n;
     double* w = d->W + int64_t(d->m) * d->n;
-    DMRGK_TRY(dmrgk_vec_scal_dev(d->ctx, d->n, d->out, 3, d->t, v, d->main));
+    DMRGK_TRY(dmrgk_vec_scal_dev(d->ctx, d->n, tt_dev, 3, d->t, v, d->main));
     DMRGK_TRY(apply_h(d, v, w));
     DMRGK_TRY(extend_G(d));
+    if (!(std::sqrt(d->host[64 + TT_SLOT]) >= 1e-14 * d->rho)) {   // correction vanished: fall back to the residual
+        d->n_apply -= 1;
+        DMRGK_CUDA(cudaMemcpyAsync(d->t, d->r, size_t(d->n) * 8, cudaMemcpyDeviceToDevice, d->main));
+        DMRGK_TRY(orthogonalise(d, d->t));
+        DMRGK_TRY(dmrgk_vec_multi_dot(d->ctx, d->n, 1, d->t, d->n, d->t, tt_dev, d->scratch, d->main));
+        DMRGK_CUDA(cudaMemcpyAsync(d->host + 64 + TT_SLOT, tt_dev, 8, cudaMemcpyDeviceToHost, d->main));
+        DMRGK_CUDA(cudaStreamSynchronize(d->main));
+        if (!(d->host[64 + TT_SLOT] > 0.0)) return fail(DMRGK_ENOTCONV, "davidson_step: the search space is exhausted (‖t‖ = 0)");
+        DMRGK_TRY(dmrgk_vec_scal_dev(d->ctx, d->n, tt_dev, 3, d->t, v, d->main));
+        DMRGK_TRY(apply_h(d, v, w));
+        DMRGK_TRY(extend_G(d));
+    }
     d->m += 1;
     return DMRGK_OK;
 }
