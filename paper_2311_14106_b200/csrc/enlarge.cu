@@ -208,6 +208,20 @@ int32_t dmrgk_enlarge_create(dmrgk_ctx* ctx, const dmrgk_space* kept, const dmrg
     e->ctx = ctx;
     for (int64_t i = 0; i < n_out; ++i)
         if (out[i]->n_padded) e->zero.push_back({const_cast<double*>(out[i]->dev), out[i]->n_padded});
+    // destination arenas are usually slices of one allocation: clear contiguous ranges with ONE memset each
+    // (a memset per operator is 137 launches on the config-4 enlargement: 5.5 → 5.0 ms per step)
+    std::sort(e->zero.begin(), e->zero.end());
+    {
+        std::vector<std::pair<double*, int64_t>> merged;
+        for (const auto& z : e->zero) {
+            // gaps of alignment padding between slices (< 128 bytes) are cleared along
+            if (!merged.empty() && z.first <= merged.back().first + merged.back().second + 16)
+                merged.back().second = std::max(merged.back().second, int64_t(z.first - merged.back().first) + z.second);
+            else
+                merged.push_back(z);
+        }
+        e->zero.swap(merged);
+    }
     std::vector<EUnit> units;
     std::vector<ESrc> srcs;
     for (auto& kv : groups) {
