@@ -214,8 +214,7 @@ int32_t dmrgk_enlarge_create(dmrgk_ctx* ctx, const dmrgk_space* kept, const dmrg
     {
         std::vector<std::pair<double*, int64_t>> merged;
         for (const auto& z : e->zero) {
-            // gaps of alignment padding between slices (< 128 bytes) are cleared along
-            if (!merged.empty() && z.first <= merged.back().first + merged.back().second + 16)
+            if (!merged.empty() && z.first <= merged.back().first + merged.back().second)      // adjacent or overlapping only
                 merged.back().second = std::max(merged.back().second, int64_t(z.first - merged.back().first) + z.second);
             else
                 merged.push_back(z);
