@@ -402,6 +402,16 @@ int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* si
 int32_t dmrgk_probe_gemm_loop(dmrgk_ctx* ctx, int32_t kind, int32_t ktiles, const double* buf_dev,
                               int64_t buf_doubles, double* sink_dev, double* flops, void* stream);
 
+/* Host only (no device needed): the tile boundaries the task-list builder uses for a block dimension of
+ * `extent` rows (tile_max = 64, or 128 for the tall-tile variant) or padded columns (tile_max = 64) — the
+ * balanced tiling of DESIGN.md §4.1: ceil(extent/tile_max) tiles, origins at multiples of 16, extents that
+ * differ by at most 16, larger tiles first.  Writes n + 1 boundaries (the last one = extent) to `cuts` if
+ * cap ≥ n + 1 and returns n; DMRGK_EINVAL (negative) on bad arguments.  For tests of the host logic. */
+int32_t dmrgk_plan_tile_cuts(int32_t extent, int32_t tile_max, int32_t* cuts, int32_t cap);
+/* Host only: the cost per k-tile the planner assigns to a tile of rows × cols computed elements (fragment
+ * products of its fullest warp × 4, with the latency floor for thin tiles; a full 64×64 tile costs 64). */
+int32_t dmrgk_plan_tile_cost(int32_t rows, int32_t cols);
+
 #ifdef __cplusplus
 }
 #endif

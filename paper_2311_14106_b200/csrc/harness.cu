@@ -163,3 +163,19 @@ int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* si
 }
 
 }  // extern "C"
+
+// ---- host-only views of the planner's tiling rules (tests of the host logic) ------------------------
+extern "C" int32_t dmrgk_plan_tile_cuts(int32_t extent, int32_t tile_max, int32_t* cuts, int32_t cap) {
+    if (extent < 0 || (tile_max != 64 && tile_max != 128) || !cuts)
+        return dmrgk::fail(DMRGK_EINVAL, "plan_tile_cuts: extent ≥ 0, tile_max 64 or 128, cuts not NULL");
+    std::vector<int> c;
+    dmrgk::tile_cuts(extent, tile_max, c);
+    if (int32_t(c.size()) > cap) return dmrgk::fail(DMRGK_EINVAL, "plan_tile_cuts: %d boundaries need cap ≥ %d", int(c.size()), int(c.size()));
+    for (size_t i = 0; i < c.size(); ++i) cuts[i] = c[i];
+    return int32_t(c.size()) - 1;
+}
+
+extern "C" int32_t dmrgk_plan_tile_cost(int32_t rows, int32_t cols) {
+    if (rows < 1 || cols < 1 || rows > 128 || cols > 64) return dmrgk::fail(DMRGK_EINVAL, "plan_tile_cost: 1 ≤ rows ≤ 128, 1 ≤ cols ≤ 64");
+    return int32_t(dmrgk::tile_cost(rows, cols));
+}

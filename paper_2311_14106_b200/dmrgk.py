@@ -115,6 +115,8 @@ SIGNATURES = {
     "dmrgk_op_fill_normal": (_i32, [_p, _p, _u64, _u64, _i32, _i32, _p]),
     "dmrgk_layout_fill_normal": (_i32, [_p, _p, _u64, _u64, _p]),
     "dmrgk_probe_fp64": (_i32, [_p, _i32, _i64, _p, _pf64, _p]),
+    "dmrgk_plan_tile_cuts": (_i32, [_i32, _i32, _p, _i32]),
+    "dmrgk_plan_tile_cost": (_i32, [_i32, _i32]),
     "dmrgk_probe_gemm_loop": (_i32, [_p, _i32, _i32, _p, _i64, _p, _pf64, _p]),
 }
 
@@ -631,3 +633,21 @@ def probe_fp64(ctx, kind, iters, sink, stream=None):
     fl = C.c_double()
     check(ctx.lib.dmrgk_probe_fp64(ctx.h, kind, iters, _dev(sink), C.byref(fl), _stream(stream)))
     return fl.value
+
+
+def plan_tile_cuts(extent, tile_max=64):
+    """Tile boundaries of a block dimension (host only): [0, …, extent]."""
+    lib = load()
+    out = np.zeros(extent // 16 + 3, np.int32)
+    n = lib.dmrgk_plan_tile_cuts(int(extent), int(tile_max), out.ctypes.data, len(out))
+    if n < 0:
+        raise DmrgkError(n, last_error())
+    return [int(x) for x in out[:n + 1]]
+
+
+def plan_tile_cost(rows, cols):
+    lib = load()
+    c = lib.dmrgk_plan_tile_cost(int(rows), int(cols))
+    if c < 0:
+        raise DmrgkError(c, last_error())
+    return int(c)

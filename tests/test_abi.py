@@ -80,3 +80,25 @@ def test_product_does_not_import_oracle():
         if f.endswith(".py"):
             text = open(os.path.join(ROOT, "oracle", f), encoding="utf-8").read()
             assert "paper_2311_14106_b200" not in re.sub(r'""".*?"""', "", text, flags=re.S), f
+
+
+def test_balanced_tile_plan_host_rules():
+    """The planner's tiling rules (DESIGN.md §4.1 "balanced tiles"), host only: ceil(extent/tile_max) tiles that
+    cover the extent exactly, origins at multiples of 16, extents ≤ tile_max that differ by at most 16 with the
+    larger ones first; the cost of a tile = fragment products of its fullest warp × 4 with a floor."""
+    from paper_2311_14106_b200 import dmrgk
+    for tile_max in (64, 128):
+        for extent in list(range(0, 300)) + [573, 640, 650, 794, 1000, 4096]:
+            cuts = dmrgk.plan_tile_cuts(extent, tile_max)
+            n = len(cuts) - 1
+            assert n == -(-extent // tile_max) and cuts[0] == 0 and cuts[-1] == extent
+            ext = [b - a for a, b in zip(cuts[:-1], cuts[1:])]
+            assert all(0 < e <= tile_max for e in ext) and all(c % 16 == 0 for c in cuts[:-1])
+            if n:
+                full = [-(-e // 16) for e in ext]                       # in 16-row panels
+                assert max(full) - min(full) <= 1 and full == sorted(full, reverse=True)
+    assert dmrgk.plan_tile_cuts(650) == [0, 64, 128, 192, 256, 320, 384, 448, 512, 560, 608, 650]
+    assert dmrgk.plan_tile_cost(64, 64) == 64 and dmrgk.plan_tile_cost(48, 64) == 48 and dmrgk.plan_tile_cost(52, 64) == 64
+    assert dmrgk.plan_tile_cost(128, 64) == 128 and dmrgk.plan_tile_cost(8, 8) == dmrgk.plan_tile_cost(1, 1) == 24   # the floor
+    with pytest.raises(dmrgk.DmrgkError):
+        dmrgk.plan_tile_cuts(10, 32)
