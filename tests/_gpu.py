@@ -150,13 +150,14 @@ class DeviceInputs:
         self.checked += blk.size
 
 
-def oracle_sigma_on_block(wl, inputs, a_out, b_out, psi_blocks, terms_per_call=96, want_diag=False):
+def oracle_sigma_on_block(wl, inputs, a_out, b_out, psi_blocks, terms_per_call=96, want_diag=False, coef_of=None):
     """σ[(a_out, b_out)] (and optionally diag(H_eff) on that block) from oracle.heff.sigma_blockwise.
 
     For every term only the stored L block whose APPLIED output sector is a_out and the R block whose
     applied output sector is b_out can contribute; they are fetched only if the input pair is a ψ
     block.  The term list is cut into groups (k-additivity of the sum) so that host
-    memory holds a bounded number of operator blocks at a time; the oracle itself is called unchanged."""
+    memory holds a bounded number of operator blocks at a time; the oracle itself is called unchanged.
+    ``coef_of(k, (a_in, b_in))`` supplies the per-(pair, input block) scalar of a spin-adapted problem."""
     from oracle import heff
     psi_keys = set(psi_blocks)
     terms = [(t.L, t.R, t.coef, t.trans_L, t.trans_R) for t in wl.terms]
@@ -169,8 +170,8 @@ def oracle_sigma_on_block(wl, inputs, a_out, b_out, psi_blocks, terms_per_call=9
 
     for g0 in range(0, len(terms), terms_per_call):
         ops = [{"half": s.half, "dq": tuple(s.dq), "parity": s.parity, "blocks": {}} for s in wl.ops]
-        sub = []
-        for (L, R, coef, tL, tR) in terms[g0:g0 + terms_per_call]:
+        sub, bc = [], {}
+        for k_glob, (L, R, coef, tL, tR) in enumerate(terms[g0:g0 + terms_per_call], start=g0):
             a_in, kl = needed(L, tL, a_out)
             b_in, kr = needed(R, tR, b_out)
             if a_in is None or b_in is None or (a_in, b_in) not in psi_keys:
@@ -181,10 +182,12 @@ def oracle_sigma_on_block(wl, inputs, a_out, b_out, psi_blocks, terms_per_call=9
                     inputs.check_inputs(idx, key, blk)
                     ops[idx]["blocks"][key] = blk
             sub.append((L, R, coef, tL, tR))
+            if coef_of is not None:
+                bc[(len(sub) - 1, (a_in, b_in))] = coef_of(k_glob, (a_in, b_in))
         if not sub:
             continue
         pb = heff.Problem(wl.n_charges, list(wl.sectors_A), list(wl.sectors_B), tuple(wl.target), ops, sub,
-                          psi_blocks, wl.name)
+                          psi_blocks, wl.name, bc if coef_of is not None else None)
         part = heff.sigma_blockwise(pb)[(a_out, b_out)]
         sigma = part if sigma is None else sigma + part
         if want_diag:

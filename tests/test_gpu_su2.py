@@ -91,3 +91,42 @@ def test_su2_structured_workload_vs_oracle(opts):
     assert padding_is_zero(dp, sigma)
     assert dp.heff.n_tasks == len(heff.enumerate_tasks(pb))
     assert dp.heff.flops_alg == heff.flops_alg(pb)
+
+
+def test_su2_workload_of_the_bench_sampled_blocks():
+    """`bench.py --op su2` at its full size (190 sectors (N, 2S), 12288 multiplets, K = 2702 pairs, 99 GB of
+    reduced operators), in the launch configuration that op times: σ on ≥ 8 sampled output blocks — the largest,
+    the smallest, both edges of the sector range — against the oracle's blockwise tier on operator blocks read
+    back D2H, the oracle's recoupling scalars by brute-force Clebsch–Gordan sums, the library's in closed form.
+    Error against the oracle's scale (1e-11) and per block (1e-10)."""
+    import workloads as wlmod
+    from paper_2311_14106_b200 import problem, su2
+    from _gpu import DeviceInputs, sample_output_blocks, oracle_sigma_on_block, TOL_BLOCK
+    wl = wlmod.su2_singlet_workload()
+    terms = [(t.L, t.R, t.coef, t.trans_L, t.trans_R) for t in wl.terms]
+    psi_a = [a for (a, _, _, _, _) in wlmod.psi_block_table(wl.sectors_A, wl.sectors_B, wl.target)]
+    table = su2.block_coef_table(wl.sectors_A, psi_a, su2.pair_meta(wl.ops, terms, wl.ranks))
+    dp = problem.from_workload(wl, block_coef=table)
+    inputs = DeviceInputs(wl, dp)
+    picks = sample_output_blocks(dp.table)
+    assert len(picks) >= 8
+    psi = dp.psi_fill(wl.seed, wlmod.PSI_STREAM)
+    psi_blocks = dp.to_blocks(psi)
+    got = dp.to_blocks(dp.apply(psi))
+
+    def coef_of(k, blk):
+        L, R, _, tL, _ = terms[k]
+        if L is None or R is None:
+            return 1.0
+        N, tS = wl.sectors_A[blk[0]][0]
+        d2 = wl.ops[L].dq[1] * (-1 if tL else 1)
+        x = osu2.recoupling_singlet(tS, tS + d2, wl.ranks[k]) if tS + d2 >= 0 else 0.0
+        return -x if (wl.ops[L].parity and N % 2) else x
+
+    refs = {k: oracle_sigma_on_block(wl, inputs, k[0], k[1], psi_blocks, coef_of=coef_of) for k in picks}
+    scale = max(np.abs(v).max() for v in refs.values())
+    for k, ref in refs.items():
+        err = np.abs(got[k] - ref).max()
+        assert err <= TOL_SIGMA * scale, (k, err / scale)
+        assert err <= TOL_BLOCK * np.abs(ref).max(), (k, "per-block")
+    assert inputs.checked > 0
