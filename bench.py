@@ -27,8 +27,8 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "heff_apply_fp64_tflops_in_davidson_step"
-SAMPLE_EVERY = {"4": 100, "3": 100, "3b": 268, "2": 8, "5": 143, "5r": 143}   # --impl reference: every n-th operator pair (host-generated values)
-CPU_EVERY = {"4": 20, "3": 20, "3b": 40, "2": 4, "5": 20, "5r": 20}              # cpu_baseline leg: ≈ 5 % of the pairs (values read back D2H)
+SAMPLE_EVERY = {"4": 100, "3": 100, "3b": 268, "2": 8, "5": 143, "5r": 143, "4rs": 2}   # --impl reference: every n-th operator pair (host-generated values)
+CPU_EVERY = {"4": 20, "3": 20, "3b": 40, "2": 4, "5": 20, "5r": 20, "4rs": 1}              # cpu_baseline leg: ≈ 5 % of the pairs (values read back D2H)
 UNIT = "TFLOP/s"
 
 
@@ -36,6 +36,8 @@ def make_workload(name):
     import workloads as wlmod
     if name == "4":
         return wlmod.config4()
+    if name == "4rs":
+        return wlmod.config4_realspace()     # configs[3], real-space basis: K = 50 pairs (H_A, H_B and the boundary hoppings)
     if name == "3":
         return wlmod.config3()
     if name == "3b":
@@ -879,7 +881,7 @@ def main():
     ap.add_argument("--steps", type=int, default=8)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="4", choices=["2", "3", "3b", "4", "5", "5r"])
+    ap.add_argument("--config", default="4", choices=["2", "3", "3b", "4", "4rs", "5", "5r"])
     ap.add_argument("--m-max", dest="m_max", type=int, default=16)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--kernel", type=int, default=0, choices=[0, 2, 3, 4, 5],
