@@ -10,12 +10,14 @@
 //
 // Staging (round 2): operand tiles are fetched by the TMA unit.  Every block is stored in the panel
 // layout (internal.h), in which a ≤64×16 K-major tile — and each 16×16 piece of an MN-major one — is
-// one contiguous chunk, already swizzled; ONE elected thread per k-tile issues 1–8 cp.async.bulk
-// copies (SASS UBLKCP) that complete on the stage's `full` mbarrier, the four compute warps wait on
-// it, run LDS.64 + DMMA only, and release the stage through its `empty` mbarrier.  There is no
-// __syncthreads and no per-thread address arithmetic in the k-loop.  The producer role rotates over
-// the warps (tile t is fetched by lane 0 of warp t mod 4).  2 CTAs per SM: with the warps decoupled
-// by mbarriers the DMMA pipe runs fastest at two resident warps per scheduler (profiles/r2_tma_summary.md).
+// one contiguous chunk, already swizzled; one elected lane of a dedicated PRODUCER warp issues 2–8
+// cp.async.bulk copies (SASS UBLKCP) per k-tile of 32 that complete on the stage's `full` mbarrier, the four
+// CONSUMER warps wait on it, run LDS.64 + DMMA only, and release the stage through its `empty` mbarrier.
+// There is no __syncthreads and no per-thread address arithmetic in the k-loop.  The kernel is persistent:
+// 3 CTAs per SM (2 stages of 32 KB each) claim work units from a device-side queue; the units of a block are
+// balanced tiles whose fragments are split evenly over the warp rows and columns (internal.h tile_cuts).
+// Design choices and their measurements: DESIGN.md §4.1, profiles/r2_tma_summary.md, r2_ragged.md,
+// r2_final_summary.md.
 #include "internal.h"
 #include <algorithm>
 
