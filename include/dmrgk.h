@@ -239,6 +239,21 @@ int64_t dmrgk_vec_scratch_bytes(int32_t nv);
 int32_t dmrgk_vec_multi_dot(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double* X_dev,
                             int64_t stride, const double* y_dev, double* out_dev,
                             void* scratch_dev, void* stream);
+/* The same dots with no scratch argument, for callers that cannot allocate device memory: a sweep driver
+ * whose operator arenas and staging ring already fill HBM, a host code that is handed a fixed set of
+ * device buffers and owns no allocator, or a step running beside the side-stream operator copies, which
+ * a cudaMalloc / cudaFree would stall by synchronising the device.  The per-CTA partial sums go to a
+ * 592 KiB array inside the library image (held by every GPU that loads the library until exit), so:
+ *   - nv ≤ 64, DMRGK_EINVAL beyond that (n is unlimited); arguments otherwise as dmrgk_vec_multi_dot's,
+ *     same kernels, bit-identical results;
+ *   - the call itself makes no cudaMalloc / cudaFree and no allocating library call;
+ *   - the first call on each device looks the array's device address up (cudaGetSymbolAddress, with that
+ *     device current); make that first call before any stream capture begins;
+ *   - there is one array per GPU, shared by all calls: calls that may overlap on the GPU (different
+ *     streams with no ordering between them) race on it — order them.  Nothing in it needs clearing: a
+ *     call reads only the slots it has itself written. */
+int32_t dmrgk_vec_multi_dot_noalloc(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double* X_dev,
+                                    int64_t stride, const double* y_dev, double* out_dev, void* stream);
 /* y[i] = beta·y[i] + alpha·Σ_j coef_dev[j]·X[j·stride + i]  (coefficients read from device memory,
  * nv ≤ 64; beta = 0 overwrites without reading y). */
 int32_t dmrgk_vec_multi_axpy(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double* X_dev,

@@ -9,6 +9,8 @@
 // the partials in index order), so results are bit-reproducible run to run.  No atomics.
 #include "internal.h"
 
+#include <mutex>
+
 namespace dmrgk {
 
 constexpr int VEC_THREADS = 256;
@@ -228,6 +230,78 @@ int32_t dmrgk_vec_multi_dot(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double*
     const int64_t n2 = n / 2;
     const int grid = vec_grid(n2);
     double* partial = static_cast<double*>(scratch_dev);
+    for (int j0 = 0; j0 < nv; j0 += 8) {
+        const int c = std::min(8, nv - j0);
+        if (c == 1) launch_dot1<1>(grid, st, n2, c, j0, X_dev, stride, y_dev, partial, nv);
+        else if (c <= 4) launch_dot1<4>(grid, st, n2, c, j0, X_dev, stride, y_dev, partial, nv);
+        else launch_dot1<8>(grid, st, n2, c, j0, X_dev, stride, y_dev, partial, nv);
+        DMRGK_CUDA(cudaGetLastError());
+    }
+    multi_dot_stage2<<<1, VEC_THREADS, 0, st>>>(grid, nv, partial, out_dev);
+    count_launch();
+    DMRGK_CUDA(cudaGetLastError());
+    return DMRGK_OK;
+}
+
+// ---- dmrgk_vec_multi_dot_noalloc: the same dots for callers that have no device memory to give ----
+// dmrgk_vec_multi_dot needs a caller-allocated scratch buffer for its per-CTA partial sums.  Some users
+// of this library cannot supply one: a sweep driver that has already handed the whole of HBM to the
+// operator arenas and the staging ring (config 5 is sized to do exactly that), a C or Fortran host
+// code that is given a fixed set of device buffers by its framework and owns no allocator, or a step
+// running next to the side-stream operator copies, where a cudaMalloc / cudaFree would synchronise the
+// device and stall that overlap.  For them the partial sums live in the array below, which is part
+// of the library image: every GPU that loads libdmrgk.so holds these 592 KiB until the process exits.
+//
+//   * limit: nv ≤ DMRGK_NOALLOC_MAX_NV (64); n is not limited (the grid is capped at VEC_MAX_BLOCKS).
+//   * nothing has to start at zero: stage 2 reads partial[b][j] only for b < grid, j < nv, and stage 1
+//     of the same call has written every one of those, so the previous call's contents are never read.
+//   * there is ONE array per GPU, shared by every call from every thread and stream: two calls whose
+//     kernels can overlap on the GPU (different streams, no ordering between them) race on it.
+//   * `vec_noalloc_partials` as written in HOST code is only the host-side stand-in of the symbol, not a
+//     device address; the kernels get the address cudaGetSymbolAddress returns, fetched once per device
+//     with that device current, by the first call on that device.  That first call therefore does a
+//     little set-up work (it may load the module) and should be made before any stream capture begins.
+constexpr int DMRGK_NOALLOC_MAX_NV = 64;
+constexpr int DMRGK_NOALLOC_MAX_DEVICES = 64;
+static __device__ __align__(256) double vec_noalloc_partials[size_t(VEC_MAX_BLOCKS) * DMRGK_NOALLOC_MAX_NV];
+
+static std::mutex g_noalloc_mu;
+static double* g_noalloc_ptr[DMRGK_NOALLOC_MAX_DEVICES] = {};   // device address of the array, per device
+
+// Device address of vec_noalloc_partials on `device` (which must be current).  No allocation.
+static int32_t noalloc_partials(int device, double** out) {
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_ptr[device]) {
+        double* p = nullptr;
+        DMRGK_CUDA(cudaGetSymbolAddress(reinterpret_cast<void**>(&p), vec_noalloc_partials));
+        if (!p) return fail(DMRGK_ECUDA, "vec_multi_dot_noalloc: cudaGetSymbolAddress returned NULL");
+        g_noalloc_ptr[device] = p;
+    }
+    *out = g_noalloc_ptr[device];
+    return DMRGK_OK;
+}
+
+int32_t dmrgk_vec_multi_dot_noalloc(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double* X_dev, int64_t stride,
+                                    const double* y_dev, double* out_dev, void* stream) {
+    DMRGK_TRY(check_vec("vec_multi_dot_noalloc", ctx, n));
+    if (nv < 0) return fail(DMRGK_EINVAL, "vec_multi_dot_noalloc: nv < 0");
+    if (nv > DMRGK_NOALLOC_MAX_NV)
+        return fail(DMRGK_EINVAL, "vec_multi_dot_noalloc: nv = %d exceeds the built-in scratch (at most %d vectors per "
+                                  "call; use dmrgk_vec_multi_dot with your own scratch, or split the call)",
+                    nv, DMRGK_NOALLOC_MAX_NV);
+    if (ctx->device < 0 || ctx->device >= DMRGK_NOALLOC_MAX_DEVICES)
+        return fail(DMRGK_EINVAL, "vec_multi_dot_noalloc: device %d outside [0, %d)", ctx->device, DMRGK_NOALLOC_MAX_DEVICES);
+    if (nv == 0) return DMRGK_OK;
+    if (!X_dev || !y_dev || !out_dev) return fail(DMRGK_EINVAL, "vec_multi_dot_noalloc: NULL pointer");
+    if (stride & 1) return fail(DMRGK_EINVAL, "vec_multi_dot_noalloc: stride must be even");
+    if (!aligned128(X_dev) || !aligned128(y_dev) || (stride & 15))
+        return fail(DMRGK_EALIGN, "vec_multi_dot_noalloc: vectors must be 128-byte aligned (stride a multiple of 16)");
+    DMRGK_CUDA(cudaSetDevice(ctx->device));
+    double* partial = nullptr;
+    DMRGK_TRY(noalloc_partials(ctx->device, &partial));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t n2 = n / 2;
+    const int grid = vec_grid(n2);
     for (int j0 = 0; j0 < nv; j0 += 8) {
         const int c = std::min(8, nv - j0);
         if (c == 1) launch_dot1<1>(grid, st, n2, c, j0, X_dev, stride, y_dev, partial, nv);

@@ -95,6 +95,7 @@ SIGNATURES = {
     "dmrgk_enlarge_apply": (_i32, [_p, _p]),
     "dmrgk_vec_scratch_bytes": (_i64, [_i32]),
     "dmrgk_vec_multi_dot": (_i32, [_p, _i64, _i32, _p, _i64, _p, _p, _p, _p]),
+    "dmrgk_vec_multi_dot_noalloc": (_i32, [_p, _i64, _i32, _p, _i64, _p, _p, _p]),
     "dmrgk_vec_multi_axpy": (_i32, [_p, _i64, _i32, _p, _i64, _p, _f64, _f64, _p, _p]),
     "dmrgk_vec_axpby": (_i32, [_p, _i64, _f64, _p, _f64, _p, _p]),
     "dmrgk_vec_dot": (_i32, [_p, _i64, _p, _p, _p, _p, _p]),
@@ -583,6 +584,14 @@ def vec_scratch_bytes(nv):
 
 def vec_multi_dot(ctx, n, nv, X, stride, y, out, scratch, stream=None):
     check(ctx.lib.dmrgk_vec_multi_dot(ctx.h, n, nv, _dev(X), stride, _dev(y), _dev(out), _dev(scratch), _stream(stream)))
+
+
+def vec_multi_dot_noalloc(ctx, n, nv, X, stride, y, out, stream=None):
+    """vec_multi_dot without the scratch tensor, for callers that cannot allocate device memory (HBM already
+    full of operators, no allocator of their own, or a cudaMalloc would stall the overlapped operator copies):
+    the partial sums use a fixed array inside libdmrgk.so.  nv ≤ 64; one array per GPU, so calls that may
+    overlap on the GPU race; make the first call on a device before any stream capture (include/dmrgk.h)."""
+    check(ctx.lib.dmrgk_vec_multi_dot_noalloc(ctx.h, n, nv, _dev(X), stride, _dev(y), _dev(out), _stream(stream)))
 
 
 def vec_multi_axpy(ctx, n, nv, X, stride, coef, alpha, beta, y, stream=None):
