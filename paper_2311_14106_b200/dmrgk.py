@@ -555,13 +555,31 @@ class Davidson:
         return m.value, na.value
 
     def set_allreduce(self, fn):
-        """fn(device pointer, n doubles) -> 0: called after every apply of the driver (k-sharding hook)."""
+        """fn(device pointer, n doubles) -> 0: called after every apply of the driver (k-sharding hook), with
+        the solver's main stream made torch's current stream for the duration of the call.  A non-zero return
+        or an exception in fn makes the driver fail with ESTATE."""
         if fn is None:
             self._reduce_cb = None
             check(self.lib.dmrgk_davidson_set_allreduce(self.h, None, None))
             return
         proto = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)
-        self._reduce_cb = proto(lambda ptr, n, stream, user: int(fn(int(ptr), int(n))))
+
+        def trampoline(ptr, n, stream, user):
+            # fn runs with the solver's main stream as torch's current stream, whatever stream the caller
+            # has made current since: a collective issued by fn is then ordered after the apply that wrote
+            # the vector.  An exception must not unwind through the C frames: it becomes a non-zero
+            # status, which the driver reports as DMRGK_ESTATE.
+            try:
+                import torch
+                s = torch.cuda.ExternalStream(int(stream)) if stream else torch.cuda.default_stream()
+                with torch.cuda.stream(s):
+                    return int(fn(int(ptr), int(n)))
+            except BaseException:          # noqa: BLE001 — nothing may propagate into ctypes
+                import traceback
+                traceback.print_exc()
+                return -1
+
+        self._reduce_cb = proto(trampoline)
         check(self.lib.dmrgk_davidson_set_allreduce(self.h, C.cast(self._reduce_cb, C.c_void_p), None))
 
     def __del__(self):

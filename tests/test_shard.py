@@ -134,3 +134,55 @@ def test_shards_applied_one_after_the_other_and_davidson_hook():
     dav.start(psi)
     theta, rn, n_apply, ok = dav.solve(None)
     assert ok and abs(theta - th_ref) <= 1e-9 * max(1.0, abs(th_ref))
+    # the same two results against the oracle (not only CUDA against CUDA): the summed σ against the
+    # per-task NumPy products of the full pair list, θ against the lowest eigenvalue of the dense H_eff
+    from _gpu import rel_max, TOL_SIGMA
+    prob = heff.problem_from_workload(wl)              # ψ from the host recipe (the device fill is pinned to it)
+    assert rel_max(full.to_blocks(total), heff.sigma_blockwise(prob)) <= TOL_SIGMA
+    H = heff.dense_heff(prob)
+    e0 = np.linalg.eigvalsh(H)[0]
+    assert abs(theta - e0) <= 1e-9 * max(1.0, abs(e0))
+
+
+@pytest.mark.gpu
+def test_allreduce_hook_runs_on_the_solver_stream_and_reports_failures():
+    """The hook's work must be ordered on the solver's main stream even when the caller has made another
+    stream current in the meantime (an NCCL all-reduce issued on the wrong stream would read W before the
+    apply has written it); a hook that raises, or returns non-zero, stops the driver with ESTATE."""
+    torch = pytest.importorskip("torch")
+    from paper_2311_14106_b200 import dmrgk, problem, shard
+    wl = _workload()
+    full = problem.from_workload(wl)
+    psi = full.psi_fill(wl.seed, wlmod.PSI_STREAM)
+    dav_ref = full.davidson(m_max=8, tol=1e-9, max_iter=400)
+    dav_ref.start(psi)
+    th_ref = dav_ref.solve(None)[0]
+    parts = [shard.ShardedProblem(wl, r, 2) for r in range(2)]
+    me, other = parts
+    dav = me.dp.davidson(m_max=8, tol=1e-9, max_iter=400, diag_hook=lambda d: d.add_(other.dp.diag()))
+    seen = []
+
+    def hook(ptr, n):
+        seen.append(torch.cuda.current_stream().cuda_stream)
+        W = me.dp.W
+        j = (ptr - W.data_ptr()) // (8 * n)
+        W[j * n:(j + 1) * n].add_(other.dp.apply(me.dp.V[j * n:(j + 1) * n]))
+        return 0
+
+    dav.set_allreduce(hook)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):                      # a foreign current stream while the driver runs
+        assert torch.cuda.current_stream().cuda_stream != me.dp.stream.cuda_stream
+        dav.start(psi)
+        theta, rn, n_apply, ok = dav.solve(None)
+    assert ok and abs(theta - th_ref) <= 1e-9 * max(1.0, abs(th_ref))
+    assert seen and all(s == me.dp.stream.cuda_stream for s in seen)
+
+    def bad(ptr, n):
+        raise RuntimeError("boom")
+
+    for fn in (bad, lambda ptr, n: 3):
+        dav.set_allreduce(fn)
+        with pytest.raises(dmrgk.DmrgkError) as e:
+            dav.start(psi)
+        assert e.value.status == dmrgk.ESTATE
