@@ -263,7 +263,8 @@ int32_t dmrgk_vec_multi_axpy(dmrgk_ctx* ctx, int64_t n, int32_t nv, const double
 int32_t dmrgk_vec_axpby(dmrgk_ctx* ctx, int64_t n, double alpha, const double* x_dev, double beta,
                         double* y_dev, void* stream);
 /* y = f·x with f from a device scalar a = *alpha_dev: mode 0: f = a, 1: f = 1/a, 2: f = sqrt(a),
- * 3: f = 1/sqrt(a)  (normalisation by a squared norm without a host round trip).  y may alias x. */
+ * 3: f = 1/sqrt(a)  (normalisation by a squared norm without a host round trip).  y may alias x.
+ * In the inverse modes a = 0 gives f = 0, not Inf: a vector that vanished stays a zero vector. */
 int32_t dmrgk_vec_scal_dev(dmrgk_ctx* ctx, int64_t n, const double* alpha_dev, int32_t mode,
                            const double* x_dev, double* y_dev, void* stream);
 /* out[0] = x·y ;  out[0] = ‖x‖₂ ;  y += alpha·x ;  x *= alpha  (host scalars; dot / nrm2 results land in
@@ -304,7 +305,11 @@ int32_t dmrgk_davidson_step(dmrgk_davidson* d, double* theta, double* resnorm, i
  * Returns DMRGK_ENOTCONV (θ and x still written) when max_iter is reached. */
 int32_t dmrgk_davidson_solve(dmrgk_davidson* d, double* theta, double* resnorm, double* x_dev,
                              int32_t* n_apply);
-/* Current subspace size m. */
+/* Current subspace size m, and the number of H_eff applies run since davidson_start (the start's own
+ * included).  A step runs exactly one apply, except when the preconditioned correction vanishes after
+ * orthogonalisation (it lies in the span of the basis — e.g. an exactly diagonal H_eff): that is only
+ * known when ‖t‖² comes back with the Rayleigh entries, so the step then redoes the new basis vector from
+ * the residual and has run two. */
 int32_t dmrgk_davidson_query(const dmrgk_davidson* d, int32_t* m, int32_t* n_apply);
 /* Multi-GPU k-sharding hook (the sum over operator pairs
  * is split over the GPUs, ψ is replicated, σ is the sum of the ranks' partial results).  When set, fn

@@ -261,8 +261,9 @@ int32_t dmrgk_davidson_step(dmrgk_davidson* d, double* theta, double* resnorm, i
     DMRGK_TRY(dmrgk_vec_scal_dev(d->ctx, d->n, tt_dev, 3, d->t, v, d->main));
     DMRGK_TRY(apply_h(d, v, w));
     DMRGK_TRY(extend_G(d));
-    if (!(std::sqrt(d->host[64 + TT_SLOT]) >= 1e-14 * d->rho)) {   // correction vanished: fall back to the residual
-        d->n_apply -= 1;
+    // correction vanished: fall back to the residual.  The apply above was wasted on a zero or noise vector
+    // (finite: the scaling kernel maps 1/0 to 0) and stays counted in n_apply — the count is of applies run.
+    if (!(std::sqrt(d->host[64 + TT_SLOT]) >= 1e-14 * d->rho)) {
         DMRGK_CUDA(cudaMemcpyAsync(d->t, d->r, size_t(d->n) * 8, cudaMemcpyDeviceToDevice, d->main));
         DMRGK_TRY(orthogonalise(d, d->t));
         DMRGK_TRY(dmrgk_vec_multi_dot(d->ctx, d->n, 1, d->t, d->n, d->t, tt_dev, d->scratch, d->main));

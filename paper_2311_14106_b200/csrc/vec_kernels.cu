@@ -134,7 +134,7 @@ scal_dev_kernel(int64_t n2, const double* __restrict__ alpha_dev, int inv, int s
                 const double2* __restrict__ x, double2* __restrict__ y) {
     double a = *alpha_dev;
     if (sqrt_first) a = sqrt(a);
-    const double f = inv ? 1.0 / a : a;
+    const double f = inv ? (a != 0.0 ? 1.0 / a : 0.0) : a;   // 1/0 → 0: a vanished vector stays a zero vector, never Inf/NaN
     for (int64_t i = int64_t(blockIdx.x) * VEC_THREADS + threadIdx.x; i < n2;
          i += int64_t(gridDim.x) * VEC_THREADS) {
         double2 v = x[i];
