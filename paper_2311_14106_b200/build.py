@@ -104,8 +104,30 @@ def built_hash():
 
 def build(force=False, verbose=False):
     """Compile and link; returns the path of libdmrgk.so.  Raises on any compiler error.  An object is
-    recompiled when the hash of its source, the headers and the flags differs from its stamp."""
+    recompiled when the hash of its source, the headers and the flags differs from its stamp.
+
+    Safe to call from several processes at once (every rank of a torchrun job, parallel test workers):
+    the whole build runs under an exclusive lock on _build/.lock, so the later callers wait and then find
+    the stamps up to date; objects and the library are written under temporary names and renamed into
+    place, so a process that dlopens the library meanwhile sees the old file or the new one, never half."""
+    import fcntl
     os.makedirs(OUT, exist_ok=True)
+    with open(os.path.join(OUT, ".lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            return _build_locked(force, verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _write_stamp(path, value):
+    tmp = f"{path}.hash.tmp{os.getpid()}"
+    with open(tmp, "w") as f:
+        f.write(value)
+    os.replace(tmp, path + ".hash")
+
+
+def _build_locked(force, verbose):
     nvcc = _nvcc()
     srcs = sources()
     ghash = source_hash()
@@ -117,12 +139,15 @@ def build(force=False, verbose=False):
         if not force and os.path.exists(obj) and _stamp(obj) == want:
             return None
         extra = [f'-DDMRGK_SOURCE_HASH="{ghash}"'] if os.path.basename(src) == VERSION_SOURCE else []
-        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+        tmp = f"{obj}.tmp{os.getpid()}.o"
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", tmp]
         p = subprocess.run(cmd, capture_output=True, text=True)
         if p.returncode != 0:
+            if os.path.exists(tmp):
+                os.remove(tmp)
             raise RuntimeError(f"nvcc failed on {src}:\n{p.stdout}\n{p.stderr}")
-        with open(obj + ".hash", "w") as f:
-            f.write(want)
+        os.replace(tmp, obj)
+        _write_stamp(obj, want)
         return p.stderr if verbose else "compiled"
 
     with ThreadPoolExecutor(max_workers=min(8, len(srcs))) as ex:
@@ -132,12 +157,15 @@ def build(force=False, verbose=False):
             if lg:
                 print(f"--- {os.path.basename(s)}\n{lg}")
     if force or any(logs) or built_hash() != ghash:
-        cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs
+        tmp = f"{LIB}.tmp{os.getpid()}.so"
+        cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs
         p = subprocess.run(cmd, capture_output=True, text=True)
         if p.returncode != 0:
+            if os.path.exists(tmp):
+                os.remove(tmp)
             raise RuntimeError(f"link failed:\n{p.stdout}\n{p.stderr}")
-        with open(LIB + ".hash", "w") as f:
-            f.write(ghash)
+        os.replace(tmp, LIB)
+        _write_stamp(LIB, ghash)
     return LIB
 
 

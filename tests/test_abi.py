@@ -102,3 +102,26 @@ def test_balanced_tile_plan_host_rules():
     assert dmrgk.plan_tile_cost(128, 64) == 128 and dmrgk.plan_tile_cost(8, 8) == dmrgk.plan_tile_cost(1, 1) == 24   # the floor
     with pytest.raises(dmrgk.DmrgkError):
         dmrgk.plan_tile_cuts(10, 32)
+
+
+def test_build_is_serialised_by_a_file_lock():
+    """Several processes may call build() at once (torchrun ranks, parallel test workers): it runs under an
+    exclusive lock on _build/.lock.  While this process holds that lock a second process's build() waits; once
+    released it returns the library path (nothing to recompile: the stamps are current)."""
+    import fcntl
+    import subprocess
+    import sys
+    import time
+    from paper_2311_14106_b200 import build as b
+    b.build()
+    with open(os.path.join(b.OUT, ".lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        p = subprocess.Popen([sys.executable, "-c", "from paper_2311_14106_b200 import build as b; print(b.build())"],
+                             cwd=ROOT, stdout=subprocess.PIPE, text=True)
+        time.sleep(3.0)
+        assert p.poll() is None                     # still waiting for the lock
+        fcntl.flock(lock, fcntl.LOCK_UN)
+    out, _ = p.communicate(timeout=120)
+    assert p.returncode == 0 and out.strip().endswith("libdmrgk.so")
+    assert b.built_hash() == b.source_hash()
+    assert not [f for f in os.listdir(b.OUT) if ".tmp" in f]
