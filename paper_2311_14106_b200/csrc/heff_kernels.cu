@@ -611,14 +611,22 @@ static int32_t setup_kernel(K* fn, int threads, int smem, int min_ctas, int* res
     return DMRGK_OK;
 }
 
+// Set up at context creation.  Only the product variants (0 and its eager-claim twin 5) are required: a
+// measurement variant that misses its residency target on some device is recorded as unavailable and
+// refused where it is asked for (gemm_kernel_available), it does not take the whole library down.
+static bool g_variant_ok[6] = {false, true, false, false, false, false};   // 1 = scalar check kernel, no set-up needed
+
 int32_t gemm_kernel_setup() {
     DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3, LATE>, P_NTHREADS, smem_bytes(4, ST64), 3, &g_gemm_ctas_per_sm));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST96, 2, LATE>, P_NTHREADS, smem_bytes(4, ST96), 2, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 2, LATE>, P_NTHREADS, smem_bytes(4, ST64), 2, nullptr));
-    DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<8, ST96T, 2, LATE>, P_NTHREADS, smem_bytes(8, ST96T), 2, nullptr));
     DMRGK_TRY(setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 3, EAGER>, P_NTHREADS, smem_bytes(4, ST64), 3, nullptr));
+    g_variant_ok[0] = g_variant_ok[5] = true;
+    g_variant_ok[2] = setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST96, 2, LATE>, P_NTHREADS, smem_bytes(4, ST96), 2, nullptr) == DMRGK_OK;
+    g_variant_ok[3] = setup_kernel(heff_gemm_dmma_persistent_kernel<4, ST64, 2, LATE>, P_NTHREADS, smem_bytes(4, ST64), 2, nullptr) == DMRGK_OK;
+    g_variant_ok[4] = setup_kernel(heff_gemm_dmma_persistent_kernel<8, ST96T, 2, LATE>, P_NTHREADS, smem_bytes(8, ST96T), 2, nullptr) == DMRGK_OK;
     return DMRGK_OK;
 }
+
+bool gemm_kernel_available(int kernel) { return kernel >= 0 && kernel <= 5 && g_variant_ok[kernel]; }
 
 int gemm_tile_m(int kernel) { return kernel == 4 ? 128 : 64; }
 int gemm_ctas(int kernel) { return (kernel == 0 || kernel == 1 || kernel == 5) ? 3 : 2; }

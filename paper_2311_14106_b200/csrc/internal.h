@@ -224,6 +224,7 @@ static inline int64_t tile_cost(int rows, int cols) {
 // kernel launchers (heff_kernels.cu)
 // `counter_dev`: a zeroed int the persistent kernel uses as its unit queue head (one per launch in flight)
 // `short_units`: the launch's units average fewer k-tiles than the late look-ahead needs (variant 0 then claims eagerly)
+bool gemm_kernel_available(int kernel);   // false for a measurement variant whose residency target this device misses
 int32_t launch_gemm_units(int kernel, const Unit* units_dev, const Seg* segs_dev, int64_t n_units,
                           const Bases& bases, cudaStream_t st, int* counter_dev, int n_sm, bool short_units);
 constexpr int SHORT_UNIT_TILES = 8;   // = the late look-ahead of the GEMM kernel, in k-tiles

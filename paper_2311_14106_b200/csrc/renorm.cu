@@ -65,6 +65,8 @@ int32_t dmrgk_renorm_create(dmrgk_ctx* ctx, const dmrgk_iso* phi, int64_t n_ops,
     if (opts) o = *opts;
     const bool default_chunk = o.t_chunk_bytes <= 0;
     if (o.kernel < 0 || o.kernel > 5) return fail(DMRGK_EINVAL, "renorm_create: bad options");
+    if (!gemm_kernel_available(o.kernel))
+        return fail(DMRGK_EINVAL, "renorm_create: kernel variant %d is not resident on this device (use 0)", o.kernel);
     for (int64_t i = 0; i < n_ops; ++i) {
         if (!in[i] || !out[i]) return fail(DMRGK_EINVAL, "renorm_create: operator %lld is NULL", (long long)i);
         if (in[i]->space != phi->enl) return fail(DMRGK_ESHAPE, "renorm_create: in[%lld] is not on phi's enlarged space", (long long)i);

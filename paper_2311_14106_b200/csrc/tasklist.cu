@@ -130,6 +130,8 @@ int32_t dmrgk_heff_create_blockcoef(dmrgk_ctx* ctx, const dmrgk_layout* layout, 
     if (o.ring_bytes < 0 || (o.kernel < 0 || o.kernel > 5) || o.order_policy < 0 || o.order_policy > 2 ||
         (o.per_pair_output != 0 && o.per_pair_output != 1))
         return fail(DMRGK_EINVAL, "heff_create: bad options");
+    if (!gemm_kernel_available(o.kernel))
+        return fail(DMRGK_EINVAL, "heff_create: kernel variant %d is not resident on this device (use 0)", o.kernel);
     const int64_t ring_part = (o.ring_bytes / 3) / 128 * 128;   // three parts: see dmrgk_heff_apply
 
     const dmrgk_space *SA = layout->A, *SB = layout->B;

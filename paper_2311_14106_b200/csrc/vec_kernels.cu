@@ -129,9 +129,21 @@ axpby_kernel(int64_t n2, double alpha, const double2* __restrict__ x, double bet
     }
 }
 
+// x = alpha·x in place (one pointer: the two-pointer kernels above promise __restrict__)
+__global__ void __launch_bounds__(VEC_THREADS)
+scal_kernel(int64_t n2, double alpha, double2* x) {
+    for (int64_t i = int64_t(blockIdx.x) * VEC_THREADS + threadIdx.x; i < n2;
+         i += int64_t(gridDim.x) * VEC_THREADS) {
+        double2 v = x[i];
+        v.x *= alpha;
+        v.y *= alpha;
+        x[i] = v;
+    }
+}
+
 __global__ void __launch_bounds__(VEC_THREADS)
 scal_dev_kernel(int64_t n2, const double* __restrict__ alpha_dev, int inv, int sqrt_first,
-                const double2* __restrict__ x, double2* __restrict__ y) {
+                const double2* x, double2* y) {      // y may alias x (in-place normalisation): no __restrict__
     double a = *alpha_dev;
     if (sqrt_first) a = sqrt(a);
     const double f = inv ? (a != 0.0 ? 1.0 / a : 0.0) : a;   // 1/0 → 0: a vanished vector stays a zero vector, never Inf/NaN
@@ -425,7 +437,16 @@ int32_t dmrgk_vec_axpy(dmrgk_ctx* ctx, int64_t n, double alpha, const double* x_
 }
 
 int32_t dmrgk_vec_scal(dmrgk_ctx* ctx, int64_t n, double alpha, double* x_dev, void* stream) {
-    return dmrgk_vec_axpby(ctx, n, alpha, x_dev, 0.0, x_dev, stream);   // x = alpha·x + 0·x, element by element
+    DMRGK_TRY(check_vec("vec_scal", ctx, n));
+    if (n == 0) return DMRGK_OK;
+    if (!x_dev) return fail(DMRGK_EINVAL, "vec_scal: NULL pointer");
+    if (!aligned128(x_dev)) return fail(DMRGK_EALIGN, "vec_scal: vector must be 128-byte aligned");
+    DMRGK_CUDA(cudaSetDevice(ctx->device));
+    const int64_t n2 = n / 2;
+    scal_kernel<<<vec_grid(n2), VEC_THREADS, 0, (cudaStream_t)stream>>>(n2, alpha, reinterpret_cast<double2*>(x_dev));
+    count_launch();
+    DMRGK_CUDA(cudaGetLastError());
+    return DMRGK_OK;
 }
 
 }  // extern "C"
