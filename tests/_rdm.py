@@ -48,3 +48,86 @@ def rdm_fock(d, space, x):
     psi[d.rows] = dmrg.projector(space, d.rows) @ x
     cpsi = [ci @ psi for ci in c]
     return np.array([[float(cpsi[i] @ cpsi[j]) for j in range(n)] for i in range(n)])
+
+
+# ---- two-particle reduced density matrix ("one- and two-body reduced density matrices";
+#      the two-mode entropies of the mode optimisation need it) ----
+def split_string(string, n_A):
+    """A product of creators / annihilators  o_1 o_2 … o_m  (``string`` = [(mode, dagger)], modes of A are
+    < n_A) rewritten as  sign · (A-operators in their order) · (B-operators in their order).
+
+    Operators on different modes anticommute, so every B-operator that stands left of an A-operator costs
+    one factor −1 when the A-operator is moved past it.  With the halves' own Jordan–Wigner strings
+     the reordered product is  (Ã · P_A^π) ⊗ B̃ ,  π = number of B-operators mod 2."""
+    sign, seen_B = 1.0, 0
+    part_A, part_B = [], []
+    for mode, dagger in string:
+        if mode < n_A:
+            part_A.append((mode, dagger))
+            if seen_B & 1:
+                sign = -sign
+        else:
+            part_B.append((mode - n_A, dagger))
+            seen_B += 1
+    return sign, part_A, part_B
+
+
+def string_pairs(d, space, strings):
+    """(Problem without ψ, kept) for a list of operator strings: one operator pair per string that conserves
+    the charges (the others have expectation value 0 by symmetry and get no pair); ``kept`` = their indices."""
+    n_A, n_B = space.A.n_modes, space.B.n_modes
+    a, b = fock.annihilators(n_A), fock.annihilators(n_B)
+    mc = d.mc
+    nc = mc.shape[1]
+    PhiA, PhiB = space.A.Phi, space.B.Phi
+    pb = Problem(nc, list(space.sectors_A), list(space.sectors_B), tuple(space.target), name="strings")
+    kept = []
+
+    def shift(part, offset):
+        dq = [0] * nc
+        for mode, dagger in part:
+            for c in range(nc):
+                dq[c] += int(mc[mode + offset][c]) * (1 if dagger else -1)
+        return tuple(dq)
+
+    def product(part, ann):
+        M = np.eye(ann[0].shape[0])
+        for mode, dagger in part:
+            M = M @ (ann[mode].T if dagger else ann[mode])
+        return M
+
+    def add_op(half, part, parity):
+        Phi, sectors, ann, off = (PhiA, space.sectors_A, a, 0) if half == "A" else (PhiB, space.sectors_B, b, n_A)
+        dq = shift(part, off)
+        pb.ops.append({"half": half, "dq": dq, "parity": parity,
+                       "blocks": _cut_blocks(Phi.T @ (product(part, ann) @ Phi), sectors, dq)})
+        return len(pb.ops) - 1
+
+    for idx, string in enumerate(strings):
+        sign, part_A, part_B = split_string(string, n_A)
+        if any(x + y != 0 for x, y in zip(shift(part_A, 0), shift(part_B, n_A))):
+            continue
+        parity = len(part_B) & 1
+        assert (len(part_A) & 1) == parity       # charge conservation makes both halves odd or both even
+        L = add_op("A", part_A, parity) if part_A else None
+        R = add_op("B", part_B, parity) if part_B else None
+        pb.terms.append((L, R, sign, False, False))
+        kept.append(idx)
+    return pb, kept
+
+
+def rdm2_strings(n):
+    """Labels (i, j, k, l), i < j, k < l, and the strings c†_i c†_j c_k c_l of Γ_ijkl = ⟨c†_i c†_j c_k c_l⟩;
+    the other elements follow from Γ_ijkl = −Γ_jikl = −Γ_ijlk."""
+    pairs = [(i, j) for i in range(n) for j in range(i + 1, n)]
+    labels = [(i, j, k, l) for (i, j) in pairs for (k, l) in pairs]
+    return labels, [[(i, True), (j, True), (k, False), (l, False)] for (i, j, k, l) in labels]
+
+
+def rdm2_fock(d, space, x, labels):
+    """Γ_ijkl = ⟨Ψ| c†_i c†_j c_k c_l |Ψ⟩ with Ψ = P x in the full Fock space (the definition), per label."""
+    n = d.n
+    c = fock.annihilators(n)
+    psi = np.zeros(2 ** n)
+    psi[d.rows] = dmrg.projector(space, d.rows) @ x
+    return np.array([float(psi @ (c[i].T @ (c[j].T @ (c[k] @ (c[l] @ psi))))) for (i, j, k, l) in labels])

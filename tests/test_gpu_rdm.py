@@ -57,3 +57,32 @@ def test_one_particle_rdm_of_a_dmrg_bond(make, bond, N):
     for (i, j), v in zip(labels, got):
         assert abs(v - gamma[i, j]) <= 1e-11, (i, j)
     assert abs(sum(v for (i, j), v in zip(labels, got) if i == j) - N) <= 1e-11
+
+
+@pytest.mark.parametrize("make,bond,N", [(spinless_3x3(64), 4, 4), (spinless_3x3(6), 3, 4), (hubbard_ring(8), 1, 4)])
+def test_two_particle_rdm_of_a_dmrg_bond(make, bond, N):
+    """Γ_ijkl = ⟨c†_i c†_j c_k c_l⟩, i < j, k < l (the two-mode quantities of PAPER.md:88), through
+    dmrgk_heff_expect on the pair list of the strings split across the cut — one pair per charge-conserving
+    string, reordering sign as the coefficient — against the Fock-space definition at 1e-11, plus the partial
+    trace Σ_j Γ_ijjk = (N − 1) γ_ik against the Fock-space one-particle matrix."""
+    from _rdm import rdm2_strings, rdm2_fock, string_pairs
+    T, V, mc, site_modes, target, D = make
+    d = dmrg.SimpleDMRG(T, V, mc, site_modes, target, D=D, seed=2)
+    d.warmup_to(bond)
+    space = d.space_at(bond)
+    Heff, P = d.heff_at(space)
+    E, x = dmrg.lowest_eigenpair(Heff)
+    labels, strings = rdm2_strings(d.n)
+    pb, kept = string_pairs(d, space, strings)
+    pb.psi = dmrg.vec_to_blocks(space, x)
+    dp = device_problem(pb, per_pair_output=1)
+    got = dp.expect(dp.psi_from_host(pb.psi), len(pb.terms)).cpu().numpy()
+    ref = rdm2_fock(d, space, x, labels)
+    assert np.abs(got - ref[kept]).max() <= 1e-11
+    assert np.abs(got - heff.expectation_per_pair(pb)).max() <= 1e-11
+    n = d.n
+    G = np.zeros((n, n, n, n))
+    for idx, v in zip(kept, got):
+        i, j, k, l = labels[idx]
+        G[i, j, k, l], G[j, i, k, l], G[i, j, l, k], G[j, i, l, k] = v, -v, -v, v
+    assert np.abs(np.einsum("ijjk->ik", G) - (N - 1) * rdm_fock(d, space, x)).max() <= 1e-10
