@@ -27,8 +27,8 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "heff_apply_fp64_tflops_in_davidson_step"
-SAMPLE_EVERY = {"4": 100, "3": 100, "3b": 268, "2": 8, "5": 143, "5r": 143, "4rs": 2}   # --impl reference: every n-th operator pair (host-generated values)
-CPU_EVERY = {"4": 20, "3": 20, "3b": 40, "2": 4, "5": 20, "5r": 20, "4rs": 1}              # cpu_baseline leg: ≈ 5 % of the pairs (values read back D2H)
+SAMPLE_EVERY = {"4": 100, "3": 100, "3b": 268, "2": 8, "5": 143, "5r": 143, "4rs": 2, "1": 1}   # --impl reference: every n-th operator pair (host-generated values)
+CPU_EVERY = {"4": 20, "3": 20, "3b": 40, "2": 4, "5": 20, "5r": 20, "4rs": 1, "1": 1}              # cpu_baseline leg: ≈ 5 % of the pairs (values read back D2H)
 UNIT = "TFLOP/s"
 
 
@@ -46,6 +46,11 @@ def make_workload(name):
         return wlmod.config5()      # executed subset; "5": part of it streamed from pinned host memory, "5r": all resident
     if name == "2":
         return wlmod.synthetic_config2()
+    if name == "1":
+        # configs[0]'s SHAPE ("latency only"): 4×4 spinless torus cut 8|8, D = 64 (M = 128), the dense
+        # mode-rotated term list (K = 154), seeded values.  The operators of the real bond come out of a DMRG sweep, which
+        # only the oracle has (tests/_gpu.config1_problem is that parity case); the timing needs the shape, not the state.
+        return wlmod.lattice_workload("spinless", 8, 128, seed=1, name="config1_shape_spinless4x4_rotated_K154_D64")
     raise SystemExit(f"unknown --config {name}")
 
 
@@ -287,7 +292,9 @@ def davidson_bench(dp, wl, args, world, local, steps, warmup, make_davidson=None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(dp.stream)
+    m_seen = []
     for _ in range(steps):
+        m_seen.append(dav.query()[0])
         theta, rho, _ = dav.step()
     e1.record(dp.stream)
     barrier()
@@ -298,10 +305,94 @@ def davidson_bench(dp, wl, args, world, local, steps, warmup, make_davidson=None
     clk = clocks.stop()
     ms_total = max_over_ranks(ms_total, world, "cuda")
     return {"psi": psi, "ms_step": ms_total / steps, "launches": int(launches), "prof_ms": prof_ms, "prof_n": prof_n,
-            "clocks": clk, "theta": theta, "rho": rho}
+            "clocks": clk, "theta": theta, "rho": rho, "m_range": [min(m_seen), max(m_seen)] if m_seen else None}
+
+
+EXTRA_ROWS = [   # (key, bench.py arguments): the other workloads DESIGN.md quotes, each run as its own process
+    ("config1", ["--config", "1", "--steps", "20", "--warmup", "5", "--no-extras"]),
+    ("config3b", ["--config", "3b", "--steps", "3", "--warmup", "3", "--no-cpu", "--no-extras"]),
+    ("config4rs", ["--config", "4rs", "--steps", "5", "--warmup", "3", "--no-cpu", "--no-extras"]),
+    ("config5r", ["--config", "5r", "--steps", "3", "--warmup", "3", "--no-cpu", "--no-extras"]),
+    ("config5", ["--config", "5", "--steps", "3", "--warmup", "3", "--no-cpu", "--no-extras"]),
+    ("su2", ["--op", "su2", "--steps", "3", "--warmup", "3"]),
+    ("expect", ["--op", "expect", "--steps", "3", "--warmup", "2"]),
+    ("enlarge", ["--op", "enlarge", "--steps", "10", "--warmup", "3"]),
+]
+
+
+def brief(line):
+    """The fields of a bench line that an extras row keeps."""
+    cfg, roof = line.get("config", {}), line.get("roofline", {})
+    row = {"metric": line.get("metric"), "value": line.get("value"), "unit": line.get("unit"), "workload": cfg.get("workload"),
+           "ms_per_step": line.get("ms_per_step"), "steps": line.get("steps"), "warmup": line.get("warmup"),
+           "gpu_launches": line.get("gpu_launches"),
+           "roofline": {k: roof.get(k) for k in ("bound", "achieved", "peak", "unit", "frac", "frac_of_cublas_dgemm") if k in roof},
+           "clocks": line.get("clocks")}
+    for k in ("apply_burst", "cpu_baseline"):
+        if k in line:
+            row[k] = line[k]
+    if "e2e" in line:
+        row["e2e_value"] = line["e2e"].get("value")
+    for k in ("K_pairs", "tasks", "flops_alg_per_apply", "staged_ops", "staged_bytes_per_apply", "op_bytes_resident",
+              "davidson_m_of_timed_steps", "pairs_per_second", "tiles", "kept_bytes", "formed_bytes"):
+        if k in cfg:
+            row[k] = cfg[k]
+    return row
+
+
+def extra_rows_in_subprocesses():
+    """Every other row the documents quote, measured in the same driver run: one `python bench.py …` process per row,
+    started after the headline workload's device memory has been released (the rows need up to 150 GB themselves).
+    A row that fails, times out or runs out of memory records its error; it cannot touch the headline numbers."""
+    import gc
+    import subprocess
+    import torch
+    gc.collect()
+    torch.cuda.empty_cache()
+    free, total = torch.cuda.mem_get_info()
+    rows = {"device_free_bytes_before_rows": int(free), "how": "python bench.py <args> per row, one process each, one after the other"}
+    for key, argv in EXTRA_ROWS:
+        t0 = time.perf_counter()
+        try:
+            p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py")] + argv, cwd=ROOT, capture_output=True,
+                               text=True, timeout=900)
+            lines = [ln for ln in p.stdout.splitlines() if ln.startswith("{")]
+            if p.returncode != 0 or not lines:
+                rows[key] = {"error": f"rc {p.returncode}: {(p.stderr or p.stdout)[-300:]}"}
+            else:
+                rows[key] = brief(json.loads(lines[-1]))
+                rows[key]["args"] = " ".join(argv)
+        except Exception as exc:
+            rows[key] = {"error": repr(exc)[:300]}
+        rows[key]["wall_s"] = round(time.perf_counter() - t0, 1)
+    a, b_ = rows.get("config5"), rows.get("config5r")
+    if a and b_ and "ms_per_step" in a and "ms_per_step" in b_:   # row a3: what the staging costs, and the PCIe rate it sustains
+        a["exposed_copy_ms_per_step"] = a["ms_per_step"] - b_["ms_per_step"]
+        if a.get("staged_bytes_per_apply"):
+            a["h2d_gbs_over_the_step"] = a["staged_bytes_per_apply"] / a["ms_per_step"] / 1e6
+    return rows
 
 
 def run_ours(args):
+    import torch
+    out = measure_ours(args)      # every device buffer of the headline workload dies with that frame
+    if out is None:
+        return
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank == 0 and world == 1 and not args.no_extras and args.config == "4":
+        try:
+            out.setdefault("extras", {}).update(extra_rows_in_subprocesses())
+        except Exception as exc:
+            out.setdefault("extras", {})["rows_error"] = repr(exc)[:300]
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def measure_ours(args):
     import torch
     import torch.distributed as dist
     import workloads as wlmod
@@ -324,7 +415,8 @@ def run_ours(args):
 
     wl = make_workload(args.config)
     if args.shard == "k" and world > 1:
-        return run_sharded(args, wl, rank, world, local)
+        run_sharded(args, wl, rank, world, local)
+        return None
     staged = wlmod.config5_staged_ops(wl) if args.config == "5" else []
     opts = {"ring_bytes": 6 << 30} if staged else {}
     if args.kernel:
@@ -408,7 +500,10 @@ def run_ours(args):
         "config": {"workload": wl.name, "M_A": wl.M_A, "M_B": wl.M_B, "K_pairs": len(wl.terms), "tasks": h.n_tasks,
                    "flops_alg_per_apply": h.flops_alg, "flops_exec_over_alg": h.flops_exec / h.flops_alg if h.flops_alg else None,
                    "op_bytes_resident": int(dp.op_arena.numel() * 8),
-                   "psi_elems": dp.layout.n_elems, "davidson_m_max": args.m_max, "parallelism": "replicas only",
+                   "psi_elems": dp.layout.n_elems, "davidson_m_max": args.m_max,
+                   "davidson_m_of_timed_steps": r["m_range"], "davidson_m_what": "subspace size at the start of the timed steps, [min, max]: "
+                   "m grows by one per step and collapses to 1 at m_max, so the vector-kernel share of a step varies with it",
+                   "parallelism": "replicas only",
                    "l2": "operator arena (>> 126 MB L2) is streamed once per step; no flush needed",
                    "setup_s": {"tables": round(su["structures"] + su["tasklist"], 3), "tables_what": "sector/block tables + "
                                "task-list build and upload (the paper's 'Tables', PAPER.md:142)", "seeded_fill": round(su["fill"], 3),
@@ -429,6 +524,9 @@ def run_ours(args):
                      "peak_measured": peak_measured,
                      "frac_of_measured": (achieved / peak_measured) if achieved else None,
                      "peak_measured_source": "best sustained ceiling measured in this run: register-only DMMA loop (two shapes), DFMA loop, cuBLAS DGEMM 8192^3",
+                     "peak_cublas_dgemm": ceil["dgemm_8192"]["sustained_tflops"],
+                     "frac_of_cublas_dgemm": (achieved / ceil["dgemm_8192"]["sustained_tflops"]) if achieved else None,
+                     "peak_cublas_dgemm_source": "cuBLAS DGEMM 8192^3 sustained in this run (a library-measured FP64 ceiling, not this repo's kernel)",
                      "probe_over_derived": probe_ratio,
                      "probe_agrees_with_derived": bool(abs(probe_ratio - 1.0) <= 0.03),
                      "launches": int(gemm_n), "avg_launch_ms": gemm_ms / max(gemm_n, 1),
@@ -467,10 +565,7 @@ def run_ours(args):
         out["extras"] = extras
     if rank == 0 and world == 1 and not args.no_cpu:
         out["cpu_baseline"] = cpu_baseline_from_device(dp, wl, args)
-    if rank == 0:
-        print(json.dumps(out), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    return out
 
 
 def run_sharded(args, wl, rank, world, local):
@@ -533,7 +628,12 @@ def cpu_baseline_from_device(dp, wl, args, budget_s=25.0):
         oheff.sigma_blockwise(pb)
         reps += 1
     sec = (time.perf_counter() - t0) / reps
-    return {"value": fl / sec / 1e12, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+    tiers = {}
+    if args.config == "1":      # the oracle's wall time per σ, both tiers
+        t0 = time.perf_counter()
+        oheff.sigma_dense(pb)
+        tiers = {"oracle_t2_dense_kronecker_s": time.perf_counter() - t0, "oracle_t3_blockwise_s": sec}
+    return {**tiers, "value": fl / sec / 1e12, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
             "sample": f"oracle.heff.sigma_blockwise on every {every}th operator pair ({len(ids)} of {len(wl.terms)} = "
                       f"{100.0 * len(ids) / len(wl.terms):.1f} %), all ψ blocks, {fl:.3e} flop x {reps} repeats, "
                       "operator values read back from the device arena"}
@@ -881,7 +981,7 @@ def main():
     ap.add_argument("--steps", type=int, default=8)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="4", choices=["2", "3", "3b", "4", "4rs", "5", "5r"])
+    ap.add_argument("--config", default="4", choices=["1", "2", "3", "3b", "4", "4rs", "5", "5r"])
     ap.add_argument("--m-max", dest="m_max", type=int, default=16)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--kernel", type=int, default=0, choices=[0, 2, 3, 4, 5],
