@@ -803,42 +803,6 @@ def run_enlarge(args):
         "clocks": clk}), flush=True)
 
 
-def run_loop_probe(args):
-    """--op loop_probe: the k-tile-loop skeletons of csrc/probe_gemm.cu (harness, not the product path)
-    and the register-only pipe probes in all shapes — the ceilings design decisions are judged against."""
-    import torch
-    from paper_2311_14106_b200 import dmrgk
-    torch.cuda.set_device(0)
-    ctx = dmrgk.Ctx(0)
-    st = torch.cuda.current_stream()
-    buf = (torch.rand(1 << 23, dtype=torch.float64, device="cuda") - 0.5) * 1e-3      # 64 MiB, L2-resident
-    sink = torch.zeros(16, dtype=torch.float64, device="cuda")
-    out = {"op": "loop_probe", "source_hash": dmrgk.source_hash(), "n_sm": ctx.query()[0]}
-    cs = ClockSampler(0)
-    cs.start()
-    for kind, name in ((0, "cp.async 64x64 (round-1 loop)"), (1, "cp.async.bulk + mbarrier 64x64"),
-                       (2, "cp.async.bulk + mbarrier 128x64"), (3, "cp.async producer warp + mbarrier 128x64, 2 CTAs/SM"),
-                       (4, "cp.async.bulk + mbarrier 128x64, 2 CTAs/SM, 4 stages"), (5, "cp.async.bulk + mbarrier 64x64, 2 CTAs/SM")):
-        dmrgk.probe_gemm_loop(ctx, kind, 2000, buf, sink, st)
-        best = 0.0
-        for _ in range(5):
-            box = {}
-            ms = timed(st, lambda: box.setdefault("f", dmrgk.probe_gemm_loop(ctx, kind, 20000, buf, sink, st)))
-            best = max(best, box["f"] / ms / 1e9)
-        out[f"gemm_loop_kind{kind}"] = {"what": name, "tflops": best}
-    for kind, name in ((0, "DMMA 4 CTAs x 8 warps / SM"), (2, "DMMA 1 x 4 warps / SM"), (3, "DMMA 2 x 4 warps / SM"),
-                       (4, "DMMA 3 x 4 warps / SM"), (1, "DFMA 4 x 8 warps / SM")):
-        dmrgk.probe_fp64(ctx, kind, 20000, sink, st)
-        best = 0.0
-        for _ in range(3):
-            box = {}
-            ms = timed(st, lambda: box.setdefault("f", dmrgk.probe_fp64(ctx, kind, 200000, sink, st)))
-            best = max(best, box["f"] / ms / 1e9)
-        out[f"pipe_probe_kind{kind}"] = {"what": name, "tflops": best}
-    out["clocks"] = cs.stop()
-    print(json.dumps(out), flush=True)
-
-
 def flat_workload(dim_a, dim_b, n_half=8, seed=11):
     """A lattice-shaped operator-pair list (families F0-F4 of n_half spinless modes per half) over FLAT sectors:
     every A sector has dim_a states, every B sector dim_b — all blocks the same shape, so that the cost of ragged
@@ -992,7 +956,7 @@ def main():
     ap.add_argument("--shard", default="none", choices=["none", "k"],
                     help="N > 1 only: 'none' = independent replicas (the scope of BASELINE.json), 'k' = split the operator-pair "
                          "list over the ranks and all-reduce sigma (SURVEY §8(f) NEXT-2)")
-    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "enlarge", "loop_probe", "ragged", "su2", "expect"],
+    ap.add_argument("--op", default="davidson", choices=["davidson", "renorm", "enlarge", "ragged", "su2", "expect"],
                     help="davidson (default, the headline hot path) or renorm (NEXT-1 row, its own metric)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -1001,8 +965,6 @@ def main():
         run_renorm(args)
     elif args.op == "enlarge":
         run_enlarge(args)
-    elif args.op == "loop_probe":
-        run_loop_probe(args)
     elif args.op == "ragged":
         run_ragged(args)
     elif args.op == "su2":

@@ -395,42 +395,8 @@ int32_t dmrgk_enlarge_query(const dmrgk_enlarge* plan, int64_t* n_tiles, int64_t
                             int64_t* bytes_read, int64_t* bytes_written);
 int32_t dmrgk_enlarge_apply(dmrgk_enlarge* plan, void* stream);
 
-/* ---- harness kernels (outside the hot path): seeded inputs and FP64 pipe probes ----------- */
-/* Counter-based values, bit-identical to workloads/rng.py normal12(seed, stream, index): fills the
- * packed arena of an operator / a ψ layout from the UNPADDED element index of each entry, times
- * scale (scale_mode 0: 1, 1: 1/sqrt(cols of the block)); symmetric != 0: square diagonal-sector
- * blocks get 0.5·(g(r,c)+g(c,r)).  Padding is zero-filled. */
-int32_t dmrgk_op_fill_normal(const dmrgk_op* op, double* arena_dev, uint64_t seed, uint64_t stream_id,
-                             int32_t scale_mode, int32_t symmetric, void* stream);
-int32_t dmrgk_layout_fill_normal(const dmrgk_layout* l, double* arena_dev, uint64_t seed,
-                                 uint64_t stream_id, void* stream);
-/* Φ blocks: normal12 / sqrt(rows of the block) (workloads.fill_phi_host). */
-int32_t dmrgk_iso_fill_normal(const dmrgk_iso* phi, double* arena_dev, uint64_t seed, uint64_t stream_id,
-                              void* stream);
-/* Register-only FP64 pipe probes: every warp of a full grid issues `iters` rounds of 16 independent
- * mma.sync.m8n8k4.f64 (kind 0: 4 CTAs × 8 warps per SM; kinds 2, 3, 4: 1, 2, 3 CTAs × 4 warps per SM)
- * or 32 independent fma.rn.f64 per lane (kind 1).  Returns the flops issued in *flops; the caller
- * times the stream with events. */
-int32_t dmrgk_probe_fp64(dmrgk_ctx* ctx, int32_t kind, int64_t iters, double* sink_dev,
-                         double* flops, void* stream);
-/* Skeletons of the k-tile loop of the grouped GEMM kernel (csrc/probe_gemm.cu): every CTA of a full
- * grid (3 per SM) runs `ktiles` dense k-tiles of 16 with operand tiles streamed from buf_dev (≥ 1 MiB,
- * any finite values).  kind 0: 64×64 tile staged by cp.async from every thread (the round-1 loop);
- * kind 1: 64×64 tile staged by cp.async.bulk from one elected thread with full/empty mbarriers;
- * kind 2: 128×64 tile, otherwise as kind 1; kind 3: 128×64 tile, cp.async from a dedicated producer warp
- * (2 CTAs per SM); kinds 4, 5: kinds 2, 1 at 2 CTAs per SM.  Returns the flops issued in *flops. */
-int32_t dmrgk_probe_gemm_loop(dmrgk_ctx* ctx, int32_t kind, int32_t ktiles, const double* buf_dev,
-                              int64_t buf_doubles, double* sink_dev, double* flops, void* stream);
-
-/* Host only (no device needed): the tile boundaries the task-list builder uses for a block dimension of
- * `extent` rows (tile_max = 64, or 128 for the tall-tile variant) or padded columns (tile_max = 64) — the
- * balanced tiling of DESIGN.md §4.1: ceil(extent/tile_max) tiles, origins at multiples of 16, extents that
- * differ by at most 16, larger tiles first.  Writes n + 1 boundaries (the last one = extent) to `cuts` if
- * cap ≥ n + 1 and returns n; DMRGK_EINVAL (negative) on bad arguments.  For tests of the host logic. */
-int32_t dmrgk_plan_tile_cuts(int32_t extent, int32_t tile_max, int32_t* cuts, int32_t cap);
-/* Host only: the cost per k-tile the planner assigns to a tile of rows × cols computed elements (fragment
- * products of its fullest warp × 4, with the latency floor for thin tiles; a full 64×64 tile costs 64). */
-int32_t dmrgk_plan_tile_cost(int32_t rows, int32_t cols);
+/* The seeded input fills, the FP64 pipe probes and the host-only views of the planner that tests and
+ * bench.py use are declared in dmrgk_harness.h: exported by the same library, not part of the product API. */
 
 #ifdef __cplusplus
 }

@@ -6,6 +6,7 @@
 #include <vector>
 #include <unordered_map>
 #include "../../include/dmrgk.h"
+#include "../../include/dmrgk_harness.h"
 
 namespace dmrgk {
 

@@ -1,4 +1,4 @@
-"""ctypes binding of libdmrgk.so — same names as include/dmrgk.h, argument marshalling only.
+"""ctypes binding of libdmrgk.so — same names as include/dmrgk.h (and include/dmrgk_harness.h), argument marshalling only.
 
 Every step of the hot path runs in the library's CUDA kernels; this module converts Python ints,
 NumPy arrays (host metadata) and device pointers (``torch.Tensor.data_ptr()``) into the C types of
@@ -41,7 +41,7 @@ _p, _i32, _i64, _u64, _f64 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_d
 _pp = C.POINTER(C.c_void_p)
 _pi32, _pi64, _pf64 = C.POINTER(C.c_int32), C.POINTER(C.c_int64), C.POINTER(C.c_double)
 
-# name -> (restype, argtypes); the list of symbols include/dmrgk.h declares.
+# name -> (restype, argtypes); the list of symbols include/dmrgk.h and include/dmrgk_harness.h declare.
 SIGNATURES = {
     "dmrgk_last_error": (C.c_char_p, []),
     "dmrgk_version": (C.c_char_p, []),
@@ -118,7 +118,6 @@ SIGNATURES = {
     "dmrgk_probe_fp64": (_i32, [_p, _i32, _i64, _p, _pf64, _p]),
     "dmrgk_plan_tile_cuts": (_i32, [_i32, _i32, _p, _i32]),
     "dmrgk_plan_tile_cost": (_i32, [_i32, _i32]),
-    "dmrgk_probe_gemm_loop": (_i32, [_p, _i32, _i32, _p, _i64, _p, _pf64, _p]),
 }
 
 _lib = None
@@ -647,13 +646,6 @@ def vec_residual(ctx, n, m, V, W, stride, coef, r, out, scratch, stream=None):
 
 def vec_precond(ctx, n, r, diag, theta_dev, t, stream=None):
     check(ctx.lib.dmrgk_vec_precond(ctx.h, n, _dev(r), _dev(diag), _dev(theta_dev), _dev(t), _stream(stream)))
-
-
-def probe_gemm_loop(ctx, kind, ktiles, buf, sink, stream=None):
-    fl = C.c_double()
-    check(ctx.lib.dmrgk_probe_gemm_loop(ctx.h, kind, ktiles, _dev(buf), buf.numel(), _dev(sink), C.byref(fl),
-                                        _stream(stream)))
-    return fl.value
 
 
 def probe_fp64(ctx, kind, iters, sink, stream=None):

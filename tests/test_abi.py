@@ -8,6 +8,7 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "dmrgk.h")
+HARNESS_HEADER = os.path.join(ROOT, "include", "dmrgk_harness.h")      # test / measurement aids of the same library
 
 
 @pytest.fixture(scope="module")
@@ -18,7 +19,7 @@ def lib():
 
 
 def declared_symbols():
-    src = open(HEADER, encoding="utf-8").read()
+    src = open(HEADER, encoding="utf-8").read() + open(HARNESS_HEADER, encoding="utf-8").read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(dmrgk_[a-z0-9_]+)\s*\(", src)))
 
