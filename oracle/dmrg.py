@@ -165,7 +165,10 @@ def lowest_eigenpair(H):
 class SimpleDMRG:
     """Two-site DMRG on ≤ ~18 modes with everything explicit in Fock space."""
 
-    def __init__(self, T, V, mode_charges, site_modes, target, D, seed):
+    def __init__(self, T, V, mode_charges, site_modes, target, D, seed, sector_hamiltonian=False):
+        """``sector_hamiltonian``: build H inside the target sector from bit-string actions
+        (fock.hamiltonian_sector, pinned against the Kronecker construction) instead of restricting the
+        2^n-dimensional Kronecker matrix — same matrix, needed where a dense V makes the latter too slow."""
         self.T, self.V = T, V
         self.mc = np.asarray(mode_charges, dtype=np.int64).reshape(T.shape[0], -1)
         self.n = T.shape[0]
@@ -174,7 +177,11 @@ class SimpleDMRG:
         self.target = tuple(int(x) for x in target)
         self.D = D
         self.rows = fock.sector_indices(self.n, self.mc, self.target)
-        self.H = fock.restrict(fock.hamiltonian(T, V), self.rows).tocsr()
+        if sector_hamiltonian:
+            rows, self.H = fock.hamiltonian_sector(T, V, self.mc, self.target)
+            assert np.array_equal(rows, self.rows)
+        else:
+            self.H = fock.restrict(fock.hamiltonian(T, V), self.rows).tocsr()
         self.sites = [site_basis(self.mc[m]) for m in site_modes]
         nc = self.mc.shape[1]
         self.L = {0: trivial_basis(nc)}

@@ -154,3 +154,59 @@ def hamiltonian_bits(T, V):
             if s:
                 H[index[new], col] += s * V[i, j, k, l]
     return H
+
+
+# ----------------------------------------------------------------------------
+# Eq. (1) inside one charge sector, for lattices whose 2^n × 2^n matrix with a dense V is out of reach
+# (the mode-rotated 4×4 torus: 16⁴ products of 65536-dimensional sparse matrices).  Built from the
+# bit-string action of operator strings on the sector's basis states — the construction of the pin above,
+# vectorised over states — so it shares nothing with the Kronecker matrices of `annihilators`.
+# ----------------------------------------------------------------------------
+def sector_action(string, n, cols):
+    """The operator string (as in `apply_string_bits`) applied to the basis states ``cols`` (Fock indices):
+    sparse 2^n × len(cols) matrix with entry sign at (index of the new state, position of the old one)."""
+    occ = np.stack([(cols >> (n - 1 - p)) & 1 for p in range(n)], axis=1).astype(np.int64)
+    sign = np.ones(len(cols), dtype=np.int64)
+    for kind, p in reversed(list(string)):
+        want = 1 if kind == "-" else 0
+        sign = np.where(occ[:, p] == want, sign, 0)
+        occ[:, p] = 1 - want
+        odd = occ[:, :p].sum(axis=1) & 1
+        sign = np.where(odd == 1, -sign, sign)
+    new = occ @ (1 << np.arange(n - 1, -1, -1, dtype=np.int64))
+    keep = sign != 0
+    return sp.csr_matrix((sign[keep].astype(np.float64), (new[keep], np.nonzero(keep)[0])), shape=(2 ** n, len(cols)))
+
+
+def hamiltonian_sector(T, V, mode_charges, target):
+    """(rows, H): Eq. (1) (no ½) restricted to the basis states ``rows`` of charge ``target``.
+
+    Σ_ij T_ij c†_i c_j = Σ_ij T_ij (c_i)ᵀ c_j and Σ_ijkl V_ijkl c†_i c†_j c_k c_l = Σ_kl [Σ_ij V_ijkl (c_j c_i)]ᵀ (c_k c_l),
+    with c_j and c_k c_l taken as maps from the sector into the full Fock index range; terms that would leave
+    the sector are absent because Hᵀ-side and H-side intermediate states must coincide."""
+    n = T.shape[0]
+    rows = sector_indices(n, mode_charges, target)
+    a = [sector_action([("-", j)], n, rows) for j in range(n)]
+    H = sp.csr_matrix((len(rows), len(rows)))
+    for i in range(n):
+        M = None
+        for j in range(n):
+            if T[i, j] != 0.0:
+                M = T[i, j] * a[j] if M is None else M + T[i, j] * a[j]
+        if M is not None:
+            H = H + a[i].T @ M
+    pairs = [(k, l) for k in range(n) for l in range(n) if k != l]
+    A = {kl: sector_action([("-", kl[0]), ("-", kl[1])], n, rows).tocoo() for kl in pairs}
+    for (k, l) in pairs:
+        data, r, c = [], [], []
+        for (i, j) in pairs:
+            v = V[i, j, k, l]
+            if v != 0.0:
+                m = A[(j, i)]                    # c†_i c†_j = (c_j c_i)†
+                data.append(v * m.data)
+                r.append(m.row)
+                c.append(m.col)
+        if data:
+            M = sp.csr_matrix((np.concatenate(data), (np.concatenate(r), np.concatenate(c))), shape=(2 ** n, len(rows)))
+            H = H + M.T @ A[(k, l)].tocsr()
+    return rows, H.tocsr()

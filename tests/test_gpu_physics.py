@@ -6,9 +6,9 @@ Kronecker form of the exported blocks (T2); Davidson θ at 1e-9 against `eigh` o
 
 The twins: the 3×3 spinless torus (t-t′-V, 9 modes, rotated, all of F0-F4 dense) and a 2×3 Hubbard
 torus (12 spin-orbitals, two charges (n↑, n↓), same spatial rotation for both spins).
-The rotated 4×4 variant (K = 154) of §8(d) is out of the oracle's reach: its Fock-space builder
-accumulates 16⁴ sparse 65536-dim products (> 50 min on this box), so the 3×3 torus
-carries the dense-basis spinless families instead.
+The rotated 4×4 variant (K = 154) of §8(d) — config 1's own bond with the dense term list — runs through
+`fock.hamiltonian_sector`, the Hamiltonian built inside the N = 8 sector (the 2^16-dimensional Kronecker
+builder would need 16⁴ sparse products).
 """
 import numpy as np
 import pytest
@@ -83,3 +83,38 @@ def test_rotated_twin_sigma_and_energy(make, D, families):
     assert theta >= E_ed - 1e-9                    # variational
     if make is spinless_3x3_rotated and D == 64:
         assert abs(theta - E_ed) <= TOL_ENERGY * max(1.0, abs(E_ed))
+
+
+def test_config1_rotated_twin_K154():
+    """SURVEY §8(d) row 1, second workload: the 4×4 spinless torus of config 1 in a mode-rotated basis, where
+    t and V are dense and the complementary-operator list of the middle bond has the full K = 154 pairs of the
+    formula (2 + 2·8 + 2·8 + 8·7 + 64).  The bases of bond 8|9 are those of config 1's own warm-up sweep
+    (any isometry defines a valid P†HP); H is Eq. (1) with the rotated t, V inside the N = 8 sector.
+    σ at 1e-11 against the definition P†HPψ (T1) and the per-task oracle (T3); Davidson θ at 1e-9 against eigh
+    of P†HP, and not below the exact ground energy of the torus (rotation leaves the spectrum unchanged)."""
+    T, V, mc = lattice.spinless_tV(4)
+    d = dmrg.SimpleDMRG(T, V, mc, [[i] for i in range(16)], (8,), D=64, seed=1)
+    d.warmup_to(7)
+    Tr, Vr = lattice.rotate(T, V, lattice.rotation_matrix(16, seed=7))
+    rows, H = fock.hamiltonian_sector(Tr, Vr, mc, (8,))
+    assert np.array_equal(rows, d.rows)
+    d.T, d.V, d.H = Tr, Vr, H
+    space = d.space_at(7)
+    Heff, P = d.heff_at(space)
+    x = d.guess_at(space, P)
+    pb = export.export_bond(d, space)
+    pb.psi = dmrg.vec_to_blocks(space, x)
+    assert len(pb.terms) == 2 + 2 * 8 + 2 * 8 + 8 * 7 + 64 == 154
+    assert sum(dim for _, dim in space.sectors_A) == 128
+    dp = device_problem(pb)
+    sigma = dp.apply(dp.psi_from_host(pb.psi))
+    got = dp.to_blocks(sigma)
+    assert rel_max(got, dmrg.vec_to_blocks(space, Heff @ x)) <= TOL_SIGMA
+    assert rel_max(got, heff.sigma_blockwise(pb)) <= TOL_SIGMA
+    assert padding_is_zero(dp, sigma)
+    E = np.linalg.eigvalsh(Heff)[0]
+    dav = dp.davidson(m_max=16, tol=1e-9, max_iter=3000)
+    dav.start(dp.psi_from_host(pb.psi))
+    theta, rn, n_apply, ok = dav.solve(None)
+    assert ok and abs(theta - E) <= TOL_ENERGY * max(1.0, abs(E))
+    assert theta >= -8.378565104009 - 1e-9          # tests/golden/ed_energies.txt spinless_4x4_N8; variational
